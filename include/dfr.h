@@ -1,0 +1,163 @@
+/*
+ * dfr.h — C ABI of libdfr: B200-native reprojection hot path of dfreproject
+ *         (arXiv 2505.03932; PAPER.md = /root/reference/PAPER.md).
+ *
+ * What the library computes (PAPER.md:55-69, §3.1; :71-121, §3.2):
+ *   for every pixel (i, j) of a target grid with WCS t and every source
+ *   exposure e with WCS s_e
+ *     1. target pixel -> sky      shift, SIP_A/SIP_B, CD, gnomonic (TAN)
+ *                                  deprojection + rotation
+ *     2. sky -> source pixel      inverse rotation + TAN projection, CD^-1,
+ *                                  SIP_INV_A/SIP_INV_B, shift
+ *     3. interpolate src[e] there nearest / bilinear / bicubic
+ *     4. NaN outside the source footprint
+ *     5. batched over exposures
+ *
+ * Conventions (DESIGN.md lists the readings of the paper they rest on):
+ *   - pixel indices are 0-based, x = column (fastest varying), y = row;
+ *     integer index = pixel centre; CRPIX is FITS 1-based.
+ *   - images are C-contiguous float32 [n][ny][nx].
+ *   - angles in dfr_wcs are DEGREES; CD is degrees per pixel.
+ *   - SIP sign: u <- u + A(u,v) (Shupe 2005); both polynomials
+ *     are evaluated at the pre-update (u,v).
+ *   - footprint: valid <=> -0.5 <= x < nx-0.5 and -0.5 <= y < ny-0.5;
+ *     interpolation taps are edge-replicated; bicubic = Keys, a = -0.75.
+ *
+ * Ownership: the caller owns every buffer named in a signature. The library
+ * allocates only private, stream-ordered scratch and frees it itself. WCS
+ * structs are read during the call and may be freed on return.
+ *
+ * Asynchrony: functions taking DEVICE pointers enqueue work on `stream`
+ * (a cudaStream_t passed as void*, NULL = legacy default stream) and return
+ * after enqueue; results are valid once the caller synchronises the stream.
+ * dfr_reproject_host is synchronous: it returns when `out` is complete.
+ *
+ * Errors: every function returns DFR_OK (0) or a negative dfr_status, never
+ * throws, never aborts; on a validation error nothing is written to outputs.
+ * dfr_last_error() returns thread-local text for the last failure.
+ *
+ * There is no CPU fallback: without a CUDA device every compute entry point
+ * returns DFR_ERR_CUDA.
+ */
+#ifndef DFR_H
+#define DFR_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DFR_SIP_MAX_ORDER 9                     /* SIP convention limit (Shupe 2005) */
+#define DFR_SIP_DIM (DFR_SIP_MAX_ORDER + 1)
+
+/* Packed WCS parameter set. POD, no pointers,
+ * 3280 bytes, no padding. Polynomial coefficient of u^p v^q is stored at
+ * [p*DFR_SIP_DIM + q]; entries with p+q > order are ignored; order 0 means
+ * "polynomial absent". */
+typedef struct dfr_wcs {
+    double  crpix[2];          /* CRPIX1, CRPIX2 — FITS 1-based */
+    double  crval[2];          /* ra0, dec0 in degrees              */
+    double  cd[4];             /* CD1_1, CD1_2, CD2_1, CD2_2, deg/pixel */
+    int32_t a_order, b_order, ap_order, bp_order;
+    double  a [DFR_SIP_DIM * DFR_SIP_DIM];     /* SIP_A   */
+    double  b [DFR_SIP_DIM * DFR_SIP_DIM];     /* SIP_B                          */
+    double  ap[DFR_SIP_DIM * DFR_SIP_DIM];     /* SIP_INV_A      */
+    double  bp[DFR_SIP_DIM * DFR_SIP_DIM];     /* SIP_INV_B      */
+} dfr_wcs;
+
+/* Interpolation order (PAPER.md:35 `order=`, :135 "three interpolation schemes"). */
+enum { DFR_NEAREST = 0, DFR_BILINEAR = 1, DFR_BICUBIC = 3 };
+
+typedef enum dfr_status {
+    DFR_OK = 0,
+    DFR_ERR_NULL = -1,           /* a required pointer is NULL                    */
+    DFR_ERR_SHAPE = -2,          /* n < 1, a dimension < 1, or ny*nx >= 2^31      */
+    DFR_ERR_ORDER = -3,          /* order not in {0, 1, 3}                        */
+    DFR_ERR_SIP_ORDER = -4,      /* a SIP order outside [0, DFR_SIP_MAX_ORDER]    */
+    DFR_ERR_SINGULAR_CD = -5,    /* det(CD) == 0 or not finite                    */
+    DFR_ERR_NONFINITE_WCS = -6,  /* NaN/Inf in crpix, crval, cd or used SIP terms */
+    DFR_ERR_ALIAS = -7,          /* out overlaps src_batch                        */
+    DFR_ERR_CUDA = -8            /* CUDA runtime/driver failure (see dfr_last_error) */
+} dfr_status;
+
+/* Path selection for dfr_reproject_ex / dfr_src_coords_ex.
+ *   AUTO  : tiled fast path where its verified error bound holds, exact
+ *           per-pixel path elsewhere (what dfr_reproject uses).
+ *   EXACT : every pixel through the per-pixel fp64 map, direct gathers.
+ *   TILED : as AUTO (kept distinct so tests can assert the fast path ran). */
+enum { DFR_PATH_AUTO = 0, DFR_PATH_EXACT = 1, DFR_PATH_TILED = 2 };
+
+/* ---- the hot path (calculate_reprojection) -------------- */
+
+/* Reproject n source exposures onto one target grid.
+ *   src_batch : DEVICE float32 [n][src_ny][src_nx], contiguous
+ *   src_wcs   : HOST, n entries (exposure e uses src_wcs[e])
+ *   tgt_wcs   : HOST, 1 entry
+ *   out_ny/nx : shape_out
+ *   order     : DFR_NEAREST | DFR_BILINEAR | DFR_BICUBIC
+ *   out       : DEVICE float32 [n][out_ny][out_nx]; every element is written
+ *               (value, or NaN outside the footprint of exposure e)
+ * Steps a1–a10 of SURVEY.md §8(a) all run inside the library's kernels. */
+int dfr_reproject(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+                  const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                  int32_t out_ny, int32_t out_nx, int32_t order,
+                  float *out, void *stream);
+
+/* Same, with an explicit path (DFR_PATH_*). */
+int dfr_reproject_ex(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+                     const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                     int32_t out_ny, int32_t out_nx, int32_t order,
+                     float *out, void *stream, int32_t path);
+
+/* End-to-end form with HOST buffers (">1000 exposures"; SURVEY.md
+ * §8(a) a10): src_host [n][src_ny][src_nx] and out_host [n][out_ny][out_nx]
+ * are HOST float32 arrays (pinned memory gives full PCIe rate, pageable
+ * works). Exposures are processed in batches of `batch` (<=0 selects 32); the
+ * upload of batch k+1 and the download of batch k-1 overlap the kernels of
+ * batch k on private CUDA streams. Synchronous. */
+int dfr_reproject_host(const float *src_host, int32_t n, int32_t src_ny, int32_t src_nx,
+                       const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                       int32_t out_ny, int32_t out_nx, int32_t order,
+                       float *out_host, int32_t batch);
+
+/* ---- coordinate entry points, for testing (§3.2.1 / §3.2.2) ---- */
+
+/* Pixel -> sky with WCS *w (HOST). x, y, ra_deg, dec_deg: DEVICE double[npts].
+ * Literal formulas of PAPER.md:87-95 in fp64. RA is reduced to [0,360),
+ * Dec is in [-90,90]. */
+int dfr_pix2world(const dfr_wcs *w, const double *x, const double *y, int64_t npts,
+                  double *ra_deg, double *dec_deg, void *stream);
+
+/* Sky -> pixel with WCS *w (HOST). Literal formulas of PAPER.md:101-121 in
+ * fp64; uses AP/BP only (no iterative inverse; absent AP/BP => no inverse
+ * distortion). Points >= 90 degrees from CRVAL give NaN. */
+int dfr_world2pix(const dfr_wcs *w, const double *ra_deg, const double *dec_deg, int64_t npts,
+                  double *x, double *y, void *stream);
+
+/* Test-only: the source coordinates dfr_reproject itself uses (same device
+ * functions, same tile tables), DEVICE double [n][out_ny][out_nx] each.
+ * src_ny/src_nx are needed because the fast path's tiling depends on them. */
+int dfr_src_coords(int32_t n, int32_t src_ny, int32_t src_nx,
+                   const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                   int32_t out_ny, int32_t out_nx, int32_t order,
+                   double *x, double *y, void *stream, int32_t path);
+
+/* ---- helpers ----------------------------------------------------------- */
+
+/* CD_ij = CDELT_i * PC_ij (FITS Paper I). HOST only. */
+int dfr_wcs_set_pc_cdelt(dfr_wcs *w, const double pc[4], const double cdelt[2]);
+
+/* Counters of the last dfr_reproject / dfr_reproject_ex call on this thread (HOST):
+ * stats[0] = tiles on the fast path, [1] = tiles on the exact path,
+ * [2] = tiles entirely outside the footprint, [3] = kernels launched. */
+int dfr_last_stats(int64_t stats[4]);
+
+const char *dfr_strerror(int code);
+const char *dfr_last_error(void);
+int dfr_version(void);           /* 10000*major + 100*minor + patch */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DFR_H */
