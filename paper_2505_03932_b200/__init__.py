@@ -1,0 +1,231 @@
+"""paper_2505_03932_b200 — thin Python binding of libdfr (include/dfr.h).
+
+Argument marshalling only: every step of the reprojection path runs in the
+library's CUDA kernels. torch is used for device memory and streams. There is
+no CPU fallback: if libdfr.so is missing or CUDA is unavailable the calls raise.
+This package never imports `oracle`.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_PKG, "libdfr.so")
+
+NEAREST, BILINEAR, BICUBIC = 0, 1, 3
+PATH_AUTO, PATH_EXACT, PATH_TILED = 0, 1, 2
+_ORDER_NAMES = {"nearest": 0, "nearest-neighbor": 0, "bilinear": 1, "bicubic": 3}
+
+EXPORTS = ["dfr_reproject", "dfr_reproject_ex", "dfr_reproject_host", "dfr_pix2world",
+           "dfr_world2pix", "dfr_src_coords", "dfr_wcs_set_pc_cdelt", "dfr_last_stats",
+           "dfr_strerror", "dfr_last_error", "dfr_version"]
+
+
+class DfrWCS(C.Structure):
+    """Mirror of `dfr_wcs` in include/dfr.h (3280 bytes)."""
+    _fields_ = [("crpix", C.c_double * 2), ("crval", C.c_double * 2), ("cd", C.c_double * 4),
+                ("a_order", C.c_int32), ("b_order", C.c_int32),
+                ("ap_order", C.c_int32), ("bp_order", C.c_int32),
+                ("a", C.c_double * 100), ("b", C.c_double * 100),
+                ("ap", C.c_double * 100), ("bp", C.c_double * 100)]
+
+
+class DfrError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__(f"libdfr error {code}: {text}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load libdfr.so (in-tree). Raises if it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            raise ImportError(f"{_SO} missing: run `python -m paper_2505_03932_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(_SO)
+        fp, dp, wp, vp = C.c_void_p, C.c_void_p, C.POINTER(DfrWCS), C.c_void_p
+        i32, i64 = C.c_int32, C.c_int64
+        L.dfr_reproject.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, vp]
+        L.dfr_reproject_ex.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, vp, i32]
+        L.dfr_reproject_host.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, i32]
+        L.dfr_pix2world.argtypes = [wp, dp, dp, i64, dp, dp, vp]
+        L.dfr_world2pix.argtypes = [wp, dp, dp, i64, dp, dp, vp]
+        L.dfr_src_coords.argtypes = [i32, i32, i32, wp, wp, i32, i32, i32, dp, dp, vp, i32]
+        L.dfr_wcs_set_pc_cdelt.argtypes = [wp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.dfr_last_stats.argtypes = [C.POINTER(C.c_int64)]
+        L.dfr_strerror.argtypes = [C.c_int]
+        L.dfr_strerror.restype = C.c_char_p
+        L.dfr_last_error.restype = C.c_char_p
+        L.dfr_version.restype = C.c_int
+        for name in EXPORTS:
+            getattr(L, name)
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        L = lib()
+        raise DfrError(rc, (L.dfr_last_error() or L.dfr_strerror(rc)).decode())
+
+
+def pack_wcs(w) -> DfrWCS:
+    """Pack any object with the WCS attribute names (e.g. dfr_synth.WCS)."""
+    if isinstance(w, DfrWCS):
+        return w
+    s = DfrWCS()
+    s.crpix[:] = [float(v) for v in w.crpix]
+    s.crval[:] = [float(v) for v in w.crval]
+    s.cd[:] = [float(v) for v in w.cd]
+    s.a_order, s.b_order = int(w.a_order), int(w.b_order)
+    s.ap_order, s.bp_order = int(w.ap_order), int(w.bp_order)
+    for name in ("a", "b", "ap", "bp"):
+        arr = np.ascontiguousarray(getattr(w, name), dtype=np.float64).reshape(-1)
+        if arr.size != 100:
+            raise ValueError(f"{name} must have 10x10 entries")
+        getattr(s, name)[:] = arr.tolist()
+    return s
+
+
+def pack_wcs_array(ws):
+    if isinstance(ws, C.Array):
+        return ws
+    ws = list(ws)
+    return (DfrWCS * len(ws))(*[pack_wcs(w) for w in ws])
+
+
+def _order(order) -> int:
+    if isinstance(order, str):
+        return _ORDER_NAMES[order]
+    return int(order)
+
+
+def _stream_ptr(stream):
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+def _need_cuda(t, dtype, name):
+    if not (t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise ValueError(f"{name} must be a contiguous CUDA tensor of {dtype}")
+
+
+def dfr_reproject(src_batch, src_wcs, tgt_wcs, shape_out=None, order=BILINEAR, out=None,
+                  stream=None, path=PATH_AUTO):
+    """dfr_reproject / dfr_reproject_ex (include/dfr.h). src_batch: CUDA float32
+    [n][ny][nx] (or [ny][nx]); returns the CUDA float32 [n][out_ny][out_nx] output.
+    shape_out defaults to the input shape."""
+    import torch
+    if src_batch.dim() == 2:
+        src_batch = src_batch[None]
+    _need_cuda(src_batch, torch.float32, "src_batch")
+    n, sny, snx = src_batch.shape
+    ony, onx = (sny, snx) if shape_out is None else (int(shape_out[0]), int(shape_out[1]))
+    ws = pack_wcs_array(src_wcs)
+    if len(ws) != n:
+        raise ValueError("one source WCS per exposure")
+    tw = pack_wcs(tgt_wcs)
+    if out is None:
+        out = torch.empty((n, ony, onx), dtype=torch.float32, device=src_batch.device)
+    _need_cuda(out, torch.float32, "out")
+    if tuple(out.shape) != (n, ony, onx):
+        raise ValueError("out has the wrong shape")
+    with torch.cuda.device(src_batch.device):
+        _check(lib().dfr_reproject_ex(src_batch.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx,
+                                      _order(order), out.data_ptr(), _stream_ptr(stream), int(path)))
+    return out
+
+
+def dfr_reproject_host(src_host, src_wcs, tgt_wcs, shape_out=None, order=BILINEAR, out_host=None,
+                       batch=32):
+    """dfr_reproject_host: HOST float32 arrays (numpy, or CPU torch tensors — pinned
+    for full PCIe rate) in and out; copies and kernels are pipelined inside the library."""
+    import torch
+    src_t = torch.as_tensor(src_host)
+    if src_t.dim() == 2:
+        src_t = src_t[None]
+    if src_t.is_cuda or src_t.dtype != torch.float32 or not src_t.is_contiguous():
+        raise ValueError("src_host must be a contiguous float32 host array")
+    n, sny, snx = src_t.shape
+    ony, onx = (sny, snx) if shape_out is None else (int(shape_out[0]), int(shape_out[1]))
+    ws = pack_wcs_array(src_wcs)
+    tw = pack_wcs(tgt_wcs)
+    if out_host is None:
+        out_host = torch.empty((n, ony, onx), dtype=torch.float32, pin_memory=True)
+    out_t = torch.as_tensor(out_host)
+    if out_t.is_cuda or out_t.dtype != torch.float32 or not out_t.is_contiguous() \
+            or tuple(out_t.shape) != (n, ony, onx):
+        raise ValueError("out_host must be a contiguous float32 host array [n][ny][nx]")
+    _check(lib().dfr_reproject_host(src_t.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx,
+                                    _order(order), out_t.data_ptr(), int(batch)))
+    return out_host
+
+
+def dfr_pix2world(wcs, x, y, stream=None):
+    """dfr_pix2world: x, y CUDA float64 tensors -> (ra_deg, dec_deg) CUDA float64."""
+    import torch
+    _need_cuda(x, torch.float64, "x")
+    _need_cuda(y, torch.float64, "y")
+    ra, dec = torch.empty_like(x), torch.empty_like(x)
+    w = pack_wcs(wcs)
+    with torch.cuda.device(x.device):
+        _check(lib().dfr_pix2world(C.byref(w), x.data_ptr(), y.data_ptr(), x.numel(),
+                                   ra.data_ptr(), dec.data_ptr(), _stream_ptr(stream)))
+    return ra, dec
+
+
+def dfr_world2pix(wcs, ra_deg, dec_deg, stream=None):
+    """dfr_world2pix: (ra, dec) CUDA float64 degrees -> (x, y) CUDA float64."""
+    import torch
+    _need_cuda(ra_deg, torch.float64, "ra_deg")
+    _need_cuda(dec_deg, torch.float64, "dec_deg")
+    x, y = torch.empty_like(ra_deg), torch.empty_like(ra_deg)
+    w = pack_wcs(wcs)
+    with torch.cuda.device(ra_deg.device):
+        _check(lib().dfr_world2pix(C.byref(w), ra_deg.data_ptr(), dec_deg.data_ptr(), ra_deg.numel(),
+                                   x.data_ptr(), y.data_ptr(), _stream_ptr(stream)))
+    return x, y
+
+
+def dfr_src_coords(src_wcs, tgt_wcs, src_shape, shape_out, order=BILINEAR, path=PATH_AUTO,
+                   device="cuda", stream=None):
+    """dfr_src_coords (test-only): the source coordinates the reprojection kernels
+    use, CUDA float64 [n][out_ny][out_nx] each."""
+    import torch
+    ws = pack_wcs_array(src_wcs)
+    tw = pack_wcs(tgt_wcs)
+    n = len(ws)
+    ony, onx = int(shape_out[0]), int(shape_out[1])
+    x = torch.empty((n, ony, onx), dtype=torch.float64, device=device)
+    y = torch.empty_like(x)
+    with torch.cuda.device(x.device):
+        _check(lib().dfr_src_coords(n, int(src_shape[0]), int(src_shape[1]), ws, C.byref(tw),
+                                    ony, onx, _order(order), x.data_ptr(), y.data_ptr(),
+                                    _stream_ptr(stream), int(path)))
+    return x, y
+
+
+def dfr_wcs_set_pc_cdelt(wcs: DfrWCS, pc, cdelt):
+    pc_a = (C.c_double * 4)(*[float(v) for v in pc])
+    cd_a = (C.c_double * 2)(*[float(v) for v in cdelt])
+    _check(lib().dfr_wcs_set_pc_cdelt(C.byref(wcs), pc_a, cd_a))
+    return wcs
+
+
+def dfr_last_stats():
+    arr = (C.c_int64 * 4)()
+    _check(lib().dfr_last_stats(arr))
+    return {"tiles_fast": arr[0], "tiles_exact": arr[1], "tiles_empty": arr[2], "kernels": arr[3]}
+
+
+def dfr_version() -> int:
+    return int(lib().dfr_version())

@@ -1,0 +1,319 @@
+// dfr_api.cu — the C ABI of include/dfr.h: argument validation, host
+// pre-composition, stream-ordered scratch, kernel launches. No compute happens
+// on the host beyond the O(n) per-exposure constant folding of dfr_host.cu.
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <vector>
+
+#include "dfr_internal.h"
+#include "dfr_tiled.h"
+
+namespace dfr {
+const char *last_error_cstr();
+
+static thread_local int64_t g_stats[4] = {0, 0, 0, 0};
+
+static std::once_flag g_pool_once;
+static void tune_pool()
+{
+    // keep stream-ordered scratch cached between calls (no OS round trip per call)
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return;
+    cudaMemPool_t pool;
+    if (cudaDeviceGetDefaultMemPool(&pool, dev) != cudaSuccess) return;
+    uint64_t thr = UINT64_MAX;
+    cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+}
+
+static int check_common(int32_t n, int32_t sny, int32_t snx, const dfr_wcs *sw, const dfr_wcs *tw,
+                        int32_t ony, int32_t onx, int32_t order)
+{
+    if (!sw || !tw) { set_error("NULL WCS pointer"); return DFR_ERR_NULL; }
+    if (n < 1 || sny < 1 || snx < 1 || ony < 1 || onx < 1 ||
+        (int64_t)sny * snx >= (1LL << 31) || (int64_t)ony * onx >= (1LL << 31)) {
+        set_error("bad shape: n=%d src=%dx%d out=%dx%d", n, sny, snx, ony, onx);
+        return DFR_ERR_SHAPE;
+    }
+    if (order != DFR_NEAREST && order != DFR_BILINEAR && order != DFR_BICUBIC) {
+        set_error("order %d not in {0, 1, 3}", order);
+        return DFR_ERR_ORDER;
+    }
+    int rc = validate_wcs(tw);
+    if (rc != DFR_OK) return rc;
+    for (int32_t e = 0; e < n; ++e) {
+        rc = validate_wcs(&sw[e]);
+        if (rc != DFR_OK) return rc;
+    }
+    return DFR_OK;
+}
+
+// Host constants -> device scratch (stream-ordered). Caller frees with cudaFreeAsync.
+static int upload_sources(int32_t n, const dfr_wcs *sw, const dfr_wcs *tw, cudaStream_t st,
+                          SourceDev **dev_out)
+{
+    std::vector<SourceDev> h((size_t)n);
+    for (int32_t e = 0; e < n; ++e) make_source(tw, &sw[e], &h[e]);
+    SourceDev *d = nullptr;
+    cudaError_t err = cudaMallocAsync((void **)&d, sizeof(SourceDev) * (size_t)n, st);
+    if (err != cudaSuccess) return cuda_fail(err, "cudaMallocAsync(sources)");
+    // pageable source: the runtime stages the bytes before returning, so `h` may die
+    err = cudaMemcpyAsync(d, h.data(), sizeof(SourceDev) * (size_t)n, cudaMemcpyHostToDevice, st);
+    if (err != cudaSuccess) { cudaFreeAsync(d, st); return cuda_fail(err, "cudaMemcpyAsync(sources)"); }
+    *dev_out = d;
+    return DFR_OK;
+}
+
+static int reproject_impl(const float *src, int32_t n, int32_t sny, int32_t snx,
+                          const dfr_wcs *sw, const dfr_wcs *tw, int32_t ony, int32_t onx,
+                          int32_t order, float *out, cudaStream_t st, int32_t path)
+{
+    std::call_once(g_pool_once, tune_pool);
+    TargetDev tgt;
+    make_target(tw, &tgt);
+    SourceDev *dsrc = nullptr;
+    int rc = upload_sources(n, sw, tw, st, &dsrc);
+    if (rc != DFR_OK) return rc;
+    cudaError_t err;
+    TiledStats ts = {0, 0, 0, 0};
+    if (path == DFR_PATH_EXACT) {
+        err = launch_exact_reproject(src, n, sny, snx, tgt, dsrc, ony, onx, order, out, st);
+        ts.kernels = 1;
+        ts.tiles_exact = -1;
+    } else {
+        err = launch_tiled_reproject(src, n, sny, snx, tgt, dsrc, ony, onx, order, out, st, &ts);
+    }
+    cudaFreeAsync(dsrc, st);
+    g_stats[0] = ts.tiles_fast;
+    g_stats[1] = ts.tiles_exact;
+    g_stats[2] = ts.tiles_empty;
+    g_stats[3] = ts.kernels;
+    if (err != cudaSuccess) return cuda_fail(err, "reproject launch");
+    return DFR_OK;
+}
+
+}  // namespace dfr
+
+using namespace dfr;
+
+extern "C" {
+
+int dfr_reproject_ex(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+                     const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                     int32_t out_ny, int32_t out_nx, int32_t order,
+                     float *out, void *stream, int32_t path)
+{
+    if (!src_batch || !out) { set_error("NULL image pointer"); return DFR_ERR_NULL; }
+    int rc = check_common(n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order);
+    if (rc != DFR_OK) return rc;
+    if (path != DFR_PATH_AUTO && path != DFR_PATH_EXACT && path != DFR_PATH_TILED) {
+        set_error("unknown path %d", path);
+        return DFR_ERR_ORDER;
+    }
+    const char *s0 = (const char *)src_batch, *s1 = s0 + sizeof(float) * (size_t)n * src_ny * src_nx;
+    const char *o0 = (const char *)out, *o1 = o0 + sizeof(float) * (size_t)n * out_ny * out_nx;
+    if (o0 < s1 && s0 < o1) { set_error("out overlaps src_batch"); return DFR_ERR_ALIAS; }
+    return reproject_impl(src_batch, n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order,
+                          out, (cudaStream_t)stream, path);
+}
+
+int dfr_reproject(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+                  const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                  int32_t out_ny, int32_t out_nx, int32_t order, float *out, void *stream)
+{
+    return dfr_reproject_ex(src_batch, n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order,
+                            out, stream, DFR_PATH_AUTO);
+}
+
+int dfr_src_coords(int32_t n, int32_t src_ny, int32_t src_nx,
+                   const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                   int32_t out_ny, int32_t out_nx, int32_t order,
+                   double *x, double *y, void *stream, int32_t path)
+{
+    if (!x || !y) { set_error("NULL coordinate pointer"); return DFR_ERR_NULL; }
+    int rc = check_common(n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order);
+    if (rc != DFR_OK) return rc;
+    std::call_once(g_pool_once, tune_pool);
+    cudaStream_t st = (cudaStream_t)stream;
+    TargetDev tgt;
+    make_target(tgt_wcs, &tgt);
+    SourceDev *dsrc = nullptr;
+    rc = upload_sources(n, src_wcs, tgt_wcs, st, &dsrc);
+    if (rc != DFR_OK) return rc;
+    cudaError_t err;
+    if (path == DFR_PATH_EXACT)
+        err = launch_exact_coords(n, tgt, dsrc, out_ny, out_nx, x, y, st);
+    else
+        err = launch_tiled_coords(n, src_ny, src_nx, tgt, dsrc, out_ny, out_nx, order, x, y, st);
+    cudaFreeAsync(dsrc, st);
+    if (err != cudaSuccess) return cuda_fail(err, "src_coords launch");
+    return DFR_OK;
+}
+
+static int sky_common(const dfr_wcs *w, const void *a, const void *b, const void *c, const void *d,
+                      int64_t npts, cudaStream_t st, SkyDev **dev)
+{
+    if (npts < 0) { set_error("npts < 0"); return DFR_ERR_SHAPE; }
+    if (!w || (npts > 0 && (!a || !b || !c || !d))) { set_error("NULL pointer"); return DFR_ERR_NULL; }
+    int rc = validate_wcs(w);
+    if (rc != DFR_OK) return rc;
+    std::call_once(g_pool_once, tune_pool);
+    SkyDev h;
+    make_sky(w, &h);
+    cudaError_t err = cudaMallocAsync((void **)dev, sizeof(SkyDev), st);
+    if (err != cudaSuccess) return cuda_fail(err, "cudaMallocAsync(sky)");
+    err = cudaMemcpyAsync(*dev, &h, sizeof h, cudaMemcpyHostToDevice, st);
+    if (err != cudaSuccess) { cudaFreeAsync(*dev, st); return cuda_fail(err, "cudaMemcpyAsync(sky)"); }
+    return DFR_OK;
+}
+
+int dfr_pix2world(const dfr_wcs *w, const double *x, const double *y, int64_t npts,
+                  double *ra_deg, double *dec_deg, void *stream)
+{
+    cudaStream_t st = (cudaStream_t)stream;
+    SkyDev *d = nullptr;
+    int rc = sky_common(w, x, y, ra_deg, dec_deg, npts, st, &d);
+    if (rc != DFR_OK) return rc;
+    cudaError_t err = launch_pix2world(d, x, y, npts, ra_deg, dec_deg, st);
+    cudaFreeAsync(d, st);
+    return err == cudaSuccess ? DFR_OK : cuda_fail(err, "pix2world launch");
+}
+
+int dfr_world2pix(const dfr_wcs *w, const double *ra_deg, const double *dec_deg, int64_t npts,
+                  double *x, double *y, void *stream)
+{
+    cudaStream_t st = (cudaStream_t)stream;
+    SkyDev *d = nullptr;
+    int rc = sky_common(w, ra_deg, dec_deg, x, y, npts, st, &d);
+    if (rc != DFR_OK) return rc;
+    cudaError_t err = launch_world2pix(d, ra_deg, dec_deg, npts, x, y, st);
+    cudaFreeAsync(d, st);
+    return err == cudaSuccess ? DFR_OK : cuda_fail(err, "world2pix launch");
+}
+
+// ---- end-to-end streaming form ------------------------
+namespace {
+struct Slot {
+    cudaStream_t st = nullptr;
+    float *din = nullptr, *dout = nullptr;
+    size_t in_bytes = 0, out_bytes = 0;
+};
+constexpr int kSlots = 3;
+struct HostPipe {
+    std::mutex mu;
+    int dev = -1;
+    Slot slot[kSlots];
+} g_pipe;
+
+static cudaError_t ensure_slot(Slot &s, size_t in_bytes, size_t out_bytes)
+{
+    cudaError_t err;
+    if (!s.st && (err = cudaStreamCreateWithFlags(&s.st, cudaStreamNonBlocking)) != cudaSuccess) return err;
+    if (s.in_bytes < in_bytes) {
+        if (s.din) cudaFree(s.din);
+        s.din = nullptr; s.in_bytes = 0;
+        if ((err = cudaMalloc((void **)&s.din, in_bytes)) != cudaSuccess) return err;
+        s.in_bytes = in_bytes;
+    }
+    if (s.out_bytes < out_bytes) {
+        if (s.dout) cudaFree(s.dout);
+        s.dout = nullptr; s.out_bytes = 0;
+        if ((err = cudaMalloc((void **)&s.dout, out_bytes)) != cudaSuccess) return err;
+        s.out_bytes = out_bytes;
+    }
+    return cudaSuccess;
+}
+}  // namespace
+
+int dfr_reproject_host(const float *src_host, int32_t n, int32_t src_ny, int32_t src_nx,
+                       const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                       int32_t out_ny, int32_t out_nx, int32_t order,
+                       float *out_host, int32_t batch)
+{
+    if (!src_host || !out_host) { set_error("NULL image pointer"); return DFR_ERR_NULL; }
+    int rc = check_common(n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order);
+    if (rc != DFR_OK) return rc;
+    if (batch <= 0) batch = 32;
+    if (batch > n) batch = n;
+    const size_t in_px = (size_t)src_ny * src_nx, out_px = (size_t)out_ny * out_nx;
+    std::lock_guard<std::mutex> lock(g_pipe.mu);
+    int dev = 0;
+    cudaError_t err = cudaGetDevice(&dev);
+    if (err != cudaSuccess) return cuda_fail(err, "cudaGetDevice");
+    if (g_pipe.dev != dev) {                       // buffers belong to one device
+        for (Slot &s : g_pipe.slot) {
+            if (s.din) cudaFree(s.din);
+            if (s.dout) cudaFree(s.dout);
+            if (s.st) cudaStreamDestroy(s.st);
+            s = Slot();
+        }
+        g_pipe.dev = dev;
+    }
+    const int nb = (n + batch - 1) / batch;
+    const int used = nb < kSlots ? nb : kSlots;
+    for (int k = 0; k < used; ++k) {
+        err = ensure_slot(g_pipe.slot[k], in_px * batch * sizeof(float), out_px * batch * sizeof(float));
+        if (err != cudaSuccess) return cuda_fail(err, "pipeline buffers");
+    }
+    int64_t tot[4] = {0, 0, 0, 0};
+    for (int b = 0; b < nb; ++b) {
+        Slot &s = g_pipe.slot[b % kSlots];
+        const int32_t e0 = b * batch, ne = (n - e0 < batch) ? n - e0 : batch;
+        // slot reuse is ordered by the slot's own stream: H2D(b) waits for D2H(b - kSlots)
+        err = cudaMemcpyAsync(s.din, src_host + in_px * e0, in_px * ne * sizeof(float),
+                              cudaMemcpyHostToDevice, s.st);
+        if (err != cudaSuccess) { rc = cuda_fail(err, "H2D"); break; }
+        rc = reproject_impl(s.din, ne, src_ny, src_nx, src_wcs + e0, tgt_wcs, out_ny, out_nx, order,
+                            s.dout, s.st, DFR_PATH_AUTO);
+        if (rc != DFR_OK) break;
+        for (int k = 0; k < 4; ++k) tot[k] += g_stats[k];
+        err = cudaMemcpyAsync(out_host + out_px * e0, s.dout, out_px * ne * sizeof(float),
+                              cudaMemcpyDeviceToHost, s.st);
+        if (err != cudaSuccess) { rc = cuda_fail(err, "D2H"); break; }
+    }
+    for (int k = 0; k < used; ++k) {
+        err = cudaStreamSynchronize(g_pipe.slot[k].st);
+        if (err != cudaSuccess && rc == DFR_OK) rc = cuda_fail(err, "pipeline sync");
+    }
+    for (int k = 0; k < 4; ++k) g_stats[k] = tot[k];
+    return rc;
+}
+
+int dfr_wcs_set_pc_cdelt(dfr_wcs *w, const double pc[4], const double cdelt[2])
+{
+    if (!w || !pc || !cdelt) { set_error("NULL pointer"); return DFR_ERR_NULL; }
+    w->cd[0] = cdelt[0] * pc[0];
+    w->cd[1] = cdelt[0] * pc[1];
+    w->cd[2] = cdelt[1] * pc[2];
+    w->cd[3] = cdelt[1] * pc[3];
+    return DFR_OK;
+}
+
+int dfr_last_stats(int64_t stats[4])
+{
+    if (!stats) return DFR_ERR_NULL;
+    for (int k = 0; k < 4; ++k) stats[k] = g_stats[k];
+    return DFR_OK;
+}
+
+const char *dfr_strerror(int code)
+{
+    switch (code) {
+    case DFR_OK: return "ok";
+    case DFR_ERR_NULL: return "null pointer";
+    case DFR_ERR_SHAPE: return "bad shape";
+    case DFR_ERR_ORDER: return "bad interpolation order or path";
+    case DFR_ERR_SIP_ORDER: return "SIP order out of range";
+    case DFR_ERR_SINGULAR_CD: return "singular CD matrix";
+    case DFR_ERR_NONFINITE_WCS: return "non-finite WCS field";
+    case DFR_ERR_ALIAS: return "output aliases input";
+    case DFR_ERR_CUDA: return "CUDA failure";
+    default: return "unknown error";
+    }
+}
+
+const char *dfr_last_error(void) { return dfr::last_error_cstr(); }
+
+int dfr_version(void) { return 100; }
+
+}  // extern "C"

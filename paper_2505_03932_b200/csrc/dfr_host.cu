@@ -1,0 +1,165 @@
+// dfr_host.cu — host-side WCS validation and fp64 pre-composition (no kernels).
+//
+// The per-pixel spherical trigonometry of PAPER.md:91-95 and :101-111 is
+// algebraically a fixed projective map between the two tangent planes
+// (DESIGN.md §6): with the orthonormal triad at a tangent point (ra, dec)
+//   e = (-sin ra, cos ra, 0)             east
+//   n = (-sin dec cos ra, -sin dec sin ra, cos dec)   north
+//   k = ( cos dec cos ra,  cos dec sin ra, sin dec)   towards the tangent point
+// a target-plane point (xi, eta) [radians] is the direction p = k_t + xi e_t + eta n_t
+// and its source-plane coordinates are xi_s = (p.e_s)/(p.k_s), eta_s = (p.n_s)/(p.k_s);
+// p.k_s <= 0 <=> the paper's sin(theta) <= 0. Everything that
+// depends only on the (target, exposure) pair is folded here, once, in double.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+
+#include "dfr_internal.h"
+
+namespace dfr {
+
+static thread_local std::string g_err;
+
+void set_error(const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+}
+
+const char *last_error_cstr() { return g_err.c_str(); }
+
+int cuda_fail(cudaError_t e, const char *what)
+{
+    set_error("%s: %s (%s)", what, cudaGetErrorName(e), cudaGetErrorString(e));
+    return DFR_ERR_CUDA;
+}
+
+static bool poly_finite(const double *c, int order)
+{
+    for (int p = 0; p <= order; ++p)
+        for (int q = 0; p + q <= order; ++q)
+            if (!std::isfinite(c[p * DFR_SIP_DIM + q])) return false;
+    return true;
+}
+
+int validate_wcs(const dfr_wcs *w)
+{
+    const int32_t ords[4] = {w->a_order, w->b_order, w->ap_order, w->bp_order};
+    for (int k = 0; k < 4; ++k)
+        if (ords[k] < 0 || ords[k] > DFR_SIP_MAX_ORDER) {
+            set_error("SIP order %d outside [0, %d]", ords[k], DFR_SIP_MAX_ORDER);
+            return DFR_ERR_SIP_ORDER;
+        }
+    for (int k = 0; k < 2; ++k)
+        if (!std::isfinite(w->crpix[k]) || !std::isfinite(w->crval[k])) {
+            set_error("non-finite CRPIX/CRVAL");
+            return DFR_ERR_NONFINITE_WCS;
+        }
+    for (int k = 0; k < 4; ++k)
+        if (!std::isfinite(w->cd[k])) {
+            set_error("non-finite CD");
+            return DFR_ERR_NONFINITE_WCS;
+        }
+    if (!poly_finite(w->a, w->a_order) || !poly_finite(w->b, w->b_order) ||
+        !poly_finite(w->ap, w->ap_order) || !poly_finite(w->bp, w->bp_order)) {
+        set_error("non-finite SIP coefficient");
+        return DFR_ERR_NONFINITE_WCS;
+    }
+    const double det = w->cd[0] * w->cd[3] - w->cd[1] * w->cd[2];
+    if (!(std::fabs(det) > 0.0) || !std::isfinite(det)) {
+        set_error("singular CD matrix (det = %g)", det);
+        return DFR_ERR_SINGULAR_CD;
+    }
+    return DFR_OK;
+}
+
+void pack_poly(const double *c, int order, Poly *out)
+{
+    std::memset(out, 0, sizeof *out);
+    out->order = order;
+    if (order <= 0) { out->order = 0; return; }
+    int k = 0;
+    for (int p = 0; p <= order; ++p)
+        for (int q = 0; p + q <= order; ++q) out->c[k++] = c[p * DFR_SIP_DIM + q];
+}
+
+void make_target(const dfr_wcs *t, TargetDev *out)
+{
+    out->c1 = t->crpix[0] - 1.0;
+    out->c2 = t->crpix[1] - 1.0;
+    pack_poly(t->a, t->a_order, &out->a);
+    pack_poly(t->b, t->b_order, &out->b);
+}
+
+static void triad(double ra_deg, double dec_deg, double B[9] /* columns e, n, k */)
+{
+    const double d2r = 3.14159265358979323846264338327950288 / 180.0;
+    const double sa = std::sin(ra_deg * d2r), ca = std::cos(ra_deg * d2r);
+    const double sd = std::sin(dec_deg * d2r), cdc = std::cos(dec_deg * d2r);
+    // row-major 3x3, column 0 = e, column 1 = n, column 2 = k
+    B[0] = -sa;  B[1] = -sd * ca;  B[2] = cdc * ca;
+    B[3] = ca;   B[4] = -sd * sa;  B[5] = cdc * sa;
+    B[6] = 0.0;  B[7] = cdc;       B[8] = sd;
+}
+
+static void mat3(const double *A, const double *B, double *C)   // C = A B
+{
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) {
+            double s = 0.0;
+            for (int k = 0; k < 3; ++k) s += A[3 * i + k] * B[3 * k + j];
+            C[3 * i + j] = s;
+        }
+}
+
+void make_source(const dfr_wcs *t, const dfr_wcs *s, SourceDev *out)
+{
+    const double kk = 3.14159265358979323846264338327950288 / 180.0;
+    double Bt[9], Bs[9], BsT[9], R[9], Dt[9], Es[9], T1[9];
+    triad(t->crval[0], t->crval[1], Bt);
+    triad(s->crval[0], s->crval[1], Bs);
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) BsT[3 * i + j] = Bs[3 * j + i];
+    mat3(BsT, Bt, R);                                   // rotation target frame -> source frame
+    // (xi, eta, 1) = Dt (U, V, 1): CD_t and degrees -> radians
+    const double dt[9] = {kk * t->cd[0], kk * t->cd[1], 0, kk * t->cd[2], kk * t->cd[3], 0, 0, 0, 1};
+    std::memcpy(Dt, dt, sizeof dt);
+    // (u_s c, v_s c, c) = Es (p.e_s, p.n_s, p.k_s): radians -> degrees and CD_s^-1
+    const double det = s->cd[0] * s->cd[3] - s->cd[1] * s->cd[2];
+    const double es[9] = {s->cd[3] / det / kk, -s->cd[1] / det / kk, 0,
+                          -s->cd[2] / det / kk, s->cd[0] / det / kk, 0, 0, 0, 1};
+    std::memcpy(Es, es, sizeof es);
+    mat3(R, Dt, T1);
+    mat3(Es, T1, out->m);
+    out->c1 = s->crpix[0] - 1.0;
+    out->c2 = s->crpix[1] - 1.0;
+    pack_poly(s->ap, s->ap_order, &out->ap);
+    pack_poly(s->bp, s->bp_order, &out->bp);
+}
+
+void make_sky(const dfr_wcs *w, SkyDev *out)
+{
+    const double kk = 3.14159265358979323846264338327950288 / 180.0;
+    out->c1 = w->crpix[0] - 1.0;
+    out->c2 = w->crpix[1] - 1.0;
+    out->ra0 = w->crval[0] * kk;
+    out->dec0 = w->crval[1] * kk;
+    const double det = w->cd[0] * w->cd[3] - w->cd[1] * w->cd[2];
+    for (int k = 0; k < 4; ++k) out->cd[k] = w->cd[k];
+    out->cdi[0] = w->cd[3] / det;
+    out->cdi[1] = -w->cd[1] / det;
+    out->cdi[2] = -w->cd[2] / det;
+    out->cdi[3] = w->cd[0] / det;
+    pack_poly(w->a, w->a_order, &out->a);
+    pack_poly(w->b, w->b_order, &out->b);
+    pack_poly(w->ap, w->ap_order, &out->ap);
+    pack_poly(w->bp, w->bp_order, &out->bp);
+}
+
+}  // namespace dfr

@@ -1,0 +1,223 @@
+"""-m gpu: the CUDA path (through the C ABI, via the thin binding) against the oracle,
+element by element on the same seeded inputs. Rules and tolerances: tests/parity.py."""
+import numpy as np
+import pytest
+
+import dfr_synth as S
+import oracle
+from tests import parity as PR
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+PATHS = {"exact": 1, "auto": 0}
+
+
+@pytest.fixture(scope="module")
+def P():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2505_03932_b200 as pkg
+    pkg.lib()
+    return pkg
+
+
+def run_gpu(P, w, order, path):
+    src = torch.from_numpy(w.images).cuda()
+    out = P.dfr_reproject(src, w.src_wcs, w.tgt_wcs, w.shape_out, order, path=path)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def full_parity(P, w, path, orders=None, exposures=None):
+    """Coordinates + mask + values for the listed exposures of workload w."""
+    sny, snx = w.images.shape[1:]
+    exposures = range(len(w.src_wcs)) if exposures is None else exposures
+    orders = w.orders if orders is None else orders
+    report = {}
+    outs = {o: run_gpu(P, w, o, path) for o in orders}
+    xg, yg = P.dfr_src_coords(w.src_wcs, w.tgt_wcs, (sny, snx), w.shape_out, orders[0], path=path)
+    xg, yg = xg.cpu().numpy(), yg.cpu().numpy()
+    for e in exposures:
+        xo, yo = oracle.src_coords(w.tgt_wcs, w.src_wcs[e], *w.shape_out)
+        report[("coords", e)] = PR.check_coords(xg[e], yg[e], xo, yo, w.src_wcs[e])
+        for o in orders:
+            ref = oracle.interp(w.images[e], xo.ravel(), yo.ravel(), o).reshape(w.shape_out).astype(np.float32)
+            report[(o, e)] = PR.check_image(outs[o][e], ref, xo, yo, w.images[e], o)
+    return report, outs
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_config0(P, path):
+    w = S.config0()
+    rep, outs = full_parity(P, w, PATHS[path])
+    # the oracle's own whole-path entry point agrees with src_coords + interp used above
+    ref = oracle.reproject(w.images, w.src_wcs, w.tgt_wcs, w.shape_out, 1)
+    m = np.isnan(ref[0])
+    assert abs(m.mean() - 0.024) < 0.004
+    assert rep[(1, 0)]["max"] <= PR.VALUE_TOL * rep[(1, 0)]["dr"]
+    print("C0", path, rep)
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_config1(P, path):
+    w = S.config1()
+    rep, _ = full_parity(P, w, PATHS[path])
+    assert abs(rep[(1, 0)]["nan_frac"] - 0.007) < 0.004
+    print("C1", path, rep)
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+@pytest.mark.parametrize("order", [0, 1, 3])
+def test_ragged_shapes_all_orders(P, path, order):
+    """Sizes that are not multiples of any tile, rotated + SIP, mask on all four sides."""
+    rng = np.random.default_rng(21)
+    sny, snx, ony, onx = 131, 203, 150, 177
+    img = S.make_image(sny, snx, 40, rng)
+    src = S.add_sip(S.make_wcs(snx, sny, 150.0, 2.0, 0.0, S.PIXSCALE), 3, snx / 2.0, rng, amp=1e-4)
+    tgt = S.add_sip(S.make_wcs(onx, ony, 150.003, 2.002, 17.0, S.PIXSCALE * 1.07), 4, onx / 2.0, rng, amp=1e-4)
+    w = S.Workload("ragged", img[None], [src], tgt, (ony, onx), (order,))
+    rep, _ = full_parity(P, w, PATHS[path])
+    assert 0.05 < rep[(order, 0)]["nan_frac"] < 0.9
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_stress_sip_coordinates(P, path):
+    """~9 px distortion: a percent-level SIP error would show far above 1e-4 px."""
+    src, tgt = S.stress_sip_pair()
+    xg, yg = P.dfr_src_coords([src], tgt, (1024, 1024), (1024, 1024), 1, path=PATHS[path])
+    xo, yo = oracle.src_coords(tgt, src, 1024, 1024)
+    st = PR.check_coords(xg[0].cpu().numpy(), yg[0].cpu().numpy(), xo, yo, src)
+    print("stress", path, st)
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_identity_and_integer_shift(P, path):
+    rng = np.random.default_rng(5)
+    img = S.make_image(70, 90, 10, rng)
+    w = S.make_wcs(90, 70, 10.0, -40.0, 0.0, S.PIXSCALE)
+    src = torch.from_numpy(img).cuda()
+    out = P.dfr_reproject(src, [w], w, None, 0, path=PATHS[path]).cpu().numpy()[0]
+    assert np.array_equal(out, img)                     # nearest: bit exact, no NaN
+    t = w.copy()
+    t.crpix = (w.crpix[0] + 7, w.crpix[1] - 3)
+    out = P.dfr_reproject(src, [w], t, None, 0, path=PATHS[path]).cpu().numpy()[0]
+    assert np.array_equal(out[:67, 7:], img[3:, :83])
+    assert np.isnan(out[67:, :]).all() and np.isnan(out[:, :7]).all()
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_degenerate_inputs(P, path):
+    # 1x1 image onto 1x1 and 3x5 grids
+    img = np.array([[42.0]], dtype=np.float32)
+    w = S.make_wcs(1, 1, 20.0, 30.0, 0.0, S.PIXSCALE)
+    src = torch.from_numpy(img).cuda()
+    for o in (0, 1, 3):
+        out = P.dfr_reproject(src, [w], w, (1, 1), o, path=PATHS[path]).cpu().numpy()
+        assert out.shape == (1, 1, 1) and out[0, 0, 0] == 42.0
+    t = S.make_wcs(5, 3, 20.0, 30.0, 0.0, S.PIXSCALE)
+    out = P.dfr_reproject(src, [w], t, (3, 5), 1, path=PATHS[path]).cpu().numpy()[0]
+    ref = oracle.reproject(img, [w], t, (3, 5), 1)[0]
+    assert np.array_equal(np.isnan(out), np.isnan(ref)) and out[1, 2] == 42.0
+    # source on the far side of the sky: every pixel NaN (theta <= 0, G12)
+    far = S.make_wcs(64, 64, 200.0, -30.0, 0.0, S.PIXSCALE)
+    img2 = np.ones((64, 64), dtype=np.float32)
+    out = P.dfr_reproject(torch.from_numpy(img2).cuda(), [far], S.make_wcs(64, 64, 20.0, 30.0, 0.0, S.PIXSCALE),
+                          None, 1, path=PATHS[path]).cpu().numpy()
+    assert np.isnan(out).all()
+    # disjoint but nearby footprint: all NaN as well
+    near = S.make_wcs(64, 64, 20.5, 30.0, 0.0, S.PIXSCALE)
+    out = P.dfr_reproject(torch.from_numpy(img2).cuda(), [near], S.make_wcs(64, 64, 20.0, 30.0, 0.0, S.PIXSCALE),
+                          None, 1, path=PATHS[path]).cpu().numpy()
+    assert np.isnan(out).all()
+
+
+def test_sky_entry_points(P):
+    rng = np.random.default_rng(9)
+    w = S.add_sip(S.make_wcs(2048, 2048, 359.99, -35.5, 33.0, S.PIXSCALE), 4, 1024.0, rng, amp=1e-4)
+    x = rng.uniform(-10, 2060, 20000)
+    y = rng.uniform(-10, 2060, 20000)
+    ra, dec = P.dfr_pix2world(w, torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda())
+    ra_o, dec_o = oracle.pix2world(w, x, y)
+    d = np.abs((ra.cpu().numpy() - ra_o + 180.0) % 360.0 - 180.0)
+    assert d.max() < 1e-10 and np.abs(dec.cpu().numpy() - dec_o).max() < 1e-10
+    assert ra.min().item() >= 0.0 and ra.max().item() < 360.0
+    xb, yb = P.dfr_world2pix(w, ra, dec)
+    xo, yo = oracle.world2pix(w, ra_o, dec_o)
+    lim = 1e-7 + PR.oracle_conditioning(xo, yo, w)
+    assert np.all(np.abs(xb.cpu().numpy() - xo) < lim) and np.all(np.abs(yb.cpu().numpy() - yo) < lim)
+    # far side -> NaN
+    xf, yf = P.dfr_world2pix(w, torch.tensor([179.99], dtype=torch.float64).cuda(),
+                             torch.tensor([35.5], dtype=torch.float64).cuda())
+    assert torch.isnan(xf).all() and torch.isnan(yf).all()
+    # zero points is legal
+    e = torch.empty(0, dtype=torch.float64).cuda()
+    r0, d0 = P.dfr_pix2world(w, e, e)
+    assert r0.numel() == 0
+
+
+def test_sip_order_9(P):
+    rng = np.random.default_rng(99)
+    src = S.add_sip(S.make_wcs(300, 300, 150.0, 2.0, 0.0, S.PIXSCALE), 9, 150.0, rng, amp=1e-4)
+    tgt = S.add_sip(S.make_wcs(300, 300, 150.001, 2.001, -3.0, S.PIXSCALE), 7, 150.0, rng, amp=1e-4)
+    for path in PATHS.values():
+        xg, yg = P.dfr_src_coords([src], tgt, (300, 300), (300, 300), 1, path=path)
+        xo, yo = oracle.src_coords(tgt, src, 300, 300)
+        PR.check_coords(xg[0].cpu().numpy(), yg[0].cpu().numpy(), xo, yo, src)
+
+
+def test_config2_batch_full_size(P):
+    """configs[2] at full size in the launch configuration bench.py times (batch 32 in one
+    call): three exposures element by element, plus 40 000 sampled pixels over all 32
+    computed one by one by the oracle."""
+    w = S.config2()
+    out = run_gpu(P, w, 1, 0)
+    st = P.dfr_last_stats()
+    sny, snx = w.images.shape[1:]
+    fr = []
+    for e in (0, 13, 31):
+        xo, yo = oracle.src_coords(w.tgt_wcs, w.src_wcs[e], *w.shape_out)
+        ref = oracle.interp(w.images[e], xo.ravel(), yo.ravel(), 1).reshape(w.shape_out).astype(np.float32)
+        r = PR.check_image(out[e], ref, xo, yo, w.images[e], 1)
+        fr.append(r["nan_frac"])
+    assert 0.005 < np.mean(fr) < 0.12
+    rng = np.random.default_rng(222)
+    for e in range(32):
+        ii = rng.integers(0, 2048, 1250).astype(np.float64)
+        jj = rng.integers(0, 2048, 1250).astype(np.float64)
+        ra, dec = oracle.pix2world(w.tgt_wcs, ii, jj)
+        xo, yo = oracle.world2pix(w.src_wcs[e], ra, dec)
+        ref = oracle.interp(w.images[e], xo, yo, 1).astype(np.float32)
+        got = out[e][jj.astype(int), ii.astype(int)]
+        band = PR.edge_band(xo, yo, sny, snx)
+        assert np.array_equal(np.isnan(got)[~band], np.isnan(ref)[~band])
+        ok = ~np.isnan(got) & ~np.isnan(ref)
+        assert np.max(np.abs(got[ok] - ref[ok])) <= PR.VALUE_TOL * PR.dyn_range(w.images[e])
+    print("C2 stats", st)
+
+
+def test_config3_three_orders(P):
+    w = S.config3()
+    rep, _ = full_parity(P, w, 0)
+    assert abs(rep[(1, 0)]["nan_frac"] - 0.075) < 0.01
+    print("C3", rep)
+
+
+def test_config4_stream_sample(P):
+    """configs[4] on the seeded sample of exposures (0, 31, 32, 511, 1023) through the
+    HOST-buffer streaming entry point, 2 exposures per batch so batches pipeline."""
+    idx = (0, 31, 32, 511, 1023)
+    w = S.config4(idx)
+    src = torch.from_numpy(w.images).pin_memory()
+    out = P.dfr_reproject_host(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1, batch=2)
+    out = out.numpy()
+    inside = []
+    for t in range(len(idx)):
+        xo, yo = oracle.src_coords(w.tgt_wcs, w.src_wcs[t], *w.shape_out)
+        ref = oracle.interp(w.images[t], xo.ravel(), yo.ravel(), 1).reshape(w.shape_out).astype(np.float32)
+        r = PR.check_image(out[t], ref, xo, yo, w.images[t], 1)
+        inside.append(1 - r["nan_frac"])
+    assert abs(np.mean(inside) - 0.25) < 0.01
+    # same result from the device-buffer entry point
+    dev = P.dfr_reproject(torch.from_numpy(w.images[:2]).cuda(), w.src_wcs[:2], w.tgt_wcs, w.shape_out, 1)
+    assert np.array_equal(np.nan_to_num(dev.cpu().numpy(), nan=-1), np.nan_to_num(out[:2], nan=-1))
