@@ -221,8 +221,14 @@ def main():
 
     # ---- dominant kernel, timed live by the library's own events on the launching stream
     kern_ms = None
-    if hasattr(P, "dfr_profile"):
-        kern_ms = P.dfr_profile(lambda: step(), repeats=min(args.steps, 10))
+    if path == P.PATH_AUTO:
+        P.dfr_profile_enable(True)
+        ms = []
+        for _ in range(min(args.steps, 10)):
+            step()
+            ms.append(P.dfr_profile_last())          # waits for the call's last event
+        P.dfr_profile_enable(False)
+        kern_ms = {"setup_ms": statistics.mean(m[0] for m in ms), "main_ms": statistics.mean(m[1] for m in ms)}
     nan_frac = float(torch.isnan(out).float().mean().item())
 
     # ---- e2e: HOST pinned buffers through dfr_reproject_host (copies inside the timed region)
@@ -252,20 +258,23 @@ def main():
 
     # ---- roofline: algorithmic bytes = 4 B stored per output pixel + 4 B per source pixel read once
     hbm, which, sm_max = peaks()
-    alg_bytes = 4.0 * BATCH * NPIX * NPIX + 4.0 * BATCH * NPIX * NPIX * (1.0 - 0.0)
+    # (8 B per output pixel is the upper bound SURVEY.md §8(d) states; the
+    # source pixels outside every output footprint and the NaN pixels are NOT subtracted)
+    alg_bytes = 8.0 * BATCH * NPIX * NPIX
     dom_ms = kern_ms["main_ms"] if kern_ms else statistics.median(per_step)
     achieved = alg_bytes / (dom_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s",
                 "frac": achieved / hbm, "traffic": None, "peak_source": which,
                 "kernel": "tiled_reproject_kernel" if kern_ms else "whole dfr_reproject call",
-                "kernel_ms": dom_ms, "algorithmic_bytes_per_launch": alg_bytes}
+                "kernel_ms": dom_ms, "setup_kernels_ms": kern_ms["setup_ms"] if kern_ms else None,
+                "algorithmic_bytes_per_launch": alg_bytes}
 
     cpu = None
     if not args.no_cpu_baseline:
-        n_exp = 4
+        n_exp = BATCH
         v, dt, cores = time_oracle(w, n_exp)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"first {n_exp} of the 32 exposures, full 2048x2048 frames ({dt:.1f} s wall)"}
+               "sample": f"all {n_exp} exposures of the step, full 2048x2048 frames, once ({dt:.1f} s wall)"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,

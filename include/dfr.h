@@ -153,6 +153,13 @@ int dfr_wcs_set_pc_cdelt(dfr_wcs *w, const double pc[4], const double cdelt[2]);
  * [2] = tiles entirely outside the footprint, [3] = kernels launched. */
 int dfr_last_stats(int64_t stats[4]);
 
+/* Timing hooks used by bench.py: when enabled (per host thread), dfr_reproject*
+ * records CUDA events on the caller's stream around its own kernels.
+ * dfr_profile_last waits for the last call and returns ms[0] = setup kernels
+ * (per-tile fit), ms[1] = main reprojection kernel. */
+int dfr_profile_enable(int on);
+int dfr_profile_last(float ms[2]);
+
 const char *dfr_strerror(int code);
 const char *dfr_last_error(void);
 int dfr_version(void);           /* 10000*major + 100*minor + patch */

@@ -21,6 +21,7 @@ _ORDER_NAMES = {"nearest": 0, "nearest-neighbor": 0, "bilinear": 1, "bicubic": 3
 
 EXPORTS = ["dfr_reproject", "dfr_reproject_ex", "dfr_reproject_host", "dfr_pix2world",
            "dfr_world2pix", "dfr_src_coords", "dfr_wcs_set_pc_cdelt", "dfr_last_stats",
+           "dfr_profile_enable", "dfr_profile_last",
            "dfr_strerror", "dfr_last_error", "dfr_version"]
 
 
@@ -60,6 +61,8 @@ def lib():
         L.dfr_src_coords.argtypes = [i32, i32, i32, wp, wp, i32, i32, i32, dp, dp, vp, i32]
         L.dfr_wcs_set_pc_cdelt.argtypes = [wp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.dfr_last_stats.argtypes = [C.POINTER(C.c_int64)]
+        L.dfr_profile_enable.argtypes = [C.c_int]
+        L.dfr_profile_last.argtypes = [C.POINTER(C.c_float)]
         L.dfr_strerror.argtypes = [C.c_int]
         L.dfr_strerror.restype = C.c_char_p
         L.dfr_last_error.restype = C.c_char_p
@@ -225,6 +228,17 @@ def dfr_last_stats():
     arr = (C.c_int64 * 4)()
     _check(lib().dfr_last_stats(arr))
     return {"tiles_fast": arr[0], "tiles_exact": arr[1], "tiles_empty": arr[2], "kernels": arr[3]}
+
+
+def dfr_profile_enable(on: bool):
+    _check(lib().dfr_profile_enable(1 if on else 0))
+
+
+def dfr_profile_last():
+    """(setup_ms, main_ms) of the last dfr_reproject call on this thread."""
+    ms = (C.c_float * 2)()
+    _check(lib().dfr_profile_last(ms))
+    return float(ms[0]), float(ms[1])
 
 
 def dfr_version() -> int:

@@ -12,8 +12,6 @@
 namespace dfr {
 const char *last_error_cstr();
 
-static thread_local int64_t g_stats[4] = {0, 0, 0, 0};
-
 static std::once_flag g_pool_once;
 static void tune_pool()
 {
@@ -48,11 +46,47 @@ static int check_common(int32_t n, int32_t sny, int32_t snx, const dfr_wcs *sw, 
     return DFR_OK;
 }
 
+// Per-thread record of the last call: tile counters land in pinned host memory through an
+// async copy; dfr_last_stats waits for it. Also the optional timing events (dfr_profile_*).
+struct LastCall {
+    int32_t *pinned = nullptr;          // 3 counters: fast, exact, empty
+    cudaEvent_t done = nullptr;
+    bool pending = false;
+    int64_t kernels = 0;
+    bool tiled = false;
+    ProfileEvents prof = {nullptr, nullptr, nullptr, false};
+};
+static thread_local LastCall g_last;
+static thread_local int64_t g_stats_acc[4] = {0, 0, 0, 0};   // used by dfr_reproject_host
+static thread_local bool g_accumulate = false;
+
+static cudaError_t ensure_last()
+{
+    cudaError_t err;
+    if (!g_last.pinned && (err = cudaMallocHost((void **)&g_last.pinned, 4 * sizeof(int32_t))) != cudaSuccess) return err;
+    if (!g_last.done && (err = cudaEventCreateWithFlags(&g_last.done, cudaEventDisableTiming)) != cudaSuccess) return err;
+    return cudaSuccess;
+}
+
+static void collect_stats(int64_t out[4])
+{
+    out[0] = out[1] = out[2] = 0;
+    out[3] = g_last.kernels;
+    if (g_last.tiled && g_last.pending) {
+        cudaEventSynchronize(g_last.done);
+        out[0] = g_last.pinned[0];
+        out[1] = g_last.pinned[1];
+        out[2] = g_last.pinned[2];
+    } else if (!g_last.tiled) {
+        out[1] = -1;                                          // exact path: no tiles
+    }
+}
+
 // Host constants -> device scratch (stream-ordered). Caller frees with cudaFreeAsync.
 static int upload_sources(int32_t n, const dfr_wcs *sw, const dfr_wcs *tw, cudaStream_t st,
-                          SourceDev **dev_out)
+                          std::vector<SourceDev> &h, SourceDev **dev_out)
 {
-    std::vector<SourceDev> h((size_t)n);
+    h.resize((size_t)n);
     for (int32_t e = 0; e < n; ++e) make_source(tw, &sw[e], &h[e]);
     SourceDev *d = nullptr;
     cudaError_t err = cudaMallocAsync((void **)&d, sizeof(SourceDev) * (size_t)n, st);
@@ -69,25 +103,42 @@ static int reproject_impl(const float *src, int32_t n, int32_t sny, int32_t snx,
                           int32_t order, float *out, cudaStream_t st, int32_t path)
 {
     std::call_once(g_pool_once, tune_pool);
+    if (g_accumulate && g_last.pending) {         // previous batch of a streaming call
+        int64_t t[4];
+        collect_stats(t);
+        for (int k = 0; k < 4; ++k) g_stats_acc[k] += t[k];
+    }
+    g_last.pending = false;
     TargetDev tgt;
     make_target(tw, &tgt);
+    std::vector<SourceDev> hsrc;
     SourceDev *dsrc = nullptr;
-    int rc = upload_sources(n, sw, tw, st, &dsrc);
+    int rc = upload_sources(n, sw, tw, st, hsrc, &dsrc);
     if (rc != DFR_OK) return rc;
     cudaError_t err;
     TiledStats ts = {0, 0, 0, 0};
     if (path == DFR_PATH_EXACT) {
+        if (g_last.prof.enabled) cudaEventRecord(g_last.prof.setup_begin, st), cudaEventRecord(g_last.prof.main_begin, st);
         err = launch_exact_reproject(src, n, sny, snx, tgt, dsrc, ony, onx, order, out, st);
-        ts.kernels = 1;
-        ts.tiles_exact = -1;
+        if (g_last.prof.enabled) cudaEventRecord(g_last.prof.main_end, st);
+        g_last.kernels = 1;
+        g_last.tiled = false;
     } else {
-        err = launch_tiled_reproject(src, n, sny, snx, tgt, dsrc, ony, onx, order, out, st, &ts);
+        int32_t *dcnt = nullptr;
+        err = ensure_last();
+        if (err == cudaSuccess) err = cudaMallocAsync((void **)&dcnt, 4 * sizeof(int32_t), st);
+        if (err == cudaSuccess)
+            err = launch_tiled_reproject(src, n, sny, snx, tgt, dsrc, hsrc.data(), ony, onx, order, out, st,
+                                         dcnt, &ts, &g_last.prof);
+        if (err == cudaSuccess)
+            err = cudaMemcpyAsync(g_last.pinned, dcnt, 3 * sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+        if (err == cudaSuccess) err = cudaEventRecord(g_last.done, st);
+        if (dcnt) cudaFreeAsync(dcnt, st);
+        g_last.kernels = ts.kernels;
+        g_last.tiled = true;
+        g_last.pending = (err == cudaSuccess);
     }
     cudaFreeAsync(dsrc, st);
-    g_stats[0] = ts.tiles_fast;
-    g_stats[1] = ts.tiles_exact;
-    g_stats[2] = ts.tiles_empty;
-    g_stats[3] = ts.kernels;
     if (err != cudaSuccess) return cuda_fail(err, "reproject launch");
     return DFR_OK;
 }
@@ -138,7 +189,8 @@ int dfr_src_coords(int32_t n, int32_t src_ny, int32_t src_nx,
     TargetDev tgt;
     make_target(tgt_wcs, &tgt);
     SourceDev *dsrc = nullptr;
-    rc = upload_sources(n, src_wcs, tgt_wcs, st, &dsrc);
+    std::vector<SourceDev> hsrc;
+    rc = upload_sources(n, src_wcs, tgt_wcs, st, hsrc, &dsrc);
     if (rc != DFR_OK) return rc;
     cudaError_t err;
     if (path == DFR_PATH_EXACT)
@@ -255,7 +307,9 @@ int dfr_reproject_host(const float *src_host, int32_t n, int32_t src_ny, int32_t
         err = ensure_slot(g_pipe.slot[k], in_px * batch * sizeof(float), out_px * batch * sizeof(float));
         if (err != cudaSuccess) return cuda_fail(err, "pipeline buffers");
     }
-    int64_t tot[4] = {0, 0, 0, 0};
+    for (int k = 0; k < 4; ++k) g_stats_acc[k] = 0;
+    g_last.pending = false;
+    g_accumulate = true;
     for (int b = 0; b < nb; ++b) {
         Slot &s = g_pipe.slot[b % kSlots];
         const int32_t e0 = b * batch, ne = (n - e0 < batch) ? n - e0 : batch;
@@ -266,7 +320,6 @@ int dfr_reproject_host(const float *src_host, int32_t n, int32_t src_ny, int32_t
         rc = reproject_impl(s.din, ne, src_ny, src_nx, src_wcs + e0, tgt_wcs, out_ny, out_nx, order,
                             s.dout, s.st, DFR_PATH_AUTO);
         if (rc != DFR_OK) break;
-        for (int k = 0; k < 4; ++k) tot[k] += g_stats[k];
         err = cudaMemcpyAsync(out_host + out_px * e0, s.dout, out_px * ne * sizeof(float),
                               cudaMemcpyDeviceToHost, s.st);
         if (err != cudaSuccess) { rc = cuda_fail(err, "D2H"); break; }
@@ -275,7 +328,14 @@ int dfr_reproject_host(const float *src_host, int32_t n, int32_t src_ny, int32_t
         err = cudaStreamSynchronize(g_pipe.slot[k].st);
         if (err != cudaSuccess && rc == DFR_OK) rc = cuda_fail(err, "pipeline sync");
     }
-    for (int k = 0; k < 4; ++k) g_stats[k] = tot[k];
+    g_accumulate = false;
+    if (g_last.pending) {
+        int64_t t[4];
+        collect_stats(t);
+        for (int k = 0; k < 4; ++k) g_stats_acc[k] += t[k];
+        g_last.pending = false;
+    }
+    g_last.kernels = -1;                 // marks "use the accumulated totals"
     return rc;
 }
 
@@ -292,8 +352,37 @@ int dfr_wcs_set_pc_cdelt(dfr_wcs *w, const double pc[4], const double cdelt[2])
 int dfr_last_stats(int64_t stats[4])
 {
     if (!stats) return DFR_ERR_NULL;
-    for (int k = 0; k < 4; ++k) stats[k] = g_stats[k];
+    if (g_last.kernels == -1) {
+        for (int k = 0; k < 4; ++k) stats[k] = g_stats_acc[k];
+        return DFR_OK;
+    }
+    collect_stats(stats);
     return DFR_OK;
+}
+
+int dfr_profile_enable(int on)
+{
+    ProfileEvents &p = g_last.prof;
+    if (on && !p.setup_begin) {
+        cudaError_t err;
+        if ((err = cudaEventCreate(&p.setup_begin)) != cudaSuccess ||
+            (err = cudaEventCreate(&p.main_begin)) != cudaSuccess ||
+            (err = cudaEventCreate(&p.main_end)) != cudaSuccess)
+            return cuda_fail(err, "cudaEventCreate");
+    }
+    p.enabled = on != 0;
+    return DFR_OK;
+}
+
+int dfr_profile_last(float ms[2])
+{
+    ProfileEvents &p = g_last.prof;
+    if (!ms) return DFR_ERR_NULL;
+    if (!p.enabled || !p.main_end) { set_error("profiling is not enabled"); return DFR_ERR_ORDER; }
+    cudaError_t err = cudaEventSynchronize(p.main_end);
+    if (err == cudaSuccess) err = cudaEventElapsedTime(&ms[0], p.setup_begin, p.main_begin);
+    if (err == cudaSuccess) err = cudaEventElapsedTime(&ms[1], p.main_begin, p.main_end);
+    return err == cudaSuccess ? DFR_OK : cuda_fail(err, "profile events");
 }
 
 const char *dfr_strerror(int code)

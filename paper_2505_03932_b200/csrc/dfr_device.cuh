@@ -12,7 +12,7 @@ namespace dfr {
 
 // sum_{p+q<=order} c[p][q] u^p v^q by nested Horner (north_star
 // "SIP is evaluated by Horner's rule"). Works for Poly in param or global space.
-__device__ __forceinline__ double poly_eval(const Poly &P, double u, double v)
+__host__ __device__ __forceinline__ double poly_eval(const Poly &P, double u, double v)
 {
     const int n = P.order;
     if (n <= 0) return 0.0;
@@ -28,7 +28,7 @@ __device__ __forceinline__ double poly_eval(const Poly &P, double u, double v)
 }
 
 // a1-a2: target pixel (i, j) -> distorted offsets (U, V).
-__device__ __forceinline__ void target_uv(const TargetDev &t, double i, double j,
+__host__ __device__ __forceinline__ void target_uv(const TargetDev &t, double i, double j,
                                           double &U, double &V)
 {
     const double u = i - t.c1, v = j - t.c2;
@@ -39,14 +39,14 @@ __device__ __forceinline__ void target_uv(const TargetDev &t, double i, double j
 // a3-a6: (U, V) -> fractional source pixel (x, y) for one exposure
 // (PAPER.md:91-121 in the projective form of dfr_host.cu). NaN when the sky
 // point is >= 90 deg from the source tangent point.
-__device__ __forceinline__ void source_xy(const SourceDev &s, double U, double V,
+__host__ __device__ __forceinline__ void source_xy(const SourceDev &s, double U, double V,
                                           double &x, double &y)
 {
     const double a = fma(s.m[0], U, fma(s.m[1], V, s.m[2]));
     const double b = fma(s.m[3], U, fma(s.m[4], V, s.m[5]));
     const double c = fma(s.m[6], U, fma(s.m[7], V, s.m[8]));
     if (!(c > 0.0)) {
-        x = y = __longlong_as_double(0x7ff8000000000000ULL);
+        x = y = NAN;
         return;
     }
     const double rc = 1.0 / c;

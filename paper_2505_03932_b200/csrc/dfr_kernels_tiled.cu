@@ -1,25 +1,657 @@
-// dfr_kernels_tiled.cu — tiled fast path (placeholder: routes to the exact path
-// until the tile kernels land; stats report every tile as "exact").
+// dfr_kernels_tiled.cu — the tiled fast path.
+//
+// The pixel map target -> source (a1-a6 of SURVEY.md §8(a)) is smooth, so on a
+// 32x32 output tile it is reproduced to < FIT_TOL px by a bicubic polynomial in
+// the tile-local offsets. Three kernels per dfr_reproject call:
+//
+//   target_nodes_kernel   (fp64) a1-a2 at 25 sample points per tile — shared by the
+//                         whole batch, as SURVEY.md §8(a) a10 notes.
+//   tile_setup_kernel     (fp64) a3-a6 at those points per (exposure, tile); fits the
+//                         cubic through 16 Chebyshev nodes, VERIFIES it against the
+//                         exact map at 9 other points, bounds the source footprint,
+//                         classifies the tile FAST / EXACT / EMPTY.
+//   tiled_reproject_kernel (fp32) per 64x64 CTA tile: the source bounding box is staged
+//                         into shared memory by one TMA box load; each warp walks one
+//                         32x32 tile, 3 FFMA per coordinate per pixel, floor by a
+//                         round-down add, gathers from shared memory, coalesced
+//                         128-byte row stores. Pixels whose taps leave the staged box
+//                         or touch the image rim, and all pixels of EXACT tiles, take
+//                         the exact/global-gather code of dfr_device.cuh.
+#include <cuda.h>
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+
+#include "dfr_device.cuh"
 #include "dfr_tiled.h"
 
 namespace dfr {
 
-cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
-                                   const TargetDev &tgt, const SourceDev *srcdev,
-                                   int ony, int onx, int order, float *out, cudaStream_t st,
-                                   TiledStats *stats)
+// ---------------------------------------------------------------------------------
+// constants of the fit
+// ---------------------------------------------------------------------------------
+struct FitConsts {
+    double W[4][4];            // monomial coefficients of the Lagrange basis: L_a(s) = sum_p W[p][a] s^p
+    double pts[NPTS][2];       // sample points (s, t) in [-1, 1]^2; pixel offset = 16 s
+};
+
+static FitConsts make_fit_consts()
 {
-    stats->tiles_fast = 0;
-    stats->tiles_exact = -1;
-    stats->tiles_empty = 0;
-    stats->kernels = 1;
-    return launch_exact_reproject(src, n, sny, snx, tgt, srcdev, ony, onx, order, out, st);
+    FitConsts f;
+    double s[4];
+    for (int a = 0; a < 4; ++a) s[a] = std::cos((2 * a + 1) * 3.14159265358979323846 / 8.0);
+    for (int a = 0; a < 4; ++a) {
+        double b[3];
+        int m = 0;
+        for (int k = 0; k < 4; ++k)
+            if (k != a) b[m++] = s[k];
+        const double den = (s[a] - b[0]) * (s[a] - b[1]) * (s[a] - b[2]);
+        f.W[3][a] = 1.0 / den;
+        f.W[2][a] = -(b[0] + b[1] + b[2]) / den;
+        f.W[1][a] = (b[0] * b[1] + b[0] * b[2] + b[1] * b[2]) / den;
+        f.W[0][a] = -(b[0] * b[1] * b[2]) / den;
+    }
+    for (int b = 0; b < 4; ++b)
+        for (int a = 0; a < 4; ++a) {
+            f.pts[4 * b + a][0] = s[a];
+            f.pts[4 * b + a][1] = s[b];
+        }
+    const double h = 0.70710678118654752440;
+    const double chk[9][2] = {{0, 0}, {h, h}, {-h, h}, {h, -h}, {-h, -h}, {1, 1}, {-1, 1}, {1, -1}, {-1, -1}};
+    for (int k = 0; k < 9; ++k) {
+        f.pts[16 + k][0] = chk[k][0];
+        f.pts[16 + k][1] = chk[k][1];
+    }
+    return f;
 }
 
-cudaError_t launch_tiled_coords(int n, int, int, const TargetDev &tgt, const SourceDev *srcdev,
-                                int ony, int onx, int, double *x, double *y, cudaStream_t st)
+constexpr double kHalf = 0.5 * TS;            // 16: pixel offset of s = 1
+constexpr double kCentre = 0.5 * (TS - 1);    // 15.5: tile centre relative to its first pixel
+
+// ---------------------------------------------------------------------------------
+// setup kernels (fp64)
+// ---------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+target_nodes_kernel(const __grid_constant__ TargetDev tgt, const __grid_constant__ FitConsts fc,
+                    int tiles_x, int ntile, double2 *__restrict__ uv)
 {
-    return launch_exact_coords(n, tgt, srcdev, ony, onx, x, y, st);
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= ntile * NPTS) return;
+    const int tile = idx / NPTS, k = idx - tile * NPTS;
+    const int tx0 = (tile % tiles_x) * TS, ty0 = (tile / tiles_x) * TS;
+    double U, V;
+    target_uv(tgt, tx0 + kCentre + kHalf * fc.pts[k][0], ty0 + kCentre + kHalf * fc.pts[k][1], U, V);
+    uv[idx] = make_double2(U, V);
+}
+
+__global__ void __launch_bounds__(128)
+tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ srcdev,
+                  const __grid_constant__ FitConsts fc, int n, int ntile, int sny, int snx,
+                  TileRec *__restrict__ recs, int32_t *__restrict__ counters)
+{
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = idx < (long long)n * ntile;
+    int flag = -1;
+    if (live) {
+        const int e = (int)(idx % n), tile = (int)(idx / n);   // lanes of a warp: same tile, different exposure
+        const SourceDev &s = srcdev[e];
+        const double2 *p = uv + (size_t)tile * NPTS;
+        double Cx[4][4], Cy[4][4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+            for (int b = 0; b < 4; ++b) Cx[a][b] = Cy[a][b] = 0.0;
+        bool finite = true;
+        double xmin = 1e300, xmax = -1e300, ymin = 1e300, ymax = -1e300;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            const double2 q = p[k];
+            double x, y;
+            source_xy(s, q.x, q.y, x, y);
+            finite = finite && isfinite(x) && isfinite(y);
+            xmin = fmin(xmin, x); xmax = fmax(xmax, x);
+            ymin = fmin(ymin, y); ymax = fmax(ymax, y);
+            const int a = k & 3, b = k >> 2;
+#pragma unroll
+            for (int pp = 0; pp < 4; ++pp)
+#pragma unroll
+                for (int qq = 0; qq < 4; ++qq) {
+                    const double w = fc.W[pp][a] * fc.W[qq][b];
+                    Cx[pp][qq] = fma(w, x, Cx[pp][qq]);
+                    Cy[pp][qq] = fma(w, y, Cy[pp][qq]);
+                }
+        }
+        // verify the fit against the exact map at 9 other points (centre, T4 extrema, corners)
+        double resid = 0.0;
+        for (int k = 16; k < NPTS; ++k) {
+            const double2 q = p[k];
+            double x, y;
+            source_xy(s, q.x, q.y, x, y);
+            finite = finite && isfinite(x) && isfinite(y);
+            xmin = fmin(xmin, x); xmax = fmax(xmax, x);
+            ymin = fmin(ymin, y); ymax = fmax(ymax, y);
+            const double ss = fc.pts[k][0], tt = fc.pts[k][1];
+            double px = 0.0, py = 0.0;
+#pragma unroll
+            for (int qq = 3; qq >= 0; --qq) {
+                const double rx = fma(fma(fma(Cx[3][qq], ss, Cx[2][qq]), ss, Cx[1][qq]), ss, Cx[0][qq]);
+                const double ry = fma(fma(fma(Cy[3][qq], ss, Cy[2][qq]), ss, Cy[1][qq]), ss, Cy[0][qq]);
+                px = fma(px, tt, rx);
+                py = fma(py, tt, ry);
+            }
+            resid = fmax(resid, fmax(fabs(px - x), fabs(py - y)));
+        }
+        TileRec r;
+        r.pad_ = 0;
+        flag = TILE_EXACT;
+        r.ix0 = r.iy0 = r.bx0 = r.by0 = r.bx1 = r.by1 = 0;
+        if (finite && fabs(xmin) < 1e9 && fabs(xmax) < 1e9 && fabs(ymin) < 1e9 && fabs(ymax) < 1e9) {
+            const double bx = floor(Cx[0][0]), by = floor(Cy[0][0]);
+            r.ix0 = (int)bx; r.iy0 = (int)by;
+            r.bx0 = (int)floor(xmin); r.bx1 = (int)floor(xmax);
+            r.by0 = (int)floor(ymin); r.by1 = (int)floor(ymax);
+            const bool small = (r.bx1 - r.bx0) < 2048 && (r.by1 - r.by0) < 2048 &&
+                               abs(r.bx0 - r.ix0) < 2048 && abs(r.bx1 - r.ix0) < 2048 &&
+                               abs(r.by0 - r.iy0) < 2048 && abs(r.by1 - r.iy0) < 2048;
+            if (resid <= (double)FIT_TOL && small) {
+                // outside the footprint [-0.5, n-0.5) by a 2 px margin on one side => all NaN
+                const bool out = (xmax + 2.0 < -0.5) || (xmin - 2.0 >= snx - 0.5) ||
+                                 (ymax + 2.0 < -0.5) || (ymin - 2.0 >= sny - 0.5);
+                flag = out ? TILE_EMPTY : TILE_FAST;
+            }
+            Cx[0][0] -= bx;
+            Cy[0][0] -= by;
+        }
+        r.flag = flag;
+        double sq = 1.0;
+#pragma unroll
+        for (int qq = 0; qq < 4; ++qq) {
+            double sp = sq;
+#pragma unroll
+            for (int pp = 0; pp < 4; ++pp) {
+                r.cx[4 * qq + pp] = (float)(Cx[pp][qq] * sp);
+                r.cy[4 * qq + pp] = (float)(Cy[pp][qq] * sp);
+                sp *= 1.0 / kHalf;
+            }
+            sq *= 1.0 / kHalf;
+        }
+        recs[(size_t)e * ntile + tile] = r;
+    }
+    if (counters) {
+        for (int f = 0; f < 3; ++f) {
+            const int c = __syncthreads_count(flag == f);
+            if (threadIdx.x == 0 && c) atomicAdd(&counters[f], c);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------
+// pieces of the main kernel
+// ---------------------------------------------------------------------------------
+constexpr float kMagic = 12582912.0f;              // 1.5 * 2^23: ulp 1 on [2^23, 2^24)
+constexpr int kMagicBits = 0x4B400000;
+
+template <int ORDER> struct Taps;
+template <> struct Taps<DFR_NEAREST>  { static constexpr int lo = 0, hi = 1; };   // rint in {floor, floor+1}
+template <> struct Taps<DFR_BILINEAR> { static constexpr int lo = 0, hi = 1; };
+template <> struct Taps<DFR_BICUBIC>  { static constexpr int lo = 1, hi = 2; };
+
+struct TiledParams {
+    const float *src;
+    float *out;
+    const TileRec *recs;
+    const SourceDev *srcdev;
+    int n, sny, snx, ony, onx;
+    int tiles_x, tiles_y, ctas_x, ctas_y;
+    int BW, BH;                                    // staged box (STAGE) in source pixels
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
+{
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+
+// Per-axis constants of the fast gather: valid floor/rint index range and address bias.
+struct AxisFast {
+    int C;              // k = float_as_int(T) - C  is the index relative to `lo`
+    unsigned cnt;       // valid <=> (unsigned)k < cnt
+};
+
+// index range [A_lo, A_hi] of the base tap for which every tap is inside the image AND
+// inside the staged box [o, o + B)
+template <int ORDER>
+__device__ __forceinline__ void axis_range(int n, int o, int B, int &A_lo, int &A_hi)
+{
+    if (ORDER == DFR_NEAREST) { A_lo = max(0, o); A_hi = min(n - 1, o + B - 1); }
+    else if (ORDER == DFR_BILINEAR) { A_lo = max(0, o); A_hi = min(n - 2, o + B - 2); }
+    else { A_lo = max(1, o + 1); A_hi = min(n - 3, o + B - 3); }
+}
+
+// Slow pixel of a FAST tile: polynomial coordinate, rim/out-of-box handling by the exact
+// footprint rule and edge-replicated global gathers.
+template <int ORDER>
+__device__ __noinline__ float slow_poly_pixel(const float *__restrict__ img, int sny, int snx,
+                                              int ix0, int iy0, float xl, float yl)
+{
+    const double x = (double)ix0 + (double)xl, y = (double)iy0 + (double)yl;
+    if (!in_footprint(x, y, sny, snx)) return qnanf();
+    return sample_global<ORDER>(img, sny, snx, x, y);
+}
+
+template <int ORDER>
+__device__ __noinline__ float exact_pixel(const float *__restrict__ img, int sny, int snx,
+                                          const TargetDev &tgt, const SourceDev &s, int i, int j)
+{
+    double U, V, x, y;
+    target_uv(tgt, (double)i, (double)j, U, V);
+    source_xy(s, U, V, x, y);
+    if (!in_footprint(x, y, sny, snx)) return qnanf();
+    return sample_global<ORDER>(img, sny, snx, x, y);
+}
+
+// Gather + interpolate from a dense [..][pitch] float array whose element (0,0) is the
+// first tap of base index (k_x, k_y) = (0, 0).
+template <int ORDER, typename Ptr>
+__device__ __forceinline__ float gather(Ptr base, int pitch, int kx, int ky, float fx, float fy)
+{
+    Ptr p = base + ky * pitch + kx;
+    if (ORDER == DFR_NEAREST) return p[0];
+    if (ORDER == DFR_BILINEAR) {
+        const float s00 = p[0], s10 = p[1], s01 = p[pitch], s11 = p[pitch + 1];
+        const float top = fmaf(fx, s10 - s00, s00);
+        const float bot = fmaf(fx, s11 - s01, s01);
+        return fmaf(fy, bot - top, top);
+    }
+    float wx[4], wy[4];
+    keys_weights(fx, wx);
+    keys_weights(fy, wy);
+    float acc = 0.0f;
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+        Ptr r = p + m * pitch;
+        float row = wx[0] * r[0];
+        row = fmaf(wx[1], r[1], row);
+        row = fmaf(wx[2], r[2], row);
+        row = fmaf(wx[3], r[3], row);
+        acc = fmaf(wy[m], row, acc);
+    }
+    return acc;
+}
+
+// ---------------------------------------------------------------------------------
+// main kernel: one CTA per 64x64 output tile per exposure, one warp per 32x32 tile
+// ---------------------------------------------------------------------------------
+template <int ORDER, bool STAGE>
+__global__ void __launch_bounds__(32 * CTA_T * CTA_T)
+tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_constant__ TargetDev tgt,
+                       const __grid_constant__ CUtensorMap tmap)
+{
+    extern __shared__ __align__(128) float box[];
+    __shared__ __align__(8) unsigned long long mbar;
+    __shared__ int s_bb[CTA_T * CTA_T][5];
+    __shared__ int s_box[3];
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int ctas = P.ctas_x * P.ctas_y;
+    const int e = blockIdx.x / ctas;
+    const int rem = blockIdx.x - e * ctas;
+    const int cty = rem / P.ctas_x, ctx = rem - cty * P.ctas_x;
+    const int ttx = ctx * CTA_T + (warp % CTA_T), tty = cty * CTA_T + (warp / CTA_T);
+    const bool active = ttx < P.tiles_x && tty < P.tiles_y;
+    const int ntile = P.tiles_x * P.tiles_y;
+    const TileRec *rec = P.recs + ((size_t)e * ntile + (active ? tty * P.tiles_x + ttx : 0));
+
+    int flag = TILE_EMPTY, ix0 = 0, iy0 = 0, bx0 = 0, by0 = 0, bx1 = 0, by1 = 0;
+    if (active) {
+        const int4 h0 = __ldg(reinterpret_cast<const int4 *>(&rec->ix0));       // ix0 iy0 bx0 by0
+        const int4 h1 = __ldg(reinterpret_cast<const int4 *>(&rec->bx1));       // bx1 by1 flag pad
+        ix0 = h0.x; iy0 = h0.y; bx0 = h0.z; by0 = h0.w; bx1 = h1.x; by1 = h1.y; flag = h1.z;
+    }
+
+    int ox = 0, oy = 0;                 // origin of the staged box in source pixels
+    bool has_box = false;
+    if (STAGE) {
+        if (lane == 0) {
+            s_bb[warp][0] = (active && flag == TILE_FAST) ? 1 : 0;
+            s_bb[warp][1] = bx0; s_bb[warp][2] = by0; s_bb[warp][3] = bx1; s_bb[warp][4] = by1;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int any = 0, mx = 0x7fffffff, my = 0x7fffffff;
+            for (int w = 0; w < CTA_T * CTA_T; ++w)
+                if (s_bb[w][0]) { any = 1; mx = min(mx, s_bb[w][1]); my = min(my, s_bb[w][2]); }
+            s_box[0] = any;
+            if (any) {
+                // TMA wants a 16-byte aligned start along x (measured on B200: an unaligned
+                // inner coordinate faults with "illegal instruction"): round down to 4 floats
+                mx = (mx - (Taps<ORDER>::lo + 1)) & ~3;
+                my -= Taps<ORDER>::lo + 1;
+                s_box[1] = mx; s_box[2] = my;
+                const uint32_t bar = smem_u32(&mbar), dst = smem_u32(box);
+                asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+                asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                const uint32_t bytes = (uint32_t)(P.BW * P.BH * sizeof(float));
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+                asm volatile(
+                    "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                    ::"r"(dst), "l"(&tmap), "r"(mx), "r"(my), "r"(e), "r"(bar) : "memory");
+            }
+        }
+        __syncthreads();
+        has_box = s_box[0] != 0;
+        ox = s_box[1]; oy = s_box[2];
+        if (has_box) {
+            const uint32_t bar = smem_u32(&mbar);
+            uint32_t done = 0;
+            while (!done) {
+                asm volatile(
+                    "{\n\t.reg .pred p;\n\t"
+                    "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                    "selp.u32 %0, 1, 0, p;\n\t}"
+                    : "=r"(done) : "r"(bar), "r"(0u) : "memory");
+            }
+        }
+    }
+    if (!active) return;
+
+    const int tx0 = ttx * TS, ty0 = tty * TS;
+    const int col = tx0 + lane;
+    const bool col_ok = col < P.onx;
+    const int rows = min(TS, P.ony - ty0);
+    float *__restrict__ orow = P.out + ((size_t)e * P.ony + ty0) * P.onx + col;
+    const float *__restrict__ img = P.src + (size_t)e * P.sny * P.snx;
+
+    if (flag == TILE_EMPTY) {
+        if (col_ok)
+            for (int r = 0; r < rows; ++r) orow[(size_t)r * P.onx] = qnanf();
+        return;
+    }
+    if (flag == TILE_EXACT) {
+        if (col_ok)
+            for (int r = 0; r < rows; ++r)
+                orow[(size_t)r * P.onx] = exact_pixel<ORDER>(img, P.sny, P.snx, tgt, P.srcdev[e], col, ty0 + r);
+        return;
+    }
+
+    // ---- FAST tile: per-lane column polynomials in dj
+    float X[4], Y[4];
+    {
+        const float di = (float)lane - (float)kCentre;
+        const float4 *c4 = reinterpret_cast<const float4 *>(rec->cx);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const float4 a = __ldg(c4 + q), b = __ldg(c4 + 4 + q);
+            X[q] = fmaf(fmaf(fmaf(a.w, di, a.z), di, a.y), di, a.x);
+            Y[q] = fmaf(fmaf(fmaf(b.w, di, b.z), di, b.y), di, b.x);
+        }
+    }
+    // ---- per-axis fast-gather constants (a FAST tile in a STAGE kernel always has a box)
+    int Alx, Ahx, Aly, Ahy;
+    if (STAGE) {
+        axis_range<ORDER>(P.snx, ox, P.BW, Alx, Ahx);
+        axis_range<ORDER>(P.sny, oy, P.BH, Aly, Ahy);
+    } else {
+        axis_range<ORDER>(P.snx, -(1 << 28), 1 << 30, Alx, Ahx);
+        axis_range<ORDER>(P.sny, -(1 << 28), 1 << 30, Aly, Ahy);
+    }
+    const int pitch = STAGE ? P.BW : P.snx;
+    const unsigned cntx = (unsigned)max(Ahx - Alx + 1, 0), cnty = (unsigned)max(Ahy - Aly + 1, 0);
+    const int Cx = kMagicBits - ix0 + Alx, Cy = kMagicBits - iy0 + Aly;
+    // element (k = 0) of the gather array = first tap of base index (Alx, Aly)
+    const int tlo = (ORDER == DFR_BICUBIC) ? 1 : 0;
+    const float *__restrict__ gbase = img + ((long long)(Aly - tlo) * P.snx + (Alx - tlo));
+    const float *sbase = box + ((Aly - tlo - oy) * P.BW + (Alx - tlo - ox));
+
+#pragma unroll 4
+    for (int r = 0; r < rows; ++r) {
+        const float dj = (float)r - (float)kCentre;
+        const float xl = fmaf(fmaf(fmaf(X[3], dj, X[2]), dj, X[1]), dj, X[0]);
+        const float yl = fmaf(fmaf(fmaf(Y[3], dj, Y[2]), dj, Y[1]), dj, Y[0]);
+        float Tx, Ty;
+        if (ORDER == DFR_NEAREST) { Tx = xl + kMagic; Ty = yl + kMagic; }          // rint (half-even)
+        else { Tx = __fadd_rd(xl, kMagic); Ty = __fadd_rd(yl, kMagic); }            // floor
+        const float fx = xl - (Tx - kMagic), fy = yl - (Ty - kMagic);
+        const int kx = __float_as_int(Tx) - Cx, ky = __float_as_int(Ty) - Cy;
+        float val;
+        if ((unsigned)kx < cntx && (unsigned)ky < cnty) {
+            if (STAGE) val = gather<ORDER, const float *>(sbase, pitch, kx, ky, fx, fy);
+            else val = gather<ORDER, const float *__restrict__>(gbase, pitch, kx, ky, fx, fy);
+        } else {
+            val = slow_poly_pixel<ORDER>(img, P.sny, P.snx, ix0, iy0, xl, yl);
+        }
+        if (col_ok) orow[(size_t)r * P.onx] = val;
+    }
+}
+
+// coordinates the tiled path uses (dfr_src_coords): same records, same polynomial code
+__global__ void __launch_bounds__(32 * CTA_T * CTA_T)
+tiled_coords_kernel(const __grid_constant__ TiledParams P, const __grid_constant__ TargetDev tgt,
+                    double *__restrict__ xo, double *__restrict__ yo)
+{
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int ctas = P.ctas_x * P.ctas_y;
+    const int e = blockIdx.x / ctas;
+    const int rem = blockIdx.x - e * ctas;
+    const int cty = rem / P.ctas_x, ctx = rem - cty * P.ctas_x;
+    const int ttx = ctx * CTA_T + (warp % CTA_T), tty = cty * CTA_T + (warp / CTA_T);
+    if (!(ttx < P.tiles_x && tty < P.tiles_y)) return;
+    const int ntile = P.tiles_x * P.tiles_y;
+    const TileRec *rec = P.recs + ((size_t)e * ntile + tty * P.tiles_x + ttx);
+    const int flag = rec->flag, ix0 = rec->ix0, iy0 = rec->iy0;
+    const int tx0 = ttx * TS, ty0 = tty * TS, col = tx0 + lane;
+    if (col >= P.onx) return;
+    const int rows = min(TS, P.ony - ty0);
+    const size_t o = ((size_t)e * P.ony + ty0) * P.onx + col;
+    if (flag == TILE_EXACT) {
+        for (int r = 0; r < rows; ++r) {
+            double U, V, x, y;
+            target_uv(tgt, (double)col, (double)(ty0 + r), U, V);
+            source_xy(P.srcdev[e], U, V, x, y);
+            xo[o + (size_t)r * P.onx] = x;
+            yo[o + (size_t)r * P.onx] = y;
+        }
+        return;
+    }
+    float X[4], Y[4];
+    const float di = (float)lane - (float)kCentre;
+    const float4 *c4 = reinterpret_cast<const float4 *>(rec->cx);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const float4 a = __ldg(c4 + q), b = __ldg(c4 + 4 + q);
+        X[q] = fmaf(fmaf(fmaf(a.w, di, a.z), di, a.y), di, a.x);
+        Y[q] = fmaf(fmaf(fmaf(b.w, di, b.z), di, b.y), di, b.x);
+    }
+    for (int r = 0; r < rows; ++r) {
+        const float dj = (float)r - (float)kCentre;
+        const float xl = fmaf(fmaf(fmaf(X[3], dj, X[2]), dj, X[1]), dj, X[0]);
+        const float yl = fmaf(fmaf(fmaf(Y[3], dj, Y[2]), dj, Y[1]), dj, Y[0]);
+        xo[o + (size_t)r * P.onx] = (double)ix0 + (double)xl;
+        yo[o + (size_t)r * P.onx] = (double)iy0 + (double)yl;
+    }
+}
+
+// ---------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *,
+                                  const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
+                                  const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn get_encode()
+{
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+constexpr int kMaxBoxBytes = 36 * 1024;          // keeps >= 6 CTAs (24 warps) per SM
+
+// Source-pixel extent of a 64x64 output tile, probed in fp64 on the host at the centre and
+// corners of the output grid for (a sample of) the exposures. Returns false if no probe is finite.
+static bool probe_extent(const TargetDev &tgt, const SourceDev *hs, int n, int ony, int onx,
+                         double &ext_x, double &ext_y)
+{
+    const int span = TS * CTA_T;
+    const double px[5] = {0.0, (double)std::max(onx - span, 0), 0.0, (double)std::max(onx - span, 0),
+                          std::max(0.5 * (onx - span), 0.0)};
+    const double py[5] = {0.0, 0.0, (double)std::max(ony - span, 0), (double)std::max(ony - span, 0),
+                          std::max(0.5 * (ony - span), 0.0)};
+    const int step = n > 64 ? n / 64 : 1;
+    bool any = false;
+    ext_x = ext_y = 0.0;
+    for (int e = 0; e < n; e += step)
+        for (int k = 0; k < 5; ++k) {
+            double xmin = 1e300, xmax = -1e300, ymin = 1e300, ymax = -1e300;
+            bool fin = true;
+            for (int c = 0; c < 9; ++c) {
+                const double i = px[k] + (c % 3) * 0.5 * (span - 1), j = py[k] + (c / 3) * 0.5 * (span - 1);
+                double U, V, x, y;
+                target_uv(tgt, i, j, U, V);
+                source_xy(hs[e], U, V, x, y);
+                fin = fin && std::isfinite(x) && std::isfinite(y);
+                xmin = std::fmin(xmin, x); xmax = std::fmax(xmax, x);
+                ymin = std::fmin(ymin, y); ymax = std::fmax(ymax, y);
+            }
+            if (!fin) continue;
+            any = true;
+            ext_x = std::fmax(ext_x, xmax - xmin);
+            ext_y = std::fmax(ext_y, ymax - ymin);
+        }
+    return any;
+}
+
+template <int ORDER, bool STAGE>
+static cudaError_t launch_main(const TiledParams &P, const TargetDev &tgt, const CUtensorMap &tmap,
+                               size_t smem, cudaStream_t st)
+{
+    auto kern = tiled_reproject_kernel<ORDER, STAGE>;
+    if (STAGE) {      // per device, cheap: set every time
+        cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxBoxBytes);
+        if (err != cudaSuccess) return err;
+    }
+    const long long blocks = (long long)P.ctas_x * P.ctas_y * P.n;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    kern<<<(unsigned)blocks, 32 * CTA_T * CTA_T, smem, st>>>(P, tgt, tmap);
+    return cudaGetLastError();
+}
+
+struct Scratch {
+    double2 *uv = nullptr;
+    TileRec *recs = nullptr;
+};
+
+static cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const SourceDev *srcdev,
+                             int ony, int onx, cudaStream_t st, int32_t *counters, Scratch &sc,
+                             TiledParams &P)
+{
+    static const FitConsts fc = make_fit_consts();
+    P.n = n; P.sny = sny; P.snx = snx; P.ony = ony; P.onx = onx;
+    P.tiles_x = (onx + TS - 1) / TS;
+    P.tiles_y = (ony + TS - 1) / TS;
+    P.ctas_x = (P.tiles_x + CTA_T - 1) / CTA_T;
+    P.ctas_y = (P.tiles_y + CTA_T - 1) / CTA_T;
+    P.srcdev = srcdev;
+    const int ntile = P.tiles_x * P.tiles_y;
+    cudaError_t err;
+    if ((err = cudaMallocAsync((void **)&sc.uv, sizeof(double2) * (size_t)ntile * NPTS, st)) != cudaSuccess) return err;
+    if ((err = cudaMallocAsync((void **)&sc.recs, sizeof(TileRec) * (size_t)ntile * n, st)) != cudaSuccess) return err;
+    P.recs = sc.recs;
+    if (counters && (err = cudaMemsetAsync(counters, 0, 3 * sizeof(int32_t), st)) != cudaSuccess) return err;
+    target_nodes_kernel<<<(ntile * NPTS + 127) / 128, 128, 0, st>>>(tgt, fc, P.tiles_x, ntile, sc.uv);
+    if ((err = cudaGetLastError()) != cudaSuccess) return err;
+    const long long work = (long long)ntile * n;
+    tile_setup_kernel<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(sc.uv, srcdev, fc, n, ntile, sny, snx,
+                                                                      sc.recs, counters);
+    return cudaGetLastError();
+}
+
+static void free_scratch(Scratch &sc, cudaStream_t st)
+{
+    if (sc.uv) cudaFreeAsync(sc.uv, st);
+    if (sc.recs) cudaFreeAsync(sc.recs, st);
+}
+
+cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
+                                   const TargetDev &tgt, const SourceDev *srcdev,
+                                   const SourceDev *srchost,
+                                   int ony, int onx, int order, float *out, cudaStream_t st,
+                                   int32_t *dev_counters, TiledStats *stats, ProfileEvents *prof)
+{
+    TiledParams P;
+    std::memset(&P, 0, sizeof P);
+    P.src = src;
+    P.out = out;
+    Scratch sc;
+    if (prof && prof->enabled) cudaEventRecord(prof->setup_begin, st);
+    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, ony, onx, st, dev_counters, sc, P);
+    if (err != cudaSuccess) { free_scratch(sc, st); return err; }
+
+    // ---- staging decision: box size from a host probe; TMA needs 16-byte rows
+    bool stage = false;
+    CUtensorMap tmap;
+    std::memset(&tmap, 0, sizeof tmap);
+    double ex, ey;
+    const int tlo = (order == DFR_BICUBIC) ? 1 : 0, thi = (order == DFR_BICUBIC) ? 2 : 1;
+    EncodeTiledFn enc = get_encode();
+    static const bool no_stage = std::getenv("DFR_NO_STAGE") != nullptr;   // debugging / A-B timing only
+    if (!no_stage && enc && (snx % 4 == 0) && ((uintptr_t)src % 16 == 0) && probe_extent(tgt, srchost, n, ony, onx, ex, ey)) {
+        // floor-range spread + taps + 1 px safety each side; + 3: the origin is rounded down
+        // to a multiple of 4 floats; then the width itself is rounded up to 16 bytes
+        const int bw = ((int)std::ceil(ex * 1.02) + 2 + tlo + thi + 2 + 3 + 3) & ~3;
+        const int bh = (int)std::ceil(ey * 1.02) + 2 + tlo + thi + 2;
+        if (bw <= 256 && bh <= 256 && (size_t)bw * bh * sizeof(float) <= (size_t)kMaxBoxBytes) {
+            const cuuint64_t dims[3] = {(cuuint64_t)snx, (cuuint64_t)sny, (cuuint64_t)n};
+            const cuuint64_t strides[2] = {(cuuint64_t)snx * 4, (cuuint64_t)snx * sny * 4};
+            const cuuint32_t boxd[3] = {(cuuint32_t)bw, (cuuint32_t)bh, 1};
+            const cuuint32_t estr[3] = {1, 1, 1};
+            CUresult r = enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)src, dims, strides, boxd, estr,
+                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                             CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r == CUDA_SUCCESS) { stage = true; P.BW = bw; P.BH = bh; }
+        }
+    }
+    const size_t smem = stage ? (size_t)P.BW * P.BH * sizeof(float) : 0;
+    if (prof && prof->enabled) cudaEventRecord(prof->main_begin, st);
+#define DFR_LAUNCH(O)                                                                     \
+    err = stage ? launch_main<O, true>(P, tgt, tmap, smem, st) : launch_main<O, false>(P, tgt, tmap, 0, st)
+    if (order == DFR_NEAREST) DFR_LAUNCH(DFR_NEAREST);
+    else if (order == DFR_BILINEAR) DFR_LAUNCH(DFR_BILINEAR);
+    else DFR_LAUNCH(DFR_BICUBIC);
+#undef DFR_LAUNCH
+    if (prof && prof->enabled) cudaEventRecord(prof->main_end, st);
+    free_scratch(sc, st);
+    stats->kernels = 3;
+    stats->tiles_fast = stats->tiles_exact = stats->tiles_empty = -1;   // filled from dev_counters by the caller
+    return err;
+}
+
+cudaError_t launch_tiled_coords(int n, int sny, int snx, const TargetDev &tgt,
+                                const SourceDev *srcdev, int ony, int onx, int order,
+                                double *x, double *y, cudaStream_t st)
+{
+    (void)order;
+    TiledParams P;
+    std::memset(&P, 0, sizeof P);
+    Scratch sc;
+    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, ony, onx, st, nullptr, sc, P);
+    if (err == cudaSuccess) {
+        const long long blocks = (long long)P.ctas_x * P.ctas_y * n;
+        tiled_coords_kernel<<<(unsigned)blocks, 32 * CTA_T * CTA_T, 0, st>>>(P, tgt, x, y);
+        err = cudaGetLastError();
+    }
+    free_scratch(sc, st);
+    return err;
 }
 
 }  // namespace dfr

@@ -1,17 +1,46 @@
-// dfr_tiled.h — launchers of the tiled fast path (dfr_kernels_tiled.cu).
+// dfr_tiled.h — the tiled fast path (dfr_kernels_tiled.cu): data layout of the
+// per-(exposure, tile) records and the launchers. DESIGN.md §6 describes it.
 #pragma once
 #include "dfr_internal.h"
 
 namespace dfr {
 
+constexpr int TS = 32;              // polynomial tile edge in output pixels (one warp wide)
+constexpr int CTA_T = 2;            // a CTA covers CTA_T x CTA_T polynomial tiles (64 x 64 px)
+constexpr int NPTS = 25;            // 16 interpolation nodes + 9 check points per tile
+constexpr float FIT_TOL = 2e-6f;    // px: max |cubic fit - exact map| at the check points
+
+enum { TILE_FAST = 0, TILE_EXACT = 1, TILE_EMPTY = 2 };
+
+// Per (exposure, tile) record written by tile_setup_kernel, read by the main kernels.
+// Source pixel of target pixel (tx0 + 15.5 + di, ty0 + 15.5 + dj), |di|,|dj| <= 15.5:
+//   x = ix0 + sum_{p,q<=3} cx[4q+p] di^p dj^q     (fp32 evaluation, |x - ix0| small)
+struct __align__(16) TileRec {
+    float   cx[16];
+    float   cy[16];
+    int32_t ix0, iy0;               // integer base (floor of the tile-centre source pixel)
+    int32_t bx0, by0, bx1, by1;     // inclusive range of floor(x), floor(y) over the tile
+    int32_t flag;                   // TILE_*
+    int32_t pad_;
+};
+static_assert(sizeof(TileRec) == 160, "TileRec layout");
+
 struct TiledStats {
     int64_t tiles_fast, tiles_exact, tiles_empty, kernels;
 };
 
+// Timing hooks (dfr_profile_*): events recorded around the main kernel only.
+struct ProfileEvents {
+    cudaEvent_t setup_begin, main_begin, main_end;
+    bool enabled;
+};
+
 cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
                                    const TargetDev &tgt, const SourceDev *srcdev,
+                                   const SourceDev *srchost,
                                    int ony, int onx, int order, float *out, cudaStream_t st,
-                                   TiledStats *stats);
+                                   int32_t *dev_counters /* 3 ints, zeroed here */,
+                                   TiledStats *stats, ProfileEvents *prof);
 cudaError_t launch_tiled_coords(int n, int sny, int snx, const TargetDev &tgt,
                                 const SourceDev *srcdev, int ony, int onx, int order,
                                 double *x, double *y, cudaStream_t st);

@@ -221,3 +221,44 @@ def test_config4_stream_sample(P):
     # same result from the device-buffer entry point
     dev = P.dfr_reproject(torch.from_numpy(w.images[:2]).cuda(), w.src_wcs[:2], w.tgt_wcs, w.shape_out, 1)
     assert np.array_equal(np.nan_to_num(dev.cpu().numpy(), nan=-1), np.nan_to_num(out[:2], nan=-1))
+
+
+def test_fast_path_is_taken_and_matches_exact(P):
+    """AUTO must run the tiled kernels on ordinary geometry (not silently the exact path),
+    agree with the exact path to the parity tolerance, and classify empty tiles."""
+    w = S.config1(n=1024, nstars=500)
+    src = torch.from_numpy(w.images).cuda()
+    fast = P.dfr_reproject(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1, path=P.PATH_AUTO)
+    st = P.dfr_last_stats()
+    assert st["kernels"] == 3 and st["tiles_fast"] == 32 * 32 and st["tiles_exact"] == 0
+    exact = P.dfr_reproject(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1, path=P.PATH_EXACT)
+    assert P.dfr_last_stats()["kernels"] == 1
+    f, x = fast.cpu().numpy()[0], exact.cpu().numpy()[0]
+    both = ~np.isnan(f) & ~np.isnan(x)
+    assert (np.isnan(f) != np.isnan(x)).sum() <= 8           # only on the footprint edge
+    assert np.max(np.abs(f[both] - x[both])) <= PR.VALUE_TOL * PR.dyn_range(w.images[0])
+    xf, yf = P.dfr_src_coords(w.src_wcs, w.tgt_wcs, (1024, 1024), w.shape_out, 1, path=P.PATH_AUTO)
+    xe, ye = P.dfr_src_coords(w.src_wcs, w.tgt_wcs, (1024, 1024), w.shape_out, 1, path=P.PATH_EXACT)
+    d = max((xf - xe).abs().max().item(), (yf - ye).abs().max().item())
+    print("tiled vs exact coords: max", d)
+    assert d < 2e-5
+    # a mosaic-like target: most tiles are empty
+    w4 = S.config4((7,), n=512, nstars=100, mosaic=2048)
+    out = P.dfr_reproject(torch.from_numpy(w4.images).cuda(), w4.src_wcs, w4.tgt_wcs, w4.shape_out, 1)
+    st = P.dfr_last_stats()
+    assert st["tiles_empty"] > 0.8 * 64 * 64 and st["tiles_fast"] > 0
+    ref = oracle.reproject(w4.images, w4.src_wcs, w4.tgt_wcs, w4.shape_out, 1)
+    xo, yo = oracle.src_coords(w4.tgt_wcs, w4.src_wcs[0], *w4.shape_out)
+    PR.check_image(out[0].cpu().numpy(), ref[0], xo, yo, w4.images[0], 1)
+
+
+def test_unaligned_row_pitch_uses_global_gathers(P):
+    """nx % 4 != 0 cannot be described to TMA (16-byte row pitch): the tiled kernel then
+    gathers from global memory; results must be the same."""
+    rng = np.random.default_rng(31)
+    img = S.make_image(301, 403, 60, rng)
+    src = S.add_sip(S.make_wcs(403, 301, 150.0, 2.0, 0.0, S.PIXSCALE), 3, 201.5, rng, amp=1e-5)
+    tgt = S.add_sip(S.make_wcs(390, 310, 150.002, 2.001, -2.0, S.PIXSCALE), 3, 195.0, rng, amp=1e-5)
+    w = S.Workload("odd", img[None], [src], tgt, (310, 390), (0, 1, 3))
+    rep, _ = full_parity(P, w, 0)
+    assert P.dfr_last_stats()["tiles_fast"] > 0
