@@ -196,7 +196,7 @@ int dfr_src_coords(int32_t n, int32_t src_ny, int32_t src_nx,
     if (path == DFR_PATH_EXACT)
         err = launch_exact_coords(n, tgt, dsrc, out_ny, out_nx, x, y, st);
     else
-        err = launch_tiled_coords(n, src_ny, src_nx, tgt, dsrc, out_ny, out_nx, order, x, y, st);
+        err = launch_tiled_coords(n, src_ny, src_nx, tgt, dsrc, hsrc.data(), out_ny, out_nx, order, x, y, st);
     cudaFreeAsync(dsrc, st);
     if (err != cudaSuccess) return cuda_fail(err, "src_coords launch");
     return DFR_OK;

@@ -10,19 +10,52 @@
 
 namespace dfr {
 
+// fma() on the host is a libm call unless the build enables FMA; the host only needs
+// these functions for coarse geometry probes, so plain a*b+c is fine there.
+#ifdef __CUDA_ARCH__
+#define DFR_FMA(a, b, c) fma((a), (b), (c))
+#else
+#define DFR_FMA(a, b, c) ((a) * (b) + (c))
+#endif
+
 // sum_{p+q<=order} c[p][q] u^p v^q by nested Horner (north_star
 // "SIP is evaluated by Horner's rule"). Works for Poly in param or global space.
+// The common orders are fully unrolled (no loop or index arithmetic survives).
+template <int N>
+__host__ __device__ __forceinline__ double poly_eval_fixed(const double *__restrict__ c, double u, double v)
+{
+    double r = 0.0;
+#pragma unroll
+    for (int p = N; p >= 0; --p) {
+        const int off = p * (N + 1) - (p * (p - 1)) / 2;
+        const int len = N - p + 1;
+        double inner = c[off + len - 1];
+#pragma unroll
+        for (int q = len - 2; q >= 0; --q) inner = DFR_FMA(inner, v, c[off + q]);
+        r = DFR_FMA(r, u, inner);
+    }
+    return r;
+}
+
 __host__ __device__ __forceinline__ double poly_eval(const Poly &P, double u, double v)
 {
     const int n = P.order;
-    if (n <= 0) return 0.0;
+    switch (n) {
+    case 0: return 0.0;
+    case 2: return poly_eval_fixed<2>(P.c, u, v);
+    case 3: return poly_eval_fixed<3>(P.c, u, v);
+    case 4: return poly_eval_fixed<4>(P.c, u, v);
+    case 5: return poly_eval_fixed<5>(P.c, u, v);
+    default: break;
+    }
+    if (n < 0) return 0.0;
     double r = 0.0;
     for (int p = n; p >= 0; --p) {
         const int off = p * (n + 1) - (p * (p - 1)) / 2;
         const int len = n - p + 1;
         double inner = P.c[off + len - 1];
-        for (int q = len - 2; q >= 0; --q) inner = fma(inner, v, P.c[off + q]);
-        r = fma(r, u, inner);
+        for (int q = len - 2; q >= 0; --q) inner = DFR_FMA(inner, v, P.c[off + q]);
+        r = DFR_FMA(r, u, inner);
     }
     return r;
 }
@@ -42,9 +75,9 @@ __host__ __device__ __forceinline__ void target_uv(const TargetDev &t, double i,
 __host__ __device__ __forceinline__ void source_xy(const SourceDev &s, double U, double V,
                                           double &x, double &y)
 {
-    const double a = fma(s.m[0], U, fma(s.m[1], V, s.m[2]));
-    const double b = fma(s.m[3], U, fma(s.m[4], V, s.m[5]));
-    const double c = fma(s.m[6], U, fma(s.m[7], V, s.m[8]));
+    const double a = DFR_FMA(s.m[0], U, DFR_FMA(s.m[1], V, s.m[2]));
+    const double b = DFR_FMA(s.m[3], U, DFR_FMA(s.m[4], V, s.m[5]));
+    const double c = DFR_FMA(s.m[6], U, DFR_FMA(s.m[7], V, s.m[8]));
     if (!(c > 0.0)) {
         x = y = NAN;
         return;

@@ -19,6 +19,7 @@
 //                         the exact/global-gather code of dfr_device.cuh.
 #include <cuda.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -34,6 +35,7 @@ namespace dfr {
 struct FitConsts {
     double W[4][4];            // monomial coefficients of the Lagrange basis: L_a(s) = sum_p W[p][a] s^p
     double pts[NPTS][2];       // sample points (s, t) in [-1, 1]^2; pixel offset = 16 s
+    double WW[16][16];         // WW[k][4q+p] = W[p][a_k] W[q][b_k]: node k -> coefficient of s^p t^q
 };
 
 static FitConsts make_fit_consts()
@@ -57,6 +59,9 @@ static FitConsts make_fit_consts()
             f.pts[4 * b + a][0] = s[a];
             f.pts[4 * b + a][1] = s[b];
         }
+    for (int k = 0; k < 16; ++k)
+        for (int q = 0; q < 4; ++q)
+            for (int pp = 0; pp < 4; ++pp) f.WW[k][4 * q + pp] = f.W[pp][k & 3] * f.W[q][k >> 2];
     const double h = 0.70710678118654752440;
     const double chk[9][2] = {{0, 0}, {h, h}, {-h, h}, {h, -h}, {-h, -h}, {1, 1}, {-1, 1}, {1, -1}, {-1, -1}};
     for (int k = 0; k < 9; ++k) {
@@ -82,96 +87,155 @@ target_nodes_kernel(const __grid_constant__ TargetDev tgt, const __grid_constant
     const int tx0 = (tile % tiles_x) * TS, ty0 = (tile / tiles_x) * TS;
     double U, V;
     target_uv(tgt, tx0 + kCentre + kHalf * fc.pts[k][0], ty0 + kCentre + kHalf * fc.pts[k][1], U, V);
-    uv[idx] = make_double2(U, V);
+    uv[(size_t)k * ntile + tile] = make_double2(U, V);      // [point][tile]: coalesced for the setup kernel
 }
 
+// Triangle size and row offset of an order-N packed polynomial (see Poly).
+__host__ __device__ constexpr int tri(int n) { return (n + 1) * (n + 2) / 2; }
+__host__ __device__ constexpr int tri_off(int n, int p) { return p * (n + 1) - (p * (p - 1)) / 2; }
+
+// a3-a6 with the exposure's constants in shared memory, SIP order fixed at compile time
+// (lower orders are zero-padded): sm = { m[9], c1, c2, ap[tri(N)], bp[tri(N)] }.
+// The reciprocal is a float seed + two Newton steps (c is O(1) for any valid point);
+// invalid points (c <= 0, NaN) come out as NaN.
+template <int N>
+__device__ __forceinline__ void source_xy_sm(const double *__restrict__ sm, double U, double V,
+                                             double &x, double &y)
+{
+    const double a = fma(sm[0], U, fma(sm[1], V, sm[2]));
+    const double b = fma(sm[3], U, fma(sm[4], V, sm[5]));
+    const double c = fma(sm[6], U, fma(sm[7], V, sm[8]));
+    float rf;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rf) : "f"((float)c));
+    double r = (double)rf;
+    r = r * fma(-c, r, 2.0);
+    r = r * fma(-c, r, 2.0);
+    if (!(c > 0.0)) r = __longlong_as_double(0x7ff8000000000000LL);
+    const double us = a * r, vs = b * r;
+    x = us + sm[9];
+    y = vs + sm[10];
+    if (N > 0) {
+        x += poly_eval_fixed<N>(sm + 11, us, vs);
+        y += poly_eval_fixed<N>(sm + 11 + tri(N), us, vs);
+    }
+}
+
+// One thread per (tile, exposure); a block is 128 consecutive tiles of ONE exposure so the
+// exposure's constants are staged once in shared memory and every coefficient read is a
+// broadcast LDS. The cubic is fitted separably: along s within each node row, then along t.
+template <int N>
 __global__ void __launch_bounds__(128)
 tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ srcdev,
-                  const __grid_constant__ FitConsts fc, int n, int ntile, int sny, int snx,
+                  const __grid_constant__ FitConsts fc, int e0, int ntile, int sny, int snx,
                   TileRec *__restrict__ recs, int32_t *__restrict__ counters)
 {
-    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool live = idx < (long long)n * ntile;
-    int flag = -1;
-    if (live) {
-        const int e = (int)(idx % n), tile = (int)(idx / n);   // lanes of a warp: same tile, different exposure
+    __shared__ double sm[11 + 2 * tri(N)];
+    const int e = e0 + blockIdx.y;
+    {
         const SourceDev &s = srcdev[e];
-        const double2 *p = uv + (size_t)tile * NPTS;
-        double Cx[4][4], Cy[4][4];
+        for (int k = threadIdx.x; k < 11 + 2 * tri(N); k += blockDim.x) {
+            double v;
+            if (k < 9) v = s.m[k];
+            else if (k == 9) v = s.c1;
+            else if (k == 10) v = s.c2;
+            else {
+                // slot of the order-N layout -> (p, q) -> slot of the stored order-n layout
+                const int t = (k - 11) % tri(N);
+                const Poly &P = (k - 11) < tri(N) ? s.ap : s.bp;
+                int p = 0;
+                while (p < N && tri_off(N, p + 1) <= t) ++p;
+                const int q = t - tri_off(N, p), n = P.order;
+                v = (p + q <= n) ? P.c[tri_off(n, p) + q] : 0.0;
+            }
+            sm[k] = v;
+        }
+    }
+    __syncthreads();
+    const int tile = blockIdx.x * blockDim.x + threadIdx.x;
+    int flag = -1;
+    if (tile < ntile) {
+        const double2 *p = uv + tile;
+        double Rx[4][4], Ry[4][4];                  // [node row b][power of s]
+        double nanacc = 0.0;
 #pragma unroll
-        for (int a = 0; a < 4; ++a)
+        for (int b = 0; b < 4; ++b) {
+            double xs[4], ys[4];
 #pragma unroll
-            for (int b = 0; b < 4; ++b) Cx[a][b] = Cy[a][b] = 0.0;
-        bool finite = true;
+            for (int a = 0; a < 4; ++a) {
+                const double2 q = p[(size_t)(4 * b + a) * ntile];
+                source_xy_sm<N>(sm, q.x, q.y, xs[a], ys[a]);
+                nanacc = fma(xs[a], 0.0, fma(ys[a], 0.0, nanacc));
+            }
+#pragma unroll
+            for (int pp = 0; pp < 4; ++pp) {
+                Rx[b][pp] = fma(fc.W[pp][0], xs[0], fma(fc.W[pp][1], xs[1], fma(fc.W[pp][2], xs[2], fc.W[pp][3] * xs[3])));
+                Ry[b][pp] = fma(fc.W[pp][0], ys[0], fma(fc.W[pp][1], ys[1], fma(fc.W[pp][2], ys[2], fc.W[pp][3] * ys[3])));
+            }
+        }
+        double Cx[16], Cy[16];                      // [4q + p]: coefficient of s^p t^q
+#pragma unroll
+        for (int qq = 0; qq < 4; ++qq)
+#pragma unroll
+            for (int pp = 0; pp < 4; ++pp) {
+                Cx[4 * qq + pp] = fma(fc.W[qq][0], Rx[0][pp], fma(fc.W[qq][1], Rx[1][pp], fma(fc.W[qq][2], Rx[2][pp], fc.W[qq][3] * Rx[3][pp])));
+                Cy[4 * qq + pp] = fma(fc.W[qq][0], Ry[0][pp], fma(fc.W[qq][1], Ry[1][pp], fma(fc.W[qq][2], Ry[2][pp], fc.W[qq][3] * Ry[3][pp])));
+            }
+        // verify the fit against the exact map at 9 other points (centre, T4 extrema,
+        // corners); the corners and the centre also bound the tile's source footprint
+        bool good = true;
         double xmin = 1e300, xmax = -1e300, ymin = 1e300, ymax = -1e300;
 #pragma unroll
-        for (int k = 0; k < 16; ++k) {
-            const double2 q = p[k];
-            double x, y;
-            source_xy(s, q.x, q.y, x, y);
-            finite = finite && isfinite(x) && isfinite(y);
-            xmin = fmin(xmin, x); xmax = fmax(xmax, x);
-            ymin = fmin(ymin, y); ymax = fmax(ymax, y);
-            const int a = k & 3, b = k >> 2;
-#pragma unroll
-            for (int pp = 0; pp < 4; ++pp)
-#pragma unroll
-                for (int qq = 0; qq < 4; ++qq) {
-                    const double w = fc.W[pp][a] * fc.W[qq][b];
-                    Cx[pp][qq] = fma(w, x, Cx[pp][qq]);
-                    Cy[pp][qq] = fma(w, y, Cy[pp][qq]);
-                }
-        }
-        // verify the fit against the exact map at 9 other points (centre, T4 extrema, corners)
-        double resid = 0.0;
         for (int k = 16; k < NPTS; ++k) {
-            const double2 q = p[k];
+            const double2 q = p[(size_t)k * ntile];
             double x, y;
-            source_xy(s, q.x, q.y, x, y);
-            finite = finite && isfinite(x) && isfinite(y);
-            xmin = fmin(xmin, x); xmax = fmax(xmax, x);
-            ymin = fmin(ymin, y); ymax = fmax(ymax, y);
+            source_xy_sm<N>(sm, q.x, q.y, x, y);
             const double ss = fc.pts[k][0], tt = fc.pts[k][1];
             double px = 0.0, py = 0.0;
 #pragma unroll
             for (int qq = 3; qq >= 0; --qq) {
-                const double rx = fma(fma(fma(Cx[3][qq], ss, Cx[2][qq]), ss, Cx[1][qq]), ss, Cx[0][qq]);
-                const double ry = fma(fma(fma(Cy[3][qq], ss, Cy[2][qq]), ss, Cy[1][qq]), ss, Cy[0][qq]);
+                const double rx = fma(fma(fma(Cx[4 * qq + 3], ss, Cx[4 * qq + 2]), ss, Cx[4 * qq + 1]), ss, Cx[4 * qq]);
+                const double ry = fma(fma(fma(Cy[4 * qq + 3], ss, Cy[4 * qq + 2]), ss, Cy[4 * qq + 1]), ss, Cy[4 * qq]);
                 px = fma(px, tt, rx);
                 py = fma(py, tt, ry);
             }
-            resid = fmax(resid, fmax(fabs(px - x), fabs(py - y)));
+            good = good && (fabs(px - x) <= (double)FIT_TOL) && (fabs(py - y) <= (double)FIT_TOL);   // false on NaN
+            if (k == 16 || k >= 21) {
+                xmin = fmin(xmin, x); xmax = fmax(xmax, x);
+                ymin = fmin(ymin, y); ymax = fmax(ymax, y);
+            }
         }
+        const bool finite = good && (nanacc == 0.0);
         TileRec r;
         r.pad_ = 0;
         flag = TILE_EXACT;
         r.ix0 = r.iy0 = r.bx0 = r.by0 = r.bx1 = r.by1 = 0;
         if (finite && fabs(xmin) < 1e9 && fabs(xmax) < 1e9 && fabs(ymin) < 1e9 && fabs(ymax) < 1e9) {
-            const double bx = floor(Cx[0][0]), by = floor(Cy[0][0]);
+            const double bx = floor(Cx[0]), by = floor(Cy[0]);
             r.ix0 = (int)bx; r.iy0 = (int)by;
             r.bx0 = (int)floor(xmin); r.bx1 = (int)floor(xmax);
             r.by0 = (int)floor(ymin); r.by1 = (int)floor(ymax);
             const bool small = (r.bx1 - r.bx0) < 2048 && (r.by1 - r.by0) < 2048 &&
                                abs(r.bx0 - r.ix0) < 2048 && abs(r.bx1 - r.ix0) < 2048 &&
                                abs(r.by0 - r.iy0) < 2048 && abs(r.by1 - r.iy0) < 2048;
-            if (resid <= (double)FIT_TOL && small) {
+            if (small) {
                 // outside the footprint [-0.5, n-0.5) by a 2 px margin on one side => all NaN
                 const bool out = (xmax + 2.0 < -0.5) || (xmin - 2.0 >= snx - 0.5) ||
                                  (ymax + 2.0 < -0.5) || (ymin - 2.0 >= sny - 0.5);
                 flag = out ? TILE_EMPTY : TILE_FAST;
             }
-            Cx[0][0] -= bx;
-            Cy[0][0] -= by;
+            Cx[0] -= bx;
+            Cy[0] -= by;
         }
         r.flag = flag;
+        // s = di / 16: coefficient of di^p dj^q is C[p][q] / 16^(p+q)
         double sq = 1.0;
 #pragma unroll
         for (int qq = 0; qq < 4; ++qq) {
             double sp = sq;
 #pragma unroll
             for (int pp = 0; pp < 4; ++pp) {
-                r.cx[4 * qq + pp] = (float)(Cx[pp][qq] * sp);
-                r.cy[4 * qq + pp] = (float)(Cy[pp][qq] * sp);
+                r.cx[4 * qq + pp] = (float)(Cx[4 * qq + pp] * sp);
+                r.cy[4 * qq + pp] = (float)(Cy[4 * qq + pp] * sp);
                 sp *= 1.0 / kHalf;
             }
             sq *= 1.0 / kHalf;
@@ -250,33 +314,92 @@ __device__ __noinline__ float exact_pixel(const float *__restrict__ img, int sny
     return sample_global<ORDER>(img, sny, snx, x, y);
 }
 
-// Gather + interpolate from a dense [..][pitch] float array whose element (0,0) is the
-// first tap of base index (k_x, k_y) = (0, 0).
-template <int ORDER, typename Ptr>
-__device__ __forceinline__ float gather(Ptr base, int pitch, int kx, int ky, float fx, float fy)
+// Where the fast path gathers from: the TMA-staged box in shared memory (STAGE) or the
+// source image itself (no staging). Shared loads use 32-bit shared-window addresses so
+// the address arithmetic is one IMAD + one LEA per pixel.
+template <bool STAGE> struct GatherSrc {
+    int pitch;                       // floats per row
+    uint32_t sbase;                  // STAGE: shared address of element (0, 0)
+    const float *gbase;              // !STAGE: global address of element (0, 0)
+};
+
+__device__ __forceinline__ float lds_f32(uint32_t a)
 {
-    Ptr p = base + ky * pitch + kx;
-    if (ORDER == DFR_NEAREST) return p[0];
-    if (ORDER == DFR_BILINEAR) {
-        const float s00 = p[0], s10 = p[1], s01 = p[pitch], s11 = p[pitch + 1];
-        const float top = fmaf(fx, s10 - s00, s00);
-        const float bot = fmaf(fx, s11 - s01, s01);
-        return fmaf(fy, bot - top, top);
-    }
-    float wx[4], wy[4];
-    keys_weights(fx, wx);
-    keys_weights(fy, wy);
-    float acc = 0.0f;
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ float lds_f32_4(uint32_t a)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v) : "r"(a));
+    return v;
+}
+
+// One pixel of a FAST tile: floor/rint by a magic add, range test, gather, interpolate.
+// `ok` = every tap is inside the image and inside the staged box; when it is false the
+// loads are redirected to element (0, 0) and the value is discarded by the caller.
+template <int ORDER, bool STAGE>
+__device__ __forceinline__ float fast_pixel(const GatherSrc<STAGE> &G, float xl, float yl, int Cx, int Cy,
+                                            unsigned cntx, unsigned cnty, bool &ok)
+{
+    float Tx, Ty;
+    if (ORDER == DFR_NEAREST) { Tx = xl + kMagic; Ty = yl + kMagic; }             // rint (half-even)
+    else { Tx = __fadd_rd(xl, kMagic); Ty = __fadd_rd(yl, kMagic); }               // floor
+    const float fx = xl - (Tx - kMagic), fy = yl - (Ty - kMagic);
+    const int kx = __float_as_int(Tx) - Cx, ky = __float_as_int(Ty) - Cy;
+    ok = ((unsigned)kx < cntx) && ((unsigned)ky < cnty);
+    const int idx = ok ? ky * G.pitch + kx : 0;
+    if (STAGE) {
+        const uint32_t a0 = G.sbase + 4u * (unsigned)idx;
+        if (ORDER == DFR_NEAREST) return lds_f32(a0);
+        const uint32_t p4 = 4u * (unsigned)G.pitch;
+        if (ORDER == DFR_BILINEAR) {
+            const uint32_t a1 = a0 + p4;
+            const float s00 = lds_f32(a0), s10 = lds_f32_4(a0), s01 = lds_f32(a1), s11 = lds_f32_4(a1);
+            const float top = fmaf(fx, s10 - s00, s00);
+            const float bot = fmaf(fx, s11 - s01, s01);
+            return fmaf(fy, bot - top, top);
+        }
+        float wx[4], wy[4];
+        keys_weights(fx, wx);
+        keys_weights(fy, wy);
+        float acc = 0.0f;
+        uint32_t a = a0;
 #pragma unroll
-    for (int m = 0; m < 4; ++m) {
-        Ptr r = p + m * pitch;
-        float row = wx[0] * r[0];
-        row = fmaf(wx[1], r[1], row);
-        row = fmaf(wx[2], r[2], row);
-        row = fmaf(wx[3], r[3], row);
-        acc = fmaf(wy[m], row, acc);
+        for (int m = 0; m < 4; ++m) {
+            float row = wx[0] * lds_f32(a);
+            row = fmaf(wx[1], lds_f32_4(a), row);
+            row = fmaf(wx[2], lds_f32(a + 8), row);
+            row = fmaf(wx[3], lds_f32_4(a + 8), row);
+            acc = fmaf(wy[m], row, acc);
+            a += p4;
+        }
+        return acc;
+    } else {
+        const float *__restrict__ p = G.gbase + idx;
+        if (ORDER == DFR_NEAREST) return __ldg(p);
+        if (ORDER == DFR_BILINEAR) {
+            const float s00 = __ldg(p), s10 = __ldg(p + 1), s01 = __ldg(p + G.pitch), s11 = __ldg(p + G.pitch + 1);
+            const float top = fmaf(fx, s10 - s00, s00);
+            const float bot = fmaf(fx, s11 - s01, s01);
+            return fmaf(fy, bot - top, top);
+        }
+        float wx[4], wy[4];
+        keys_weights(fx, wx);
+        keys_weights(fy, wy);
+        float acc = 0.0f;
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+            const float *__restrict__ q = p + m * G.pitch;
+            float row = wx[0] * __ldg(q);
+            row = fmaf(wx[1], __ldg(q + 1), row);
+            row = fmaf(wx[2], __ldg(q + 2), row);
+            row = fmaf(wx[3], __ldg(q + 3), row);
+            acc = fmaf(wy[m], row, acc);
+        }
+        return acc;
     }
-    return acc;
 }
 
 // ---------------------------------------------------------------------------------
@@ -358,20 +481,19 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
 
     const int tx0 = ttx * TS, ty0 = tty * TS;
     const int col = tx0 + lane;
-    const bool col_ok = col < P.onx;
+    if (col >= P.onx) return;           // ragged right edge (no block-level sync below)
     const int rows = min(TS, P.ony - ty0);
     float *__restrict__ orow = P.out + ((size_t)e * P.ony + ty0) * P.onx + col;
     const float *__restrict__ img = P.src + (size_t)e * P.sny * P.snx;
+    const size_t opitch = (size_t)P.onx;
 
     if (flag == TILE_EMPTY) {
-        if (col_ok)
-            for (int r = 0; r < rows; ++r) orow[(size_t)r * P.onx] = qnanf();
+        for (int r = 0; r < rows; ++r) orow[r * opitch] = qnanf();
         return;
     }
     if (flag == TILE_EXACT) {
-        if (col_ok)
-            for (int r = 0; r < rows; ++r)
-                orow[(size_t)r * P.onx] = exact_pixel<ORDER>(img, P.sny, P.snx, tgt, P.srcdev[e], col, ty0 + r);
+        for (int r = 0; r < rows; ++r)
+            orow[r * opitch] = exact_pixel<ORDER>(img, P.sny, P.snx, tgt, P.srcdev[e], col, ty0 + r);
         return;
     }
 
@@ -396,32 +518,56 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
         axis_range<ORDER>(P.snx, -(1 << 28), 1 << 30, Alx, Ahx);
         axis_range<ORDER>(P.sny, -(1 << 28), 1 << 30, Aly, Ahy);
     }
-    const int pitch = STAGE ? P.BW : P.snx;
     const unsigned cntx = (unsigned)max(Ahx - Alx + 1, 0), cnty = (unsigned)max(Ahy - Aly + 1, 0);
     const int Cx = kMagicBits - ix0 + Alx, Cy = kMagicBits - iy0 + Aly;
-    // element (k = 0) of the gather array = first tap of base index (Alx, Aly)
+    // gather array: element (k = 0) = first tap of base index (Alx, Aly)
     const int tlo = (ORDER == DFR_BICUBIC) ? 1 : 0;
-    const float *__restrict__ gbase = img + ((long long)(Aly - tlo) * P.snx + (Alx - tlo));
-    const float *sbase = box + ((Aly - tlo - oy) * P.BW + (Alx - tlo - ox));
+    GatherSrc<STAGE> G;
+    if (STAGE) {
+        G.pitch = P.BW;
+        G.sbase = smem_u32(box) + 4u * (unsigned)((Aly - tlo - oy) * P.BW + (Alx - tlo - ox));
+        G.gbase = nullptr;
+    } else {
+        G.pitch = P.snx;
+        G.sbase = 0;
+        G.gbase = img + ((long long)(Aly - tlo) * P.snx + (Alx - tlo));
+    }
 
-#pragma unroll 4
-    for (int r = 0; r < rows; ++r) {
-        const float dj = (float)r - (float)kCentre;
-        const float xl = fmaf(fmaf(fmaf(X[3], dj, X[2]), dj, X[1]), dj, X[0]);
-        const float yl = fmaf(fmaf(fmaf(Y[3], dj, Y[2]), dj, Y[1]), dj, Y[0]);
-        float Tx, Ty;
-        if (ORDER == DFR_NEAREST) { Tx = xl + kMagic; Ty = yl + kMagic; }          // rint (half-even)
-        else { Tx = __fadd_rd(xl, kMagic); Ty = __fadd_rd(yl, kMagic); }            // floor
-        const float fx = xl - (Tx - kMagic), fy = yl - (Ty - kMagic);
-        const int kx = __float_as_int(Tx) - Cx, ky = __float_as_int(Ty) - Cy;
-        float val;
-        if ((unsigned)kx < cntx && (unsigned)ky < cnty) {
-            if (STAGE) val = gather<ORDER, const float *>(sbase, pitch, kx, ky, fx, fy);
-            else val = gather<ORDER, const float *__restrict__>(gbase, pitch, kx, ky, fx, fy);
-        } else {
-            val = slow_poly_pixel<ORDER>(img, P.sny, P.snx, ix0, iy0, xl, yl);
+    constexpr int U = 4;                      // rows in flight per thread
+    float dj = -(float)kCentre;
+    int r = 0;
+    for (; r + U <= rows; r += U) {
+        float xl[U], yl[U], val[U];
+        bool ok[U];
+#pragma unroll
+        for (int k = 0; k < U; ++k) {
+            const float d = dj + (float)k;
+            xl[k] = fmaf(fmaf(fmaf(X[3], d, X[2]), d, X[1]), d, X[0]);
+            yl[k] = fmaf(fmaf(fmaf(Y[3], d, Y[2]), d, Y[1]), d, Y[0]);
+            val[k] = fast_pixel<ORDER, STAGE>(G, xl[k], yl[k], Cx, Cy, cntx, cnty, ok[k]);
         }
-        if (col_ok) orow[(size_t)r * P.onx] = val;
+        bool all_ok = true;
+#pragma unroll
+        for (int k = 0; k < U; ++k) all_ok = all_ok && ok[k];
+        if (!all_ok) {                        // rare: image rim, outside the staged box, NaN
+#pragma unroll
+            for (int k = 0; k < U; ++k)
+                if (!ok[k]) val[k] = slow_poly_pixel<ORDER>(img, P.sny, P.snx, ix0, iy0, xl[k], yl[k]);
+        }
+#pragma unroll
+        for (int k = 0; k < U; ++k) orow[k * opitch] = val[k];
+        orow += U * opitch;
+        dj += (float)U;
+    }
+    for (; r < rows; ++r) {                   // ragged bottom edge
+        const float xs = fmaf(fmaf(fmaf(X[3], dj, X[2]), dj, X[1]), dj, X[0]);
+        const float ys = fmaf(fmaf(fmaf(Y[3], dj, Y[2]), dj, Y[1]), dj, Y[0]);
+        bool ok1;
+        float v = fast_pixel<ORDER, STAGE>(G, xs, ys, Cx, Cy, cntx, cnty, ok1);
+        if (!ok1) v = slow_poly_pixel<ORDER>(img, P.sny, P.snx, ix0, iy0, xs, ys);
+        *orow = v;
+        orow += opitch;
+        dj += 1.0f;
     }
 }
 
@@ -497,37 +643,33 @@ static EncodeTiledFn get_encode()
 
 constexpr int kMaxBoxBytes = 36 * 1024;          // keeps >= 6 CTAs (24 warps) per SM
 
-// Source-pixel extent of a 64x64 output tile, probed in fp64 on the host at the centre and
-// corners of the output grid for (a sample of) the exposures. Returns false if no probe is finite.
+// Source-pixel extent of a 64x64 output tile, from the Jacobian of the map probed in fp64
+// on the host at the centre of the output grid, per exposure (3 map evaluations each; the
+// Jacobian varies by well under 1 % over a frame, the caller adds 2 % + fixed margins, and
+// the kernel checks every pixel against the staged box anyway). False if no probe is finite.
 static bool probe_extent(const TargetDev &tgt, const SourceDev *hs, int n, int ony, int onx,
                          double &ext_x, double &ext_y)
 {
-    const int span = TS * CTA_T;
-    const double px[5] = {0.0, (double)std::max(onx - span, 0), 0.0, (double)std::max(onx - span, 0),
-                          std::max(0.5 * (onx - span), 0.0)};
-    const double py[5] = {0.0, 0.0, (double)std::max(ony - span, 0), (double)std::max(ony - span, 0),
-                          std::max(0.5 * (ony - span), 0.0)};
-    const int step = n > 64 ? n / 64 : 1;
+    const double span = TS * CTA_T - 1;
+    const double ci = 0.5 * (onx - 1), cj = 0.5 * (ony - 1), h = 16.0;
+    double U0, V0, U1, V1, U2, V2;
+    target_uv(tgt, ci, cj, U0, V0);
+    target_uv(tgt, ci + h, cj, U1, V1);
+    target_uv(tgt, ci, cj + h, U2, V2);
+    const int step = n > 256 ? n / 256 : 1;
     bool any = false;
     ext_x = ext_y = 0.0;
-    for (int e = 0; e < n; e += step)
-        for (int k = 0; k < 5; ++k) {
-            double xmin = 1e300, xmax = -1e300, ymin = 1e300, ymax = -1e300;
-            bool fin = true;
-            for (int c = 0; c < 9; ++c) {
-                const double i = px[k] + (c % 3) * 0.5 * (span - 1), j = py[k] + (c / 3) * 0.5 * (span - 1);
-                double U, V, x, y;
-                target_uv(tgt, i, j, U, V);
-                source_xy(hs[e], U, V, x, y);
-                fin = fin && std::isfinite(x) && std::isfinite(y);
-                xmin = std::fmin(xmin, x); xmax = std::fmax(xmax, x);
-                ymin = std::fmin(ymin, y); ymax = std::fmax(ymax, y);
-            }
-            if (!fin) continue;
-            any = true;
-            ext_x = std::fmax(ext_x, xmax - xmin);
-            ext_y = std::fmax(ext_y, ymax - ymin);
-        }
+    for (int e = 0; e < n; e += step) {
+        double x0, y0, x1, y1, x2, y2;
+        source_xy(hs[e], U0, V0, x0, y0);
+        source_xy(hs[e], U1, V1, x1, y1);
+        source_xy(hs[e], U2, V2, x2, y2);
+        const double jxx = (x1 - x0) / h, jxy = (x2 - x0) / h, jyx = (y1 - y0) / h, jyy = (y2 - y0) / h;
+        if (!(std::isfinite(jxx) && std::isfinite(jxy) && std::isfinite(jyx) && std::isfinite(jyy))) continue;
+        any = true;
+        ext_x = std::fmax(ext_x, span * (std::fabs(jxx) + std::fabs(jxy)));
+        ext_y = std::fmax(ext_y, span * (std::fabs(jyx) + std::fabs(jyy)));
+    }
     return any;
 }
 
@@ -552,8 +694,8 @@ struct Scratch {
 };
 
 static cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const SourceDev *srcdev,
-                             int ony, int onx, cudaStream_t st, int32_t *counters, Scratch &sc,
-                             TiledParams &P)
+                             const SourceDev *srchost, int ony, int onx, cudaStream_t st,
+                             int32_t *counters, Scratch &sc, TiledParams &P)
 {
     static const FitConsts fc = make_fit_consts();
     P.n = n; P.sny = sny; P.snx = snx; P.ony = ony; P.onx = onx;
@@ -570,10 +712,19 @@ static cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, cons
     if (counters && (err = cudaMemsetAsync(counters, 0, 3 * sizeof(int32_t), st)) != cudaSuccess) return err;
     target_nodes_kernel<<<(ntile * NPTS + 127) / 128, 128, 0, st>>>(tgt, fc, P.tiles_x, ntile, sc.uv);
     if ((err = cudaGetLastError()) != cudaSuccess) return err;
-    const long long work = (long long)ntile * n;
-    tile_setup_kernel<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(sc.uv, srcdev, fc, n, ntile, sny, snx,
-                                                                      sc.recs, counters);
-    return cudaGetLastError();
+    // SIP order class of the batch: inverse polynomials are zero-padded up to N
+    int maxo = 0;
+    for (int e = 0; e < n; ++e) maxo = std::max(maxo, std::max(srchost[e].ap.order, srchost[e].bp.order));
+    const unsigned bx = (unsigned)((ntile + 127) / 128);
+    for (int e0 = 0; e0 < n; e0 += 65535) {
+        const dim3 grid(bx, (unsigned)std::min(n - e0, 65535));
+        if (maxo == 0) tile_setup_kernel<0><<<grid, 128, 0, st>>>(sc.uv, srcdev, fc, e0, ntile, sny, snx, sc.recs, counters);
+        else if (maxo <= 3) tile_setup_kernel<3><<<grid, 128, 0, st>>>(sc.uv, srcdev, fc, e0, ntile, sny, snx, sc.recs, counters);
+        else if (maxo <= 5) tile_setup_kernel<5><<<grid, 128, 0, st>>>(sc.uv, srcdev, fc, e0, ntile, sny, snx, sc.recs, counters);
+        else tile_setup_kernel<9><<<grid, 128, 0, st>>>(sc.uv, srcdev, fc, e0, ntile, sny, snx, sc.recs, counters);
+        if ((err = cudaGetLastError()) != cudaSuccess) return err;
+    }
+    return cudaSuccess;
 }
 
 static void free_scratch(Scratch &sc, cudaStream_t st)
@@ -594,7 +745,7 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
     P.out = out;
     Scratch sc;
     if (prof && prof->enabled) cudaEventRecord(prof->setup_begin, st);
-    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, ony, onx, st, dev_counters, sc, P);
+    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, srchost, ony, onx, st, dev_counters, sc, P);
     if (err != cudaSuccess) { free_scratch(sc, st); return err; }
 
     // ---- staging decision: box size from a host probe; TMA needs 16-byte rows
@@ -637,14 +788,14 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
 }
 
 cudaError_t launch_tiled_coords(int n, int sny, int snx, const TargetDev &tgt,
-                                const SourceDev *srcdev, int ony, int onx, int order,
+                                const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx, int order,
                                 double *x, double *y, cudaStream_t st)
 {
     (void)order;
     TiledParams P;
     std::memset(&P, 0, sizeof P);
     Scratch sc;
-    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, ony, onx, st, nullptr, sc, P);
+    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, srchost, ony, onx, st, nullptr, sc, P);
     if (err == cudaSuccess) {
         const long long blocks = (long long)P.ctas_x * P.ctas_y * n;
         tiled_coords_kernel<<<(unsigned)blocks, 32 * CTA_T * CTA_T, 0, st>>>(P, tgt, x, y);

@@ -42,7 +42,7 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
                                    int32_t *dev_counters /* 3 ints, zeroed here */,
                                    TiledStats *stats, ProfileEvents *prof);
 cudaError_t launch_tiled_coords(int n, int sny, int snx, const TargetDev &tgt,
-                                const SourceDev *srcdev, int ony, int onx, int order,
+                                const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx, int order,
                                 double *x, double *y, cudaStream_t st);
 
 }  // namespace dfr
