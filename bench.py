@@ -158,6 +158,7 @@ def main():
     import torch
     import torch.distributed as dist
     import paper_2505_03932_b200 as P
+    from paper_2505_03932_b200.shard import max_over_ranks
     P.lib()                                    # fail loudly if the CUDA library is missing
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
@@ -213,10 +214,7 @@ def main():
     if rank == 0:
         time.sleep(0.2)
         sampler.stop()
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, device="cuda")
     value = out_mpix * world * args.steps / (total_ms * 1e-3)
 
     # ---- dominant kernel, timed live by the library's own events on the launching stream
@@ -242,10 +240,8 @@ def main():
         for _ in range(args.e2e_steps):
             P.dfr_reproject_host(hsrc, ws_arr, tw, (NPIX, NPIX), P.BILINEAR, out_host=hout, batch=8)
         torch.cuda.synchronize()
-        el = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(el, op=dist.ReduceOp.MAX)
-        e2e = {"value": out_mpix * world * args.e2e_steps / float(el.item()), "unit": UNIT,
+        el = max_over_ranks(time.perf_counter() - t0, device="cuda")
+        e2e = {"value": out_mpix * world * args.e2e_steps / el, "unit": UNIT,
                "h2d_bytes_per_step": int(w.images.nbytes), "d2h_bytes_per_step": int(hout.numel() * 4),
                "steps": args.e2e_steps, "api": "dfr_reproject_host(batch=8), pinned host buffers"}
         same = bool(torch.equal(torch.nan_to_num(hout[:2], nan=-1.0), torch.nan_to_num(out[:2].cpu(), nan=-1.0)))
