@@ -180,10 +180,8 @@ tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ 
                 Cx[4 * qq + pp] = fma(fc.W[qq][0], Rx[0][pp], fma(fc.W[qq][1], Rx[1][pp], fma(fc.W[qq][2], Rx[2][pp], fc.W[qq][3] * Rx[3][pp])));
                 Cy[4 * qq + pp] = fma(fc.W[qq][0], Ry[0][pp], fma(fc.W[qq][1], Ry[1][pp], fma(fc.W[qq][2], Ry[2][pp], fc.W[qq][3] * Ry[3][pp])));
             }
-        // verify the fit against the exact map at 9 other points (centre, T4 extrema,
-        // corners); the corners and the centre also bound the tile's source footprint
+        // verify the fit against the exact map at 9 other points (centre, T4 extrema, corners)
         bool good = true;
-        double xmin = 1e300, xmax = -1e300, ymin = 1e300, ymax = -1e300;
 #pragma unroll
         for (int k = 16; k < NPTS; ++k) {
             const double2 q = p[(size_t)k * ntile];
@@ -199,11 +197,16 @@ tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ 
                 py = fma(py, tt, ry);
             }
             good = good && (fabs(px - x) <= (double)FIT_TOL) && (fabs(py - y) <= (double)FIT_TOL);   // false on NaN
-            if (k == 16 || k >= 21) {
-                xmin = fmin(xmin, x); xmax = fmax(xmax, x);
-                ymin = fmin(ymin, y); ymax = fmax(ymax, y);
-            }
         }
+        // Rigorous range of the fitted polynomial over the tile: |s|, |t| <= 31/32 < 1, so
+        // |x - C00| <= sum of the other |C_pq|. The main kernel evaluates exactly this
+        // polynomial (in fp32: + kBoxSlack), which is what makes its unchecked gathers safe.
+        double ex = 0.0, ey = 0.0;
+#pragma unroll
+        for (int k = 1; k < 16; ++k) { ex += fabs(Cx[k]); ey += fabs(Cy[k]); }
+        constexpr double kBoxSlack = 1e-3;
+        const double xmin = Cx[0] - ex - kBoxSlack, xmax = Cx[0] + ex + kBoxSlack;
+        const double ymin = Cy[0] - ey - kBoxSlack, ymax = Cy[0] + ey + kBoxSlack;
         const bool finite = good && (nanacc == 0.0);
         TileRec r;
         r.pad_ = 0;
@@ -266,7 +269,7 @@ struct TiledParams {
     float *out;
     const TileRec *recs;
     const SourceDev *srcdev;
-    int n, sny, snx, ony, onx;
+    int n, e0, sny, snx, ony, onx;                 // e0: first exposure of this launch
     int tiles_x, tiles_y, ctas_x, ctas_y;
     int BW, BH;                                    // staged box (STAGE) in source pixels
 };
@@ -403,6 +406,114 @@ __device__ __forceinline__ float fast_pixel(const GatherSrc<STAGE> &G, float xl,
 }
 
 // ---------------------------------------------------------------------------------
+// packed fp32 pairs (sm_100a FFMA2 / FADD2 / FMUL2): one issue slot for two pixels.
+// The main kernel is issue-bound, not FMA-pipe-bound (ncu, profiles/), so the rows of
+// an interior tile are walked two at a time with every FP step packed over the pair.
+// ---------------------------------------------------------------------------------
+typedef unsigned long long f32x2;
+
+__device__ __forceinline__ f32x2 pk2(float lo, float hi)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpk2(f32x2 v, float &lo, float &hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 add2_rm(f32x2 a, f32x2 b)      // round toward -inf
+{
+    f32x2 r;
+    asm("add.rm.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 splat2(float v) { return pk2(v, v); }
+
+// Keys weights (a = -0.75) on a packed pair of fractions; same formulas as keys_weights.
+__device__ __forceinline__ void keys_weights2(f32x2 t, f32x2 w[4])
+{
+    const float A = -0.75f;
+    const f32x2 one = splat2(1.0f);
+    const f32x2 t1 = add2(t, one), s = sub2(one, t), s1 = sub2(splat2(2.0f), t);
+    w[0] = fma2(fma2(fma2(splat2(A), t1, splat2(-5.0f * A)), t1, splat2(8.0f * A)), t1, splat2(-4.0f * A));
+    w[1] = fma2(fma2(splat2(A + 2.0f), t, splat2(-(A + 3.0f))), mul2(t, t), one);
+    w[2] = fma2(fma2(splat2(A + 2.0f), s, splat2(-(A + 3.0f))), mul2(s, s), one);
+    w[3] = fma2(fma2(fma2(splat2(A), s1, splat2(-5.0f * A)), s1, splat2(8.0f * A)), s1, splat2(-4.0f * A));
+}
+
+// Two rows (dj, dj + 1) of an INTERIOR tile of a STAGE kernel: every tap of every pixel is
+// inside the image and inside the staged box (bounded rigorously by the tile record), so
+// there is no range test and no address guard. K folds the shared base address and both
+// index biases: address of the first tap = Ty_bits * pitch4 + Tx_bits * 4 + K (mod 2^32).
+template <int ORDER>
+__device__ __forceinline__ f32x2 interior_pair(const f32x2 (&X)[4], const f32x2 (&Y)[4], f32x2 d,
+                                               uint32_t pitch4, uint32_t K)
+{
+    const f32x2 xl = fma2(fma2(fma2(X[3], d, X[2]), d, X[1]), d, X[0]);
+    const f32x2 yl = fma2(fma2(fma2(Y[3], d, Y[2]), d, Y[1]), d, Y[0]);
+    const f32x2 magic = splat2(kMagic);
+    f32x2 Tx, Ty;
+    if (ORDER == DFR_NEAREST) { Tx = add2(xl, magic); Ty = add2(yl, magic); }          // rint (half-even)
+    else { Tx = add2_rm(xl, magic); Ty = add2_rm(yl, magic); }                           // floor
+    float txa, txb, tya, tyb;
+    unpk2(Tx, txa, txb);
+    unpk2(Ty, tya, tyb);
+    const uint32_t aA = __float_as_uint(tya) * pitch4 + K + (__float_as_uint(txa) << 2);
+    const uint32_t aB = __float_as_uint(tyb) * pitch4 + K + (__float_as_uint(txb) << 2);
+    if (ORDER == DFR_NEAREST) return pk2(lds_f32(aA), lds_f32(aB));
+    const f32x2 fx = sub2(xl, sub2(Tx, magic)), fy = sub2(yl, sub2(Ty, magic));
+    if (ORDER == DFR_BILINEAR) {
+        const uint32_t a1A = aA + pitch4, a1B = aB + pitch4;
+        const f32x2 s00 = pk2(lds_f32(aA), lds_f32(aB)), s10 = pk2(lds_f32_4(aA), lds_f32_4(aB));
+        const f32x2 s01 = pk2(lds_f32(a1A), lds_f32(a1B)), s11 = pk2(lds_f32_4(a1A), lds_f32_4(a1B));
+        const f32x2 top = fma2(fx, sub2(s10, s00), s00);
+        const f32x2 bot = fma2(fx, sub2(s11, s01), s01);
+        return fma2(fy, sub2(bot, top), top);
+    }
+    f32x2 wx[4], wy[4];
+    keys_weights2(fx, wx);
+    keys_weights2(fy, wy);
+    f32x2 acc = 0ull;                                   // (+0.0f, +0.0f)
+    uint32_t a = aA, b = aB;
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+        f32x2 row = mul2(wx[0], pk2(lds_f32(a), lds_f32(b)));
+        row = fma2(wx[1], pk2(lds_f32_4(a), lds_f32_4(b)), row);
+        row = fma2(wx[2], pk2(lds_f32(a + 8), lds_f32(b + 8)), row);
+        row = fma2(wx[3], pk2(lds_f32_4(a + 8), lds_f32_4(b + 8)), row);
+        acc = fma2(wy[m], row, acc);
+        a += pitch4;
+        b += pitch4;
+    }
+    return acc;
+}
+
+// ---------------------------------------------------------------------------------
 // main kernel: one CTA per 64x64 output tile per exposure, one warp per 32x32 tile
 // ---------------------------------------------------------------------------------
 template <int ORDER, bool STAGE>
@@ -416,11 +527,8 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
     __shared__ int s_box[3];
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int ctas = P.ctas_x * P.ctas_y;
-    const int e = blockIdx.x / ctas;
-    const int rem = blockIdx.x - e * ctas;
-    const int cty = rem / P.ctas_x, ctx = rem - cty * P.ctas_x;
-    const int ttx = ctx * CTA_T + (warp % CTA_T), tty = cty * CTA_T + (warp / CTA_T);
+    const int e = P.e0 + blockIdx.z;                  // grid = (ctas_x, ctas_y, exposures): no divisions
+    const int ttx = blockIdx.x * CTA_T + (warp % CTA_T), tty = blockIdx.y * CTA_T + (warp / CTA_T);
     const bool active = ttx < P.tiles_x && tty < P.tiles_y;
     const int ntile = P.tiles_x * P.tiles_y;
     const TileRec *rec = P.recs + ((size_t)e * ntile + (active ? tty * P.tiles_x + ttx : 0));
@@ -536,6 +644,38 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
     constexpr int U = 4;                      // rows in flight per thread
     float dj = -(float)kCentre;
     int r = 0;
+    if (STAGE) {
+        // INTERIOR tile: the record's rigorous index range lies inside [Al, Ah] on both axes
+        // (image interior AND staged box), so no pixel needs a range test or the rim rule.
+        const int top = (ORDER == DFR_NEAREST) ? 1 : 0;          // rint(x) <= floor(x) + 1
+        const bool interior = bx0 >= Alx && bx1 + top <= Ahx && by0 >= Aly && by1 + top <= Ahy;
+        if (interior) {
+            f32x2 X2[4], Y2[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) { X2[q] = splat2(X[q]); Y2[q] = splat2(Y[q]); }
+            const uint32_t pitch4 = 4u * (unsigned)G.pitch;
+            const uint32_t K = G.sbase - pitch4 * (unsigned)Cy - 4u * (unsigned)Cx;
+            f32x2 d = pk2(dj, dj + 1.0f);
+            const f32x2 step = splat2(2.0f);
+            for (; r + U <= rows; r += U) {
+                f32x2 v[U / 2];
+#pragma unroll
+                for (int k = 0; k < U / 2; ++k) {
+                    v[k] = interior_pair<ORDER>(X2, Y2, d, pitch4, K);
+                    d = add2(d, step);
+                }
+#pragma unroll
+                for (int k = 0; k < U / 2; ++k) {
+                    float lo, hi;
+                    unpk2(v[k], lo, hi);
+                    orow[(2 * k) * opitch] = lo;
+                    orow[(2 * k + 1) * opitch] = hi;
+                }
+                orow += U * opitch;
+            }
+            dj += (float)r;
+        }
+    }
     for (; r + U <= rows; r += U) {
         float xl[U], yl[U], val[U];
         bool ok[U];
@@ -577,11 +717,8 @@ tiled_coords_kernel(const __grid_constant__ TiledParams P, const __grid_constant
                     double *__restrict__ xo, double *__restrict__ yo)
 {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int ctas = P.ctas_x * P.ctas_y;
-    const int e = blockIdx.x / ctas;
-    const int rem = blockIdx.x - e * ctas;
-    const int cty = rem / P.ctas_x, ctx = rem - cty * P.ctas_x;
-    const int ttx = ctx * CTA_T + (warp % CTA_T), tty = cty * CTA_T + (warp / CTA_T);
+    const int e = P.e0 + blockIdx.z;
+    const int ttx = blockIdx.x * CTA_T + (warp % CTA_T), tty = blockIdx.y * CTA_T + (warp / CTA_T);
     if (!(ttx < P.tiles_x && tty < P.tiles_y)) return;
     const int ntile = P.tiles_x * P.tiles_y;
     const TileRec *rec = P.recs + ((size_t)e * ntile + tty * P.tiles_x + ttx);
@@ -682,10 +819,16 @@ static cudaError_t launch_main(const TiledParams &P, const TargetDev &tgt, const
         cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxBoxBytes);
         if (err != cudaSuccess) return err;
     }
-    const long long blocks = (long long)P.ctas_x * P.ctas_y * P.n;
-    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    kern<<<(unsigned)blocks, 32 * CTA_T * CTA_T, smem, st>>>(P, tgt, tmap);
-    return cudaGetLastError();
+    if (P.ctas_y > 65535) return cudaErrorInvalidConfiguration;
+    TiledParams Q = P;
+    for (int e0 = 0; e0 < P.n; e0 += 65535) {
+        Q.e0 = e0;
+        const dim3 grid((unsigned)P.ctas_x, (unsigned)P.ctas_y, (unsigned)std::min(P.n - e0, 65535));
+        kern<<<grid, 32 * CTA_T * CTA_T, smem, st>>>(Q, tgt, tmap);
+        const cudaError_t err = cudaGetLastError();
+        if (err != cudaSuccess) return err;
+    }
+    return cudaSuccess;
 }
 
 struct Scratch {
@@ -797,9 +940,12 @@ cudaError_t launch_tiled_coords(int n, int sny, int snx, const TargetDev &tgt,
     Scratch sc;
     cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, srchost, ony, onx, st, nullptr, sc, P);
     if (err == cudaSuccess) {
-        const long long blocks = (long long)P.ctas_x * P.ctas_y * n;
-        tiled_coords_kernel<<<(unsigned)blocks, 32 * CTA_T * CTA_T, 0, st>>>(P, tgt, x, y);
-        err = cudaGetLastError();
+        for (int e0 = 0; e0 < n && err == cudaSuccess; e0 += 65535) {
+            P.e0 = e0;
+            const dim3 grid((unsigned)P.ctas_x, (unsigned)P.ctas_y, (unsigned)std::min(n - e0, 65535));
+            tiled_coords_kernel<<<grid, 32 * CTA_T * CTA_T, 0, st>>>(P, tgt, x, y);
+            err = cudaGetLastError();
+        }
     }
     free_scratch(sc, st);
     return err;
