@@ -126,8 +126,9 @@ __device__ __forceinline__ void source_xy_sm(const double *__restrict__ sm, doub
 template <int N>
 __global__ void __launch_bounds__(128)
 tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ srcdev,
-                  const __grid_constant__ FitConsts fc, int e0, int ntile, int sny, int snx,
-                  TileRec *__restrict__ recs, int32_t *__restrict__ counters)
+                  const __grid_constant__ FitConsts fc, int e0, int ntile, int tiles_x, int ctas_x,
+                  int ctas, int sny, int snx, TileRec *__restrict__ recs, int2 *__restrict__ cta_box,
+                  int32_t *__restrict__ counters)
 {
     __shared__ double sm[11 + 2 * tri(N)];
     const int e = e0 + blockIdx.y;
@@ -208,8 +209,17 @@ tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ 
         const double xmin = Cx[0] - ex - kBoxSlack, xmax = Cx[0] + ex + kBoxSlack;
         const double ymin = Cy[0] - ey - kBoxSlack, ymax = Cy[0] + ey + kBoxSlack;
         const bool finite = good && (nanacc == 0.0);
+        // Degree of the per-lane column polynomials in dj: the t^2, t^3 terms (any power of s)
+        // are dropped by the main kernel when they cannot move a coordinate by kDegTol px.
+        double q2x = 0.0, q2y = 0.0, q3x = 0.0, q3y = 0.0;
+#pragma unroll
+        for (int pp = 0; pp < 4; ++pp) {
+            q2x += fabs(Cx[8 + pp]); q2y += fabs(Cy[8 + pp]);
+            q3x += fabs(Cx[12 + pp]); q3y += fabs(Cy[12 + pp]);
+        }
+        constexpr double kDegTol = 2.5e-7;
         TileRec r;
-        r.pad_ = 0;
+        r.deg = (fmax(q2x, q2y) < kDegTol && fmax(q3x, q3y) < kDegTol) ? 1 : 3;
         flag = TILE_EXACT;
         r.ix0 = r.iy0 = r.bx0 = r.by0 = r.bx1 = r.by1 = 0;
         if (finite && fabs(xmin) < 1e9 && fabs(xmax) < 1e9 && fabs(ymin) < 1e9 && fabs(ymax) < 1e9) {
@@ -225,6 +235,13 @@ tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ 
                 const bool out = (xmax + 2.0 < -0.5) || (xmin - 2.0 >= snx - 0.5) ||
                                  (ymax + 2.0 < -0.5) || (ymin - 2.0 >= sny - 0.5);
                 flag = out ? TILE_EMPTY : TILE_FAST;
+                if (flag == TILE_FAST) {
+                    // origin of the CTA tile's staged box = min over its FAST tiles
+                    const int tty = tile / tiles_x, ttx = tile - tty * tiles_x;
+                    int2 *cb = cta_box + ((size_t)e * ctas + (tty / CTA_T) * ctas_x + ttx / CTA_T);
+                    atomicMin(&cb->x, r.bx0);
+                    atomicMin(&cb->y, r.by0);
+                }
             }
             Cx[0] -= bx;
             Cy[0] -= by;
@@ -264,10 +281,13 @@ template <> struct Taps<DFR_NEAREST>  { static constexpr int lo = 0, hi = 1; }; 
 template <> struct Taps<DFR_BILINEAR> { static constexpr int lo = 0, hi = 1; };
 template <> struct Taps<DFR_BICUBIC>  { static constexpr int lo = 1, hi = 2; };
 
+constexpr int kNoBox = 0x7f7f7f7f;                 // cudaMemset(0x7f) pattern: no FAST tile in this CTA tile
+
 struct TiledParams {
     const float *src;
     float *out;
     const TileRec *recs;
+    const int2 *cta_box;                           // [n][ctas_y][ctas_x] box origin (kNoBox: none)
     const SourceDev *srcdev;
     int n, e0, sny, snx, ony, onx;                 // e0: first exposure of this launch
     int tiles_x, tiles_y, ctas_x, ctas_y;
@@ -470,12 +490,18 @@ __device__ __forceinline__ void keys_weights2(f32x2 t, f32x2 w[4])
 // inside the image and inside the staged box (bounded rigorously by the tile record), so
 // there is no range test and no address guard. K folds the shared base address and both
 // index biases: address of the first tap = Ty_bits * pitch4 + Tx_bits * 4 + K (mod 2^32).
-template <int ORDER>
+template <int ORDER, int DEG>
 __device__ __forceinline__ f32x2 interior_pair(const f32x2 (&X)[4], const f32x2 (&Y)[4], f32x2 d,
                                                uint32_t pitch4, uint32_t K)
 {
-    const f32x2 xl = fma2(fma2(fma2(X[3], d, X[2]), d, X[1]), d, X[0]);
-    const f32x2 yl = fma2(fma2(fma2(Y[3], d, Y[2]), d, Y[1]), d, Y[0]);
+    f32x2 xl, yl;
+    if (DEG == 1) {
+        xl = fma2(X[1], d, X[0]);
+        yl = fma2(Y[1], d, Y[0]);
+    } else {
+        xl = fma2(fma2(fma2(X[3], d, X[2]), d, X[1]), d, X[0]);
+        yl = fma2(fma2(fma2(Y[3], d, Y[2]), d, Y[1]), d, Y[0]);
+    }
     const f32x2 magic = splat2(kMagic);
     f32x2 Tx, Ty;
     if (ORDER == DFR_NEAREST) { Tx = add2(xl, magic); Ty = add2(yl, magic); }          // rint (half-even)
@@ -513,6 +539,33 @@ __device__ __forceinline__ f32x2 interior_pair(const f32x2 (&X)[4], const f32x2 
     return acc;
 }
 
+// All complete groups of U rows of an interior tile; advances r and orow.
+template <int ORDER, int DEG>
+__device__ __forceinline__ void interior_rows(const f32x2 (&X2)[4], const f32x2 (&Y2)[4], uint32_t pitch4,
+                                              uint32_t K, int rows, int &r, float *__restrict__ &orow,
+                                              size_t opitch)
+{
+    constexpr int U = (ORDER == DFR_BICUBIC) ? 2 : 4;           // rows in flight per thread
+    f32x2 d = pk2(-(float)kCentre, 1.0f - (float)kCentre);
+    const f32x2 step = splat2(2.0f);
+    for (; r + U <= rows; r += U) {
+        f32x2 v[U / 2];
+#pragma unroll
+        for (int k = 0; k < U / 2; ++k) {
+            v[k] = interior_pair<ORDER, DEG>(X2, Y2, d, pitch4, K);
+            d = add2(d, step);
+        }
+#pragma unroll
+        for (int k = 0; k < U / 2; ++k) {
+            float lo, hi;
+            unpk2(v[k], lo, hi);
+            orow[(2 * k) * opitch] = lo;
+            orow[(2 * k + 1) * opitch] = hi;
+        }
+        orow += U * opitch;
+    }
+}
+
 // ---------------------------------------------------------------------------------
 // main kernel: one CTA per 64x64 output tile per exposure, one warp per 32x32 tile
 // ---------------------------------------------------------------------------------
@@ -523,8 +576,6 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
 {
     extern __shared__ __align__(128) float box[];
     __shared__ __align__(8) unsigned long long mbar;
-    __shared__ int s_bb[CTA_T * CTA_T][5];
-    __shared__ int s_box[3];
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int e = P.e0 + blockIdx.z;                  // grid = (ctas_x, ctas_y, exposures): no divisions
@@ -533,46 +584,50 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
     const int ntile = P.tiles_x * P.tiles_y;
     const TileRec *rec = P.recs + ((size_t)e * ntile + (active ? tty * P.tiles_x + ttx : 0));
 
-    int flag = TILE_EMPTY, ix0 = 0, iy0 = 0, bx0 = 0, by0 = 0, bx1 = 0, by1 = 0;
-    if (active) {
-        const int4 h0 = __ldg(reinterpret_cast<const int4 *>(&rec->ix0));       // ix0 iy0 bx0 by0
-        const int4 h1 = __ldg(reinterpret_cast<const int4 *>(&rec->bx1));       // bx1 by1 flag pad
-        ix0 = h0.x; iy0 = h0.y; bx0 = h0.z; by0 = h0.w; bx1 = h1.x; by1 = h1.y; flag = h1.z;
-    }
-
+    // ---- stage the CTA tile's source box first: its origin was reduced by the setup kernel
+    // (cta_box), so the TMA load does not wait for the tile records, which load meanwhile.
     int ox = 0, oy = 0;                 // origin of the staged box in source pixels
     bool has_box = false;
     if (STAGE) {
-        if (lane == 0) {
-            s_bb[warp][0] = (active && flag == TILE_FAST) ? 1 : 0;
-            s_bb[warp][1] = bx0; s_bb[warp][2] = by0; s_bb[warp][3] = bx1; s_bb[warp][4] = by1;
+        const int2 cb = __ldg(P.cta_box + ((size_t)e * P.ctas_y + blockIdx.y) * P.ctas_x + blockIdx.x);
+        has_box = cb.x != kNoBox;
+        // TMA wants a 16-byte aligned start along x (measured on B200: an unaligned inner
+        // coordinate faults with "illegal instruction"): round down to 4 floats
+        ox = (cb.x - (Taps<ORDER>::lo + 1)) & ~3;
+        oy = cb.y - (Taps<ORDER>::lo + 1);
+        if (threadIdx.x == 0 && has_box) {
+            const uint32_t bar = smem_u32(&mbar), dst = smem_u32(box);
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            const uint32_t bytes = (uint32_t)(P.BW * P.BH * sizeof(float));
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+            asm volatile(
+                "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                ::"r"(dst), "l"(&tmap), "r"(ox), "r"(oy), "r"(e), "r"(bar) : "memory");
         }
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            int any = 0, mx = 0x7fffffff, my = 0x7fffffff;
-            for (int w = 0; w < CTA_T * CTA_T; ++w)
-                if (s_bb[w][0]) { any = 1; mx = min(mx, s_bb[w][1]); my = min(my, s_bb[w][2]); }
-            s_box[0] = any;
-            if (any) {
-                // TMA wants a 16-byte aligned start along x (measured on B200: an unaligned
-                // inner coordinate faults with "illegal instruction"): round down to 4 floats
-                mx = (mx - (Taps<ORDER>::lo + 1)) & ~3;
-                my -= Taps<ORDER>::lo + 1;
-                s_box[1] = mx; s_box[2] = my;
-                const uint32_t bar = smem_u32(&mbar), dst = smem_u32(box);
-                asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
-                asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                const uint32_t bytes = (uint32_t)(P.BW * P.BH * sizeof(float));
-                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-                asm volatile(
-                    "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-                    ::"r"(dst), "l"(&tmap), "r"(mx), "r"(my), "r"(e), "r"(bar) : "memory");
-            }
+    }
+
+    int flag = TILE_EMPTY, ix0 = 0, iy0 = 0, bx0 = 0, by0 = 0, bx1 = 0, by1 = 0, deg = 3;
+    if (active) {
+        const int4 h0 = __ldg(reinterpret_cast<const int4 *>(&rec->ix0));       // ix0 iy0 bx0 by0
+        const int4 h1 = __ldg(reinterpret_cast<const int4 *>(&rec->bx1));       // bx1 by1 flag deg
+        ix0 = h0.x; iy0 = h0.y; bx0 = h0.z; by0 = h0.w; bx1 = h1.x; by1 = h1.y; flag = h1.z; deg = h1.w;
+    }
+    // per-lane column polynomials in dj (FAST tiles; harmless otherwise)
+    float X[4], Y[4];
+    {
+        const float di = (float)lane - (float)kCentre;
+        const float4 *c4 = reinterpret_cast<const float4 *>(rec->cx);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const float4 a = __ldg(c4 + q), b = __ldg(c4 + 4 + q);
+            X[q] = fmaf(fmaf(fmaf(a.w, di, a.z), di, a.y), di, a.x);
+            Y[q] = fmaf(fmaf(fmaf(b.w, di, b.z), di, b.y), di, b.x);
         }
-        __syncthreads();
-        has_box = s_box[0] != 0;
-        ox = s_box[1]; oy = s_box[2];
+    }
+    if (STAGE) {
+        __syncthreads();                // the mbarrier is initialised before anybody polls it
         if (has_box) {
             const uint32_t bar = smem_u32(&mbar);
             uint32_t done = 0;
@@ -605,18 +660,6 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
         return;
     }
 
-    // ---- FAST tile: per-lane column polynomials in dj
-    float X[4], Y[4];
-    {
-        const float di = (float)lane - (float)kCentre;
-        const float4 *c4 = reinterpret_cast<const float4 *>(rec->cx);
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const float4 a = __ldg(c4 + q), b = __ldg(c4 + 4 + q);
-            X[q] = fmaf(fmaf(fmaf(a.w, di, a.z), di, a.y), di, a.x);
-            Y[q] = fmaf(fmaf(fmaf(b.w, di, b.z), di, b.y), di, b.x);
-        }
-    }
     // ---- per-axis fast-gather constants (a FAST tile in a STAGE kernel always has a box)
     int Alx, Ahx, Aly, Ahy;
     if (STAGE) {
@@ -641,6 +684,7 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
         G.gbase = img + ((long long)(Aly - tlo) * P.snx + (Alx - tlo));
     }
 
+    if (deg == 1) { X[2] = X[3] = 0.0f; Y[2] = Y[3] = 0.0f; }   // same polynomial on every path
     constexpr int U = 4;                      // rows in flight per thread
     float dj = -(float)kCentre;
     int r = 0;
@@ -655,24 +699,8 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
             for (int q = 0; q < 4; ++q) { X2[q] = splat2(X[q]); Y2[q] = splat2(Y[q]); }
             const uint32_t pitch4 = 4u * (unsigned)G.pitch;
             const uint32_t K = G.sbase - pitch4 * (unsigned)Cy - 4u * (unsigned)Cx;
-            f32x2 d = pk2(dj, dj + 1.0f);
-            const f32x2 step = splat2(2.0f);
-            for (; r + U <= rows; r += U) {
-                f32x2 v[U / 2];
-#pragma unroll
-                for (int k = 0; k < U / 2; ++k) {
-                    v[k] = interior_pair<ORDER>(X2, Y2, d, pitch4, K);
-                    d = add2(d, step);
-                }
-#pragma unroll
-                for (int k = 0; k < U / 2; ++k) {
-                    float lo, hi;
-                    unpk2(v[k], lo, hi);
-                    orow[(2 * k) * opitch] = lo;
-                    orow[(2 * k + 1) * opitch] = hi;
-                }
-                orow += U * opitch;
-            }
+            if (deg == 1) interior_rows<ORDER, 1>(X2, Y2, pitch4, K, rows, r, orow, opitch);
+            else interior_rows<ORDER, 3>(X2, Y2, pitch4, K, rows, r, orow, opitch);
             dj += (float)r;
         }
     }
@@ -722,7 +750,7 @@ tiled_coords_kernel(const __grid_constant__ TiledParams P, const __grid_constant
     if (!(ttx < P.tiles_x && tty < P.tiles_y)) return;
     const int ntile = P.tiles_x * P.tiles_y;
     const TileRec *rec = P.recs + ((size_t)e * ntile + tty * P.tiles_x + ttx);
-    const int flag = rec->flag, ix0 = rec->ix0, iy0 = rec->iy0;
+    const int flag = rec->flag, ix0 = rec->ix0, iy0 = rec->iy0, deg = rec->deg;
     const int tx0 = ttx * TS, ty0 = tty * TS, col = tx0 + lane;
     if (col >= P.onx) return;
     const int rows = min(TS, P.ony - ty0);
@@ -746,6 +774,7 @@ tiled_coords_kernel(const __grid_constant__ TiledParams P, const __grid_constant
         X[q] = fmaf(fmaf(fmaf(a.w, di, a.z), di, a.y), di, a.x);
         Y[q] = fmaf(fmaf(fmaf(b.w, di, b.z), di, b.y), di, b.x);
     }
+    if (deg == 1) { X[2] = X[3] = 0.0f; Y[2] = Y[3] = 0.0f; }   // as the main kernel does
     for (int r = 0; r < rows; ++r) {
         const float dj = (float)r - (float)kCentre;
         const float xl = fmaf(fmaf(fmaf(X[3], dj, X[2]), dj, X[1]), dj, X[0]);
@@ -834,6 +863,7 @@ static cudaError_t launch_main(const TiledParams &P, const TargetDev &tgt, const
 struct Scratch {
     double2 *uv = nullptr;
     TileRec *recs = nullptr;
+    int2 *cta_box = nullptr;
 };
 
 static cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const SourceDev *srcdev,
@@ -852,6 +882,10 @@ static cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, cons
     if ((err = cudaMallocAsync((void **)&sc.uv, sizeof(double2) * (size_t)ntile * NPTS, st)) != cudaSuccess) return err;
     if ((err = cudaMallocAsync((void **)&sc.recs, sizeof(TileRec) * (size_t)ntile * n, st)) != cudaSuccess) return err;
     P.recs = sc.recs;
+    const int ctas = P.ctas_x * P.ctas_y;
+    if ((err = cudaMallocAsync((void **)&sc.cta_box, sizeof(int2) * (size_t)ctas * n, st)) != cudaSuccess) return err;
+    if ((err = cudaMemsetAsync(sc.cta_box, 0x7f, sizeof(int2) * (size_t)ctas * n, st)) != cudaSuccess) return err;
+    P.cta_box = sc.cta_box;
     if (counters && (err = cudaMemsetAsync(counters, 0, 3 * sizeof(int32_t), st)) != cudaSuccess) return err;
     target_nodes_kernel<<<(ntile * NPTS + 127) / 128, 128, 0, st>>>(tgt, fc, P.tiles_x, ntile, sc.uv);
     if ((err = cudaGetLastError()) != cudaSuccess) return err;
@@ -861,10 +895,10 @@ static cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, cons
     const unsigned bx = (unsigned)((ntile + 127) / 128);
     for (int e0 = 0; e0 < n; e0 += 65535) {
         const dim3 grid(bx, (unsigned)std::min(n - e0, 65535));
-        if (maxo == 0) tile_setup_kernel<0><<<grid, 128, 0, st>>>(sc.uv, srcdev, fc, e0, ntile, sny, snx, sc.recs, counters);
-        else if (maxo <= 3) tile_setup_kernel<3><<<grid, 128, 0, st>>>(sc.uv, srcdev, fc, e0, ntile, sny, snx, sc.recs, counters);
-        else if (maxo <= 5) tile_setup_kernel<5><<<grid, 128, 0, st>>>(sc.uv, srcdev, fc, e0, ntile, sny, snx, sc.recs, counters);
-        else tile_setup_kernel<9><<<grid, 128, 0, st>>>(sc.uv, srcdev, fc, e0, ntile, sny, snx, sc.recs, counters);
+        if (maxo == 0) tile_setup_kernel<0><<<grid, 128, 0, st>>>(sc.uv, srcdev, fc, e0, ntile, P.tiles_x, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
+        else if (maxo <= 3) tile_setup_kernel<3><<<grid, 128, 0, st>>>(sc.uv, srcdev, fc, e0, ntile, P.tiles_x, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
+        else if (maxo <= 5) tile_setup_kernel<5><<<grid, 128, 0, st>>>(sc.uv, srcdev, fc, e0, ntile, P.tiles_x, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
+        else tile_setup_kernel<9><<<grid, 128, 0, st>>>(sc.uv, srcdev, fc, e0, ntile, P.tiles_x, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
         if ((err = cudaGetLastError()) != cudaSuccess) return err;
     }
     return cudaSuccess;
@@ -874,6 +908,7 @@ static void free_scratch(Scratch &sc, cudaStream_t st)
 {
     if (sc.uv) cudaFreeAsync(sc.uv, st);
     if (sc.recs) cudaFreeAsync(sc.recs, st);
+    if (sc.cta_box) cudaFreeAsync(sc.cta_box, st);
 }
 
 cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
