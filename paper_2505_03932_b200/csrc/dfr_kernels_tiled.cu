@@ -219,7 +219,7 @@ tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ 
         }
         constexpr double kDegTol = 2.5e-7;
         TileRec r;
-        r.deg = (fmax(q2x, q2y) < kDegTol && fmax(q3x, q3y) < kDegTol) ? 1 : 3;
+        r.deg = fmax(q3x, q3y) >= kDegTol ? 3 : (fmax(q2x, q2y) >= kDegTol ? 2 : 1);
         flag = TILE_EXACT;
         r.ix0 = r.iy0 = r.bx0 = r.by0 = r.bx1 = r.by1 = 0;
         if (finite && fabs(xmin) < 1e9 && fabs(xmax) < 1e9 && fabs(ymin) < 1e9 && fabs(ymax) < 1e9) {
@@ -498,6 +498,9 @@ __device__ __forceinline__ f32x2 interior_pair(const f32x2 (&X)[4], const f32x2 
     if (DEG == 1) {
         xl = fma2(X[1], d, X[0]);
         yl = fma2(Y[1], d, Y[0]);
+    } else if (DEG == 2) {
+        xl = fma2(fma2(X[2], d, X[1]), d, X[0]);
+        yl = fma2(fma2(Y[2], d, Y[1]), d, Y[0]);
     } else {
         xl = fma2(fma2(fma2(X[3], d, X[2]), d, X[1]), d, X[0]);
         yl = fma2(fma2(fma2(Y[3], d, Y[2]), d, Y[1]), d, Y[0]);
@@ -684,7 +687,8 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
         G.gbase = img + ((long long)(Aly - tlo) * P.snx + (Alx - tlo));
     }
 
-    if (deg == 1) { X[2] = X[3] = 0.0f; Y[2] = Y[3] = 0.0f; }   // same polynomial on every path
+    if (deg < 3) { X[3] = 0.0f; Y[3] = 0.0f; }                  // same polynomial on every path
+    if (deg < 2) { X[2] = 0.0f; Y[2] = 0.0f; }
     constexpr int U = 4;                      // rows in flight per thread
     float dj = -(float)kCentre;
     int r = 0;
@@ -700,6 +704,7 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
             const uint32_t pitch4 = 4u * (unsigned)G.pitch;
             const uint32_t K = G.sbase - pitch4 * (unsigned)Cy - 4u * (unsigned)Cx;
             if (deg == 1) interior_rows<ORDER, 1>(X2, Y2, pitch4, K, rows, r, orow, opitch);
+            else if (deg == 2) interior_rows<ORDER, 2>(X2, Y2, pitch4, K, rows, r, orow, opitch);
             else interior_rows<ORDER, 3>(X2, Y2, pitch4, K, rows, r, orow, opitch);
             dj += (float)r;
         }
@@ -774,7 +779,8 @@ tiled_coords_kernel(const __grid_constant__ TiledParams P, const __grid_constant
         X[q] = fmaf(fmaf(fmaf(a.w, di, a.z), di, a.y), di, a.x);
         Y[q] = fmaf(fmaf(fmaf(b.w, di, b.z), di, b.y), di, b.x);
     }
-    if (deg == 1) { X[2] = X[3] = 0.0f; Y[2] = Y[3] = 0.0f; }   // as the main kernel does
+    if (deg < 3) { X[3] = 0.0f; Y[3] = 0.0f; }                  // as the main kernel does
+    if (deg < 2) { X[2] = 0.0f; Y[2] = 0.0f; }
     for (int r = 0; r < rows; ++r) {
         const float dj = (float)r - (float)kCentre;
         const float xl = fmaf(fmaf(fmaf(X[3], dj, X[2]), dj, X[1]), dj, X[0]);

@@ -21,7 +21,7 @@ struct __align__(16) TileRec {
     int32_t ix0, iy0;               // integer base (floor of the tile-centre source pixel)
     int32_t bx0, by0, bx1, by1;     // inclusive range of floor(x), floor(y) over the tile
     int32_t flag;                   // TILE_*
-    int32_t deg;                    // degree in dj the main kernel must keep (1 or 3)
+    int32_t deg;                    // degree in dj the main kernel must keep (1..3)
 };
 static_assert(sizeof(TileRec) == 160, "TileRec layout");
 
