@@ -4,19 +4,25 @@
 // 32x32 output tile it is reproduced to < FIT_TOL px by a bicubic polynomial in
 // the tile-local offsets. Three kernels per dfr_reproject call:
 //
-//   target_nodes_kernel   (fp64) a1-a2 at 25 sample points per tile — shared by the
-//                         whole batch, as SURVEY.md §8(a) a10 notes.
-//   tile_setup_kernel     (fp64) a3-a6 at those points per (exposure, tile); fits the
-//                         cubic through 16 Chebyshev nodes, VERIFIES it against the
-//                         exact map at 9 other points, bounds the source footprint,
-//                         classifies the tile FAST / EXACT / EMPTY.
+//   target_nodes_kernel   (fp64) a1-a2 at 25 sample points per 64x64 CTA tile — shared by
+//                         the whole batch, as SURVEY.md §8(a) a10 notes.
+//   tile_setup_kernel     (fp64) a3-a6 at those points per (exposure, CTA tile); fits the
+//                         cubic through 16 Chebyshev nodes, VERIFIES it against the exact
+//                         map at 9 other points, re-centres it on the four 32x32 tiles
+//                         (or refits each tile when the 64x64 fit fails), bounds each
+//                         tile's source footprint rigorously, classifies it FAST / EXACT /
+//                         EMPTY, picks the dj degree the main kernel must keep, and
+//                         reduces the origin of the CTA tile's staged box.
 //   tiled_reproject_kernel (fp32) per 64x64 CTA tile: the source bounding box is staged
-//                         into shared memory by one TMA box load; each warp walks one
-//                         32x32 tile, 3 FFMA per coordinate per pixel, floor by a
-//                         round-down add, gathers from shared memory, coalesced
-//                         128-byte row stores. Pixels whose taps leave the staged box
-//                         or touch the image rim, and all pixels of EXACT tiles, take
-//                         the exact/global-gather code of dfr_device.cuh.
+//                         into shared memory by one TMA box load issued before the tile
+//                         records arrive; each warp walks one 32x32 tile. INTERIOR tiles
+//                         (every tap inside the image and the box, by the record's bound)
+//                         run the packed loop: two rows per step in FFMA2/FADD2 pairs,
+//                         floor by a round-down add, no range test, one folded address
+//                         per pixel, 4 LDS, coalesced 128-byte row stores. Other FAST
+//                         tiles run the checked scalar loop; pixels whose taps leave the
+//                         staged box or touch the image rim, and all pixels of EXACT
+//                         tiles, take the exact/global-gather code of dfr_device.cuh.
 #include <cuda.h>
 
 #include <algorithm>
@@ -35,7 +41,6 @@ namespace dfr {
 struct FitConsts {
     double W[4][4];            // monomial coefficients of the Lagrange basis: L_a(s) = sum_p W[p][a] s^p
     double pts[NPTS][2];       // sample points (s, t) in [-1, 1]^2; pixel offset = 16 s
-    double WW[16][16];         // WW[k][4q+p] = W[p][a_k] W[q][b_k]: node k -> coefficient of s^p t^q
 };
 
 static FitConsts make_fit_consts()
@@ -59,9 +64,6 @@ static FitConsts make_fit_consts()
             f.pts[4 * b + a][0] = s[a];
             f.pts[4 * b + a][1] = s[b];
         }
-    for (int k = 0; k < 16; ++k)
-        for (int q = 0; q < 4; ++q)
-            for (int pp = 0; pp < 4; ++pp) f.WW[k][4 * q + pp] = f.W[pp][k & 3] * f.W[q][k >> 2];
     const double h = 0.70710678118654752440;
     const double chk[9][2] = {{0, 0}, {h, h}, {-h, h}, {h, -h}, {-h, -h}, {1, 1}, {-1, 1}, {1, -1}, {-1, -1}};
     for (int k = 0; k < 9; ++k) {
@@ -73,21 +75,24 @@ static FitConsts make_fit_consts()
 
 constexpr double kHalf = 0.5 * TS;            // 16: pixel offset of s = 1
 constexpr double kCentre = 0.5 * (TS - 1);    // 15.5: tile centre relative to its first pixel
+constexpr int kNoBox = 0x7fffffff;            // cta_box entry of a CTA tile without FAST tiles
 
 // ---------------------------------------------------------------------------------
 // setup kernels (fp64)
 // ---------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128)
 target_nodes_kernel(const __grid_constant__ TargetDev tgt, const __grid_constant__ FitConsts fc,
-                    int tiles_x, int ntile, double2 *__restrict__ uv)
+                    int ctas_x, int ctas, double2 *__restrict__ uv)
 {
+    // sample points of the 64x64 CTA tiles (the parent fit of tile_setup_kernel)
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= ntile * NPTS) return;
-    const int tile = idx / NPTS, k = idx - tile * NPTS;
-    const int tx0 = (tile % tiles_x) * TS, ty0 = (tile / tiles_x) * TS;
+    if (idx >= ctas * NPTS) return;
+    const int c = idx / NPTS, k = idx - c * NPTS;
+    constexpr double edge = TS * CTA_T;
+    const double cx0 = (c % ctas_x) * edge + 0.5 * (edge - 1), cy0 = (c / ctas_x) * edge + 0.5 * (edge - 1);
     double U, V;
-    target_uv(tgt, tx0 + kCentre + kHalf * fc.pts[k][0], ty0 + kCentre + kHalf * fc.pts[k][1], U, V);
-    uv[(size_t)k * ntile + tile] = make_double2(U, V);      // [point][tile]: coalesced for the setup kernel
+    target_uv(tgt, cx0 + 0.5 * edge * fc.pts[k][0], cy0 + 0.5 * edge * fc.pts[k][1], U, V);
+    uv[(size_t)k * ctas + c] = make_double2(U, V);          // [point][CTA tile]: coalesced for the setup kernel
 }
 
 // Triangle size and row offset of an order-N packed polynomial (see Poly).
@@ -120,15 +125,153 @@ __device__ __forceinline__ void source_xy_sm(const double *__restrict__ sm, doub
     }
 }
 
-// One thread per (tile, exposure); a block is 128 consecutive tiles of ONE exposure so the
-// exposure's constants are staged once in shared memory and every coefficient read is a
-// broadcast LDS. The cubic is fitted separably: along s within each node row, then along t.
+// Cubic fit of the pixel map over one square region: 16 Chebyshev nodes -> tensor-product
+// cubic in (s, t) in [-1, 1]^2 (separably: along s within each node row, then along t),
+// then VERIFIED against the exact map at 9 other points (centre, T4 extrema, corners).
+// uvf(k) returns the target-side (U, V) of sample point k. C[4q + p] = coefficient of s^p t^q.
+template <int N, class UVF>
+__device__ __forceinline__ bool fit_cubic(const double *__restrict__ sm, const FitConsts &fc, UVF uvf,
+                                          double (&Cx)[16], double (&Cy)[16])
+{
+    double Rx[4][4], Ry[4][4];                  // [node row b][power of s]
+    double nanacc = 0.0;
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+        double xs[4], ys[4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            const double2 q = uvf(4 * b + a);
+            source_xy_sm<N>(sm, q.x, q.y, xs[a], ys[a]);
+            nanacc = fma(xs[a], 0.0, fma(ys[a], 0.0, nanacc));
+        }
+#pragma unroll
+        for (int pp = 0; pp < 4; ++pp) {
+            Rx[b][pp] = fma(fc.W[pp][0], xs[0], fma(fc.W[pp][1], xs[1], fma(fc.W[pp][2], xs[2], fc.W[pp][3] * xs[3])));
+            Ry[b][pp] = fma(fc.W[pp][0], ys[0], fma(fc.W[pp][1], ys[1], fma(fc.W[pp][2], ys[2], fc.W[pp][3] * ys[3])));
+        }
+    }
+#pragma unroll
+    for (int qq = 0; qq < 4; ++qq)
+#pragma unroll
+        for (int pp = 0; pp < 4; ++pp) {
+            Cx[4 * qq + pp] = fma(fc.W[qq][0], Rx[0][pp], fma(fc.W[qq][1], Rx[1][pp], fma(fc.W[qq][2], Rx[2][pp], fc.W[qq][3] * Rx[3][pp])));
+            Cy[4 * qq + pp] = fma(fc.W[qq][0], Ry[0][pp], fma(fc.W[qq][1], Ry[1][pp], fma(fc.W[qq][2], Ry[2][pp], fc.W[qq][3] * Ry[3][pp])));
+        }
+    bool good = true;
+#pragma unroll
+    for (int k = 16; k < NPTS; ++k) {
+        const double2 q = uvf(k);
+        double x, y;
+        source_xy_sm<N>(sm, q.x, q.y, x, y);
+        const double ss = fc.pts[k][0], tt = fc.pts[k][1];
+        double px = 0.0, py = 0.0;
+#pragma unroll
+        for (int qq = 3; qq >= 0; --qq) {
+            const double rx = fma(fma(fma(Cx[4 * qq + 3], ss, Cx[4 * qq + 2]), ss, Cx[4 * qq + 1]), ss, Cx[4 * qq]);
+            const double ry = fma(fma(fma(Cy[4 * qq + 3], ss, Cy[4 * qq + 2]), ss, Cy[4 * qq + 1]), ss, Cy[4 * qq]);
+            px = fma(px, tt, rx);
+            py = fma(py, tt, ry);
+        }
+        good = good && (fabs(px - x) <= (double)FIT_TOL) && (fabs(py - y) <= (double)FIT_TOL);   // false on NaN
+    }
+    return good && (nanacc == 0.0);
+}
+
+// p(s0 + s'/2) as a cubic in s': the re-centring of a parent cubic (unit = 32 px) on one of
+// its halves (unit = 16 px). Exact up to fp64 rounding.
+__device__ __forceinline__ void shift_half(double &c0, double &c1, double &c2, double &c3, double s0)
+{
+    const double d0 = fma(s0, fma(s0, fma(s0, c3, c2), c1), c0);
+    const double d1 = 0.5 * fma(s0, fma(3.0 * s0, c3, 2.0 * c2), c1);
+    const double d2 = 0.25 * fma(3.0 * s0, c3, c2);
+    c0 = d0; c1 = d1; c2 = d2; c3 = 0.125 * c3;
+}
+
+// The record of one 32x32 tile from its cubic (unit = 16 px about the tile centre):
+// footprint bound, classification, dj degree, integer base, fp32 coefficients.
+// Returns the flag; (bx0, by0) is the first floor index the tile can touch.
+__device__ __forceinline__ int emit_tile(double (&Cx)[16], double (&Cy)[16], bool finite, int sny, int snx,
+                                         TileRec *__restrict__ out, int &bx0, int &by0)
+{
+    // Rigorous range of the fitted polynomial over the tile: |s|, |t| <= 31/32 < 1, so
+    // |x - C00| <= sum of the other |C_pq|. The main kernel evaluates exactly this
+    // polynomial (in fp32: + kBoxSlack), which is what makes its unchecked gathers safe.
+    double ex = 0.0, ey = 0.0;
+#pragma unroll
+    for (int k = 1; k < 16; ++k) { ex += fabs(Cx[k]); ey += fabs(Cy[k]); }
+    constexpr double kBoxSlack = 1e-3;
+    const double xmin = Cx[0] - ex - kBoxSlack, xmax = Cx[0] + ex + kBoxSlack;
+    const double ymin = Cy[0] - ey - kBoxSlack, ymax = Cy[0] + ey + kBoxSlack;
+    // Degree of the per-lane column polynomials in dj: the t^2, t^3 terms (any power of s)
+    // are dropped by the main kernel when they cannot move a coordinate by kDegTol px.
+    double q2x = 0.0, q2y = 0.0, q3x = 0.0, q3y = 0.0;
+#pragma unroll
+    for (int pp = 0; pp < 4; ++pp) {
+        q2x += fabs(Cx[8 + pp]); q2y += fabs(Cy[8 + pp]);
+        q3x += fabs(Cx[12 + pp]); q3y += fabs(Cy[12 + pp]);
+    }
+    constexpr double kDegTol = 2.5e-7;
+    TileRec r;
+    r.deg = fmax(q3x, q3y) >= kDegTol ? 3 : (fmax(q2x, q2y) >= kDegTol ? 2 : 1);
+    int flag = TILE_EXACT;
+    r.ix0 = r.iy0 = r.bx0 = r.by0 = r.bx1 = r.by1 = 0;
+    double bx = 0.0, by = 0.0;
+    if (finite && fabs(xmin) < 1e9 && fabs(xmax) < 1e9 && fabs(ymin) < 1e9 && fabs(ymax) < 1e9) {
+        bx = floor(Cx[0]); by = floor(Cy[0]);
+        r.ix0 = (int)bx; r.iy0 = (int)by;
+        r.bx0 = (int)floor(xmin); r.bx1 = (int)floor(xmax);
+        r.by0 = (int)floor(ymin); r.by1 = (int)floor(ymax);
+        const bool small = (r.bx1 - r.bx0) < 2048 && (r.by1 - r.by0) < 2048 &&
+                           abs(r.bx0 - r.ix0) < 2048 && abs(r.bx1 - r.ix0) < 2048 &&
+                           abs(r.by0 - r.iy0) < 2048 && abs(r.by1 - r.iy0) < 2048;
+        if (small) {
+            // outside the footprint [-0.5, n-0.5) by a 2 px margin on one side => all NaN
+            const bool outside = (xmax + 2.0 < -0.5) || (xmin - 2.0 >= snx - 0.5) ||
+                                 (ymax + 2.0 < -0.5) || (ymin - 2.0 >= sny - 0.5);
+            flag = outside ? TILE_EMPTY : TILE_FAST;
+        } else {
+            bx = by = 0.0;
+        }
+    }
+    r.flag = flag;
+    bx0 = r.bx0; by0 = r.by0;
+    // s = di / 16: coefficient of di^p dj^q is C[p][q] / 16^(p+q)
+    double sq = 1.0;
+#pragma unroll
+    for (int qq = 0; qq < 4; ++qq) {
+        double sp = sq;
+#pragma unroll
+        for (int pp = 0; pp < 4; ++pp) {
+            const double c0x = (qq == 0 && pp == 0) ? Cx[0] - bx : Cx[4 * qq + pp];
+            const double c0y = (qq == 0 && pp == 0) ? Cy[0] - by : Cy[4 * qq + pp];
+            r.cx[4 * qq + pp] = (float)(c0x * sp);
+            r.cy[4 * qq + pp] = (float)(c0y * sp);
+            sp *= 1.0 / kHalf;
+        }
+        sq *= 1.0 / kHalf;
+    }
+    *out = r;
+    return flag;
+}
+
+// One thread per (64x64 CTA tile, exposure); a block is 128 consecutive CTA tiles of ONE
+// exposure, so the exposure's constants are staged once in shared memory and every
+// coefficient read is a broadcast LDS. Two levels:
+//   1. the cubic is fitted and verified over the whole 64x64 CTA tile (25 map evaluations);
+//      if it holds, the four 32x32 tile records are its exact re-centrings (no more map
+//      evaluations) — 4x less fp64 work than fitting each tile;
+//   2. if it does not (strongly curved maps), each 32x32 tile gets its own fit, with the
+//      target side (a1-a2) evaluated on the fly; a tile whose own fit fails is EXACT.
+// (Measured on B200, C2: 16.8 us; four threads per CTA tile sharing the parent fit through
+// shared memory took 21-23 us — more waves of a latency-bound kernel — so this stays.)
+constexpr int kSetupThreads = 128;
+
 template <int N>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(kSetupThreads)
 tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ srcdev,
-                  const __grid_constant__ FitConsts fc, int e0, int ntile, int tiles_x, int ctas_x,
-                  int ctas, int sny, int snx, TileRec *__restrict__ recs, int2 *__restrict__ cta_box,
-                  int32_t *__restrict__ counters)
+                  const __grid_constant__ TargetDev tgt, const __grid_constant__ FitConsts fc, int e0,
+                  int tiles_x, int tiles_y, int ctas_x, int ctas, int sny, int snx,
+                  TileRec *__restrict__ recs, int2 *__restrict__ cta_box, int32_t *__restrict__ counters)
 {
     __shared__ double sm[11 + 2 * tri(N)];
     const int e = e0 + blockIdx.y;
@@ -152,120 +295,55 @@ tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ 
         }
     }
     __syncthreads();
-    const int tile = blockIdx.x * blockDim.x + threadIdx.x;
-    int flag = -1;
-    if (tile < ntile) {
-        const double2 *p = uv + tile;
-        double Rx[4][4], Ry[4][4];                  // [node row b][power of s]
-        double nanacc = 0.0;
+    const int c = blockIdx.x * kSetupThreads + threadIdx.x;
+    int nflag[3] = {0, 0, 0};
+    if (c < ctas) {
+        const int cty = c / ctas_x, ctx = c - cty * ctas_x;
+        double Px[16], Py[16];                      // parent cubic, unit = 32 px
+        const bool parent = fit_cubic<N>(sm, fc, [&](int k) { return __ldg(uv + (size_t)k * ctas + c); }, Px, Py);
+        int box_x = kNoBox, box_y = kNoBox;
+#pragma unroll 1
+        for (int sub = 0; sub < CTA_T * CTA_T; ++sub) {
+            const int ttx = ctx * CTA_T + (sub % CTA_T), tty = cty * CTA_T + (sub / CTA_T);
+            if (ttx >= tiles_x || tty >= tiles_y) continue;
+            double Cx[16], Cy[16];
+            bool good = true;
+            if (parent) {
+                const double s0 = (sub % CTA_T) ? 0.5 : -0.5, t0 = (sub / CTA_T) ? 0.5 : -0.5;
 #pragma unroll
-        for (int b = 0; b < 4; ++b) {
-            double xs[4], ys[4];
+                for (int k = 0; k < 16; ++k) { Cx[k] = Px[k]; Cy[k] = Py[k]; }
 #pragma unroll
-            for (int a = 0; a < 4; ++a) {
-                const double2 q = p[(size_t)(4 * b + a) * ntile];
-                source_xy_sm<N>(sm, q.x, q.y, xs[a], ys[a]);
-                nanacc = fma(xs[a], 0.0, fma(ys[a], 0.0, nanacc));
-            }
-#pragma unroll
-            for (int pp = 0; pp < 4; ++pp) {
-                Rx[b][pp] = fma(fc.W[pp][0], xs[0], fma(fc.W[pp][1], xs[1], fma(fc.W[pp][2], xs[2], fc.W[pp][3] * xs[3])));
-                Ry[b][pp] = fma(fc.W[pp][0], ys[0], fma(fc.W[pp][1], ys[1], fma(fc.W[pp][2], ys[2], fc.W[pp][3] * ys[3])));
-            }
-        }
-        double Cx[16], Cy[16];                      // [4q + p]: coefficient of s^p t^q
-#pragma unroll
-        for (int qq = 0; qq < 4; ++qq)
-#pragma unroll
-            for (int pp = 0; pp < 4; ++pp) {
-                Cx[4 * qq + pp] = fma(fc.W[qq][0], Rx[0][pp], fma(fc.W[qq][1], Rx[1][pp], fma(fc.W[qq][2], Rx[2][pp], fc.W[qq][3] * Rx[3][pp])));
-                Cy[4 * qq + pp] = fma(fc.W[qq][0], Ry[0][pp], fma(fc.W[qq][1], Ry[1][pp], fma(fc.W[qq][2], Ry[2][pp], fc.W[qq][3] * Ry[3][pp])));
-            }
-        // verify the fit against the exact map at 9 other points (centre, T4 extrema, corners)
-        bool good = true;
-#pragma unroll
-        for (int k = 16; k < NPTS; ++k) {
-            const double2 q = p[(size_t)k * ntile];
-            double x, y;
-            source_xy_sm<N>(sm, q.x, q.y, x, y);
-            const double ss = fc.pts[k][0], tt = fc.pts[k][1];
-            double px = 0.0, py = 0.0;
-#pragma unroll
-            for (int qq = 3; qq >= 0; --qq) {
-                const double rx = fma(fma(fma(Cx[4 * qq + 3], ss, Cx[4 * qq + 2]), ss, Cx[4 * qq + 1]), ss, Cx[4 * qq]);
-                const double ry = fma(fma(fma(Cy[4 * qq + 3], ss, Cy[4 * qq + 2]), ss, Cy[4 * qq + 1]), ss, Cy[4 * qq]);
-                px = fma(px, tt, rx);
-                py = fma(py, tt, ry);
-            }
-            good = good && (fabs(px - x) <= (double)FIT_TOL) && (fabs(py - y) <= (double)FIT_TOL);   // false on NaN
-        }
-        // Rigorous range of the fitted polynomial over the tile: |s|, |t| <= 31/32 < 1, so
-        // |x - C00| <= sum of the other |C_pq|. The main kernel evaluates exactly this
-        // polynomial (in fp32: + kBoxSlack), which is what makes its unchecked gathers safe.
-        double ex = 0.0, ey = 0.0;
-#pragma unroll
-        for (int k = 1; k < 16; ++k) { ex += fabs(Cx[k]); ey += fabs(Cy[k]); }
-        constexpr double kBoxSlack = 1e-3;
-        const double xmin = Cx[0] - ex - kBoxSlack, xmax = Cx[0] + ex + kBoxSlack;
-        const double ymin = Cy[0] - ey - kBoxSlack, ymax = Cy[0] + ey + kBoxSlack;
-        const bool finite = good && (nanacc == 0.0);
-        // Degree of the per-lane column polynomials in dj: the t^2, t^3 terms (any power of s)
-        // are dropped by the main kernel when they cannot move a coordinate by kDegTol px.
-        double q2x = 0.0, q2y = 0.0, q3x = 0.0, q3y = 0.0;
-#pragma unroll
-        for (int pp = 0; pp < 4; ++pp) {
-            q2x += fabs(Cx[8 + pp]); q2y += fabs(Cy[8 + pp]);
-            q3x += fabs(Cx[12 + pp]); q3y += fabs(Cy[12 + pp]);
-        }
-        constexpr double kDegTol = 2.5e-7;
-        TileRec r;
-        r.deg = fmax(q3x, q3y) >= kDegTol ? 3 : (fmax(q2x, q2y) >= kDegTol ? 2 : 1);
-        flag = TILE_EXACT;
-        r.ix0 = r.iy0 = r.bx0 = r.by0 = r.bx1 = r.by1 = 0;
-        if (finite && fabs(xmin) < 1e9 && fabs(xmax) < 1e9 && fabs(ymin) < 1e9 && fabs(ymax) < 1e9) {
-            const double bx = floor(Cx[0]), by = floor(Cy[0]);
-            r.ix0 = (int)bx; r.iy0 = (int)by;
-            r.bx0 = (int)floor(xmin); r.bx1 = (int)floor(xmax);
-            r.by0 = (int)floor(ymin); r.by1 = (int)floor(ymax);
-            const bool small = (r.bx1 - r.bx0) < 2048 && (r.by1 - r.by0) < 2048 &&
-                               abs(r.bx0 - r.ix0) < 2048 && abs(r.bx1 - r.ix0) < 2048 &&
-                               abs(r.by0 - r.iy0) < 2048 && abs(r.by1 - r.iy0) < 2048;
-            if (small) {
-                // outside the footprint [-0.5, n-0.5) by a 2 px margin on one side => all NaN
-                const bool out = (xmax + 2.0 < -0.5) || (xmin - 2.0 >= snx - 0.5) ||
-                                 (ymax + 2.0 < -0.5) || (ymin - 2.0 >= sny - 0.5);
-                flag = out ? TILE_EMPTY : TILE_FAST;
-                if (flag == TILE_FAST) {
-                    // origin of the CTA tile's staged box = min over its FAST tiles
-                    const int tty = tile / tiles_x, ttx = tile - tty * tiles_x;
-                    int2 *cb = cta_box + ((size_t)e * ctas + (tty / CTA_T) * ctas_x + ttx / CTA_T);
-                    atomicMin(&cb->x, r.bx0);
-                    atomicMin(&cb->y, r.by0);
+                for (int q = 0; q < 4; ++q) {       // along s, each power of t
+                    shift_half(Cx[4 * q], Cx[4 * q + 1], Cx[4 * q + 2], Cx[4 * q + 3], s0);
+                    shift_half(Cy[4 * q], Cy[4 * q + 1], Cy[4 * q + 2], Cy[4 * q + 3], s0);
                 }
-            }
-            Cx[0] -= bx;
-            Cy[0] -= by;
-        }
-        r.flag = flag;
-        // s = di / 16: coefficient of di^p dj^q is C[p][q] / 16^(p+q)
-        double sq = 1.0;
 #pragma unroll
-        for (int qq = 0; qq < 4; ++qq) {
-            double sp = sq;
-#pragma unroll
-            for (int pp = 0; pp < 4; ++pp) {
-                r.cx[4 * qq + pp] = (float)(Cx[4 * qq + pp] * sp);
-                r.cy[4 * qq + pp] = (float)(Cy[4 * qq + pp] * sp);
-                sp *= 1.0 / kHalf;
+                for (int pp = 0; pp < 4; ++pp) {    // along t, each power of s
+                    shift_half(Cx[pp], Cx[4 + pp], Cx[8 + pp], Cx[12 + pp], t0);
+                    shift_half(Cy[pp], Cy[4 + pp], Cy[8 + pp], Cy[12 + pp], t0);
+                }
+            } else {
+                const double cx0 = ttx * TS + kCentre, cy0 = tty * TS + kCentre;
+                good = fit_cubic<N>(sm, fc, [&](int k) {
+                    double U, V;
+                    target_uv(tgt, cx0 + kHalf * fc.pts[k][0], cy0 + kHalf * fc.pts[k][1], U, V);
+                    return make_double2(U, V);
+                }, Cx, Cy);
             }
-            sq *= 1.0 / kHalf;
+            int bx0, by0;
+            const int flag = emit_tile(Cx, Cy, good, sny, snx,
+                                       recs + ((size_t)e * tiles_x * tiles_y + (size_t)tty * tiles_x + ttx), bx0, by0);
+            ++nflag[flag];
+            if (flag == TILE_FAST) { box_x = min(box_x, bx0); box_y = min(box_y, by0); }
         }
-        recs[(size_t)e * ntile + tile] = r;
+        // origin of the CTA tile's staged box = min over its FAST tiles (kNoBox: none)
+        cta_box[(size_t)e * ctas + c] = make_int2(box_x, box_y);
     }
     if (counters) {
+#pragma unroll
         for (int f = 0; f < 3; ++f) {
-            const int c = __syncthreads_count(flag == f);
-            if (threadIdx.x == 0 && c) atomicAdd(&counters[f], c);
+            const int w = __reduce_add_sync(0xffffffffu, nflag[f]);
+            if ((threadIdx.x & 31) == 0 && w) atomicAdd(&counters[f], w);
         }
     }
 }
@@ -280,8 +358,6 @@ template <int ORDER> struct Taps;
 template <> struct Taps<DFR_NEAREST>  { static constexpr int lo = 0, hi = 1; };   // rint in {floor, floor+1}
 template <> struct Taps<DFR_BILINEAR> { static constexpr int lo = 0, hi = 1; };
 template <> struct Taps<DFR_BICUBIC>  { static constexpr int lo = 1, hi = 2; };
-
-constexpr int kNoBox = 0x7f7f7f7f;                 // cudaMemset(0x7f) pattern: no FAST tile in this CTA tile
 
 struct TiledParams {
     const float *src;
@@ -885,26 +961,25 @@ static cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, cons
     P.srcdev = srcdev;
     const int ntile = P.tiles_x * P.tiles_y;
     cudaError_t err;
-    if ((err = cudaMallocAsync((void **)&sc.uv, sizeof(double2) * (size_t)ntile * NPTS, st)) != cudaSuccess) return err;
+    const int ctas = P.ctas_x * P.ctas_y;
+    if ((err = cudaMallocAsync((void **)&sc.uv, sizeof(double2) * (size_t)ctas * NPTS, st)) != cudaSuccess) return err;
     if ((err = cudaMallocAsync((void **)&sc.recs, sizeof(TileRec) * (size_t)ntile * n, st)) != cudaSuccess) return err;
     P.recs = sc.recs;
-    const int ctas = P.ctas_x * P.ctas_y;
     if ((err = cudaMallocAsync((void **)&sc.cta_box, sizeof(int2) * (size_t)ctas * n, st)) != cudaSuccess) return err;
-    if ((err = cudaMemsetAsync(sc.cta_box, 0x7f, sizeof(int2) * (size_t)ctas * n, st)) != cudaSuccess) return err;
     P.cta_box = sc.cta_box;
     if (counters && (err = cudaMemsetAsync(counters, 0, 3 * sizeof(int32_t), st)) != cudaSuccess) return err;
-    target_nodes_kernel<<<(ntile * NPTS + 127) / 128, 128, 0, st>>>(tgt, fc, P.tiles_x, ntile, sc.uv);
+    target_nodes_kernel<<<(ctas * NPTS + 127) / 128, 128, 0, st>>>(tgt, fc, P.ctas_x, ctas, sc.uv);
     if ((err = cudaGetLastError()) != cudaSuccess) return err;
     // SIP order class of the batch: inverse polynomials are zero-padded up to N
     int maxo = 0;
     for (int e = 0; e < n; ++e) maxo = std::max(maxo, std::max(srchost[e].ap.order, srchost[e].bp.order));
-    const unsigned bx = (unsigned)((ntile + 127) / 128);
+    const unsigned bx = (unsigned)((ctas + kSetupThreads - 1) / kSetupThreads);
     for (int e0 = 0; e0 < n; e0 += 65535) {
         const dim3 grid(bx, (unsigned)std::min(n - e0, 65535));
-        if (maxo == 0) tile_setup_kernel<0><<<grid, 128, 0, st>>>(sc.uv, srcdev, fc, e0, ntile, P.tiles_x, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
-        else if (maxo <= 3) tile_setup_kernel<3><<<grid, 128, 0, st>>>(sc.uv, srcdev, fc, e0, ntile, P.tiles_x, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
-        else if (maxo <= 5) tile_setup_kernel<5><<<grid, 128, 0, st>>>(sc.uv, srcdev, fc, e0, ntile, P.tiles_x, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
-        else tile_setup_kernel<9><<<grid, 128, 0, st>>>(sc.uv, srcdev, fc, e0, ntile, P.tiles_x, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
+        if (maxo == 0) tile_setup_kernel<0><<<grid, 128, 0, st>>>(sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
+        else if (maxo <= 3) tile_setup_kernel<3><<<grid, 128, 0, st>>>(sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
+        else if (maxo <= 5) tile_setup_kernel<5><<<grid, 128, 0, st>>>(sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
+        else tile_setup_kernel<9><<<grid, 128, 0, st>>>(sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
         if ((err = cudaGetLastError()) != cudaSuccess) return err;
     }
     return cudaSuccess;
