@@ -262,3 +262,30 @@ def test_unaligned_row_pitch_uses_global_gathers(P):
     w = S.Workload("odd", img[None], [src], tgt, (310, 390), (0, 1, 3))
     rep, _ = full_parity(P, w, 0)
     assert P.dfr_last_stats()["tiles_fast"] > 0
+
+
+def test_two_level_setup_fallback(P):
+    """A quartic target distortion sized so that the cubic fit of a 64x64 CTA tile misses
+    FIT_TOL (error ~ c h^4 / 8 = 1.3e-5 px at h = 32) while the fit of each 32x32 tile holds
+    (8e-7 px): the setup kernel must refit per tile, not accept the parent cubic and not
+    fall to EXACT. A 100x larger quartic defeats both levels: tiles become EXACT."""
+    rng = np.random.default_rng(41)
+    img = S.make_image(512, 512, 200, rng)
+    src = S.make_wcs(512, 512, 150.0, 2.0, 0.0, S.PIXSCALE)
+    for c4, want_exact in ((1e-10, False), (1e-8, True)):
+        tgt = S.make_wcs(512, 512, 150.0005, 2.0003, 0.7, S.PIXSCALE)
+        tgt.a_order = tgt.b_order = 4
+        tgt.a[4][0] = c4
+        tgt.b[0][4] = -c4
+        w = S.Workload("quartic", img[None], [src], tgt, (512, 512), (1,))
+        rep, _ = full_parity(P, w, 0)
+        st = P.dfr_last_stats()
+        xf, yf = P.dfr_src_coords(w.src_wcs, w.tgt_wcs, (512, 512), w.shape_out, 1, path=P.PATH_AUTO)
+        xe, ye = P.dfr_src_coords(w.src_wcs, w.tgt_wcs, (512, 512), w.shape_out, 1, path=P.PATH_EXACT)
+        d = max(torch.nan_to_num(xf - xe).abs().max().item(), torch.nan_to_num(yf - ye).abs().max().item())
+        print("quartic", c4, st, "tiled vs exact", d, rep[("coords", 0)])
+        if want_exact:
+            assert st["tiles_exact"] > 0
+        else:
+            assert st["tiles_exact"] == 0 and st["tiles_fast"] > 200
+            assert d < 5e-6                   # 1.3e-5 if the parent cubic had been accepted
