@@ -60,6 +60,9 @@ def lib():
         _lib.orc_reproject.argtypes = [fp, C.c_int32, C.c_int32, C.c_int32, wp, wp,
                                        C.c_int32, C.c_int32, C.c_int32, fp]
         _lib.orc_reproject.restype = C.c_int
+        _lib.orc_stack.argtypes = [fp, C.c_int32, C.c_int32, C.c_int32, wp, wp,
+                                   C.c_int32, C.c_int32, C.c_int32, dp, fp, fp]
+        _lib.orc_stack.restype = C.c_int
         _lib.orc_cd_from_pc_cdelt.argtypes = [dp, dp, dp]
         _lib.orc_closed_iwc2sky.argtypes = [dp, dp, dp, C.c_int64, dp, dp]
         _lib.orc_closed_sky2iwc.argtypes = [dp, dp, dp, C.c_int64, dp, dp]
@@ -140,6 +143,30 @@ def reproject(images, src_wcs, tgt_wcs, shape_out, order):
     if rc != 0:
         raise ValueError("orc_reproject: bad order")
     return out
+
+
+def stack(images, src_wcs, tgt_wcs, shape_out, order, weights=None):
+    """orc_stack: (sum, wsum), float32 [ny][nx] each (orc.h; reading G17)."""
+    images = np.ascontiguousarray(images, dtype=np.float32)
+    if images.ndim == 2:
+        images = images[None]
+    n, ny, nx = images.shape
+    assert len(src_wcs) == n
+    arr = (OrcWCS * n)(*[pack(w) for w in src_wcs])
+    t = pack(tgt_wcs)
+    sum_ = np.empty((int(shape_out[0]), int(shape_out[1])), dtype=np.float32)
+    wsum = np.empty_like(sum_)
+    wp_ = None
+    if weights is not None:
+        weights, wp_ = _d(weights)
+        assert weights.size == n
+    rc = lib().orc_stack(images.ctypes.data_as(C.POINTER(C.c_float)), n, ny, nx, arr, C.byref(t),
+                         int(shape_out[0]), int(shape_out[1]), int(order), wp_,
+                         sum_.ctypes.data_as(C.POINTER(C.c_float)),
+                         wsum.ctypes.data_as(C.POINTER(C.c_float)))
+    if rc != 0:
+        raise ValueError("orc_stack: bad order")
+    return sum_, wsum
 
 
 def cd_from_pc_cdelt(pc, cdelt):

@@ -228,6 +228,34 @@ int orc_reproject(const float *src_batch, int32_t n, int32_t src_ny, int32_t src
     return 0;
 }
 
+int orc_stack(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+              const orc_wcs *src_wcs, const orc_wcs *tgt_wcs,
+              int32_t out_ny, int32_t out_nx, int32_t order, const double *weight,
+              float *sum, float *wsum)
+{
+    if (order != ORC_NEAREST && order != ORC_BILINEAR && order != ORC_BICUBIC) return -1;
+#pragma omp parallel for schedule(static)
+    for (int32_t j = 0; j < out_ny; ++j)
+        for (int32_t i = 0; i < out_nx; ++i) {
+            double ra, dec, s = 0.0, W = 0.0;
+            pix2sky_rad(tgt_wcs, (double)i, (double)j, &ra, &dec);            /* O1-O5  */
+            for (int32_t e = 0; e < n; ++e) {                                  /* exposure order */
+                const float *src = src_batch + (size_t)e * (size_t)src_ny * (size_t)src_nx;
+                double x, y;
+                sky2pix_rad(&src_wcs[e], ra, dec, &x, &y);                     /* O6-O10 */
+                double val = interp_one(src, src_ny, src_nx, x, y, order, -0.75); /* O11-O12 */
+                if (val == val) {                                              /* not NaN */
+                    const double w = weight ? weight[e] : 1.0;
+                    s += w * val;
+                    W += w;
+                }
+            }
+            sum[(size_t)j * (size_t)out_nx + (size_t)i] = (float)s;
+            wsum[(size_t)j * (size_t)out_nx + (size_t)i] = (float)W;
+        }
+    return 0;
+}
+
 void orc_cd_from_pc_cdelt(const double pc[4], const double cdelt[2], double cd[4])
 {
     cd[0] = cdelt[0] * pc[0];

@@ -63,6 +63,20 @@ int orc_reproject(const float *src_batch, int32_t n, int32_t src_ny, int32_t src
                   const orc_wcs *src_wcs, const orc_wcs *tgt_wcs,
                   int32_t out_ny, int32_t out_nx, int32_t order, float *out);
 
+/* Stacking (the paper's stated purpose of reprojection, "combined
+ * to produce a single, deeper image"; reading G17 of DESIGN.md):
+ *   sum [j][i] = sum over exposures e of weight[e] * v_e(i, j)
+ *   wsum[j][i] = sum over the same exposures of weight[e]
+ * where v_e is the value O1-O12 give for exposure e (a double, NOT rounded to float32
+ * first) and an exposure contributes to a pixel only where v_e is not NaN (outside its
+ * footprint, or NaN source pixels under the taps). Accumulated in double in exposure
+ * order, stored as float32. weight == NULL means 1 for every exposure.
+ * Returns 0, or -1 on a bad order. Pins: tests/test_oracle_stack.py (S1-S6). */
+int orc_stack(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+              const orc_wcs *src_wcs, const orc_wcs *tgt_wcs,
+              int32_t out_ny, int32_t out_nx, int32_t order, const double *weight,
+              float *sum, float *wsum);
+
 /* CD_ij = CDELT_i * PC_ij. */
 void orc_cd_from_pc_cdelt(const double pc[4], const double cdelt[2], double cd[4]);
 
