@@ -618,30 +618,156 @@ __device__ __forceinline__ f32x2 interior_pair(const f32x2 (&X)[4], const f32x2 
     return acc;
 }
 
-// All complete groups of U rows of an interior tile; advances r and orow.
-template <int ORDER, int DEG>
+// Where the values of a tile go. A sink receives the rows of a tile in increasing order:
+// rows4(v) = the next four rows, row1(v) = the next single row (ragged bottom edge).
+// StoreSink: the per-exposure output of dfr_reproject (one coalesced 128-byte row per warp).
+struct StoreSink {
+    static constexpr bool kAllLanes = false;       // lanes beyond the right edge may leave early
+    float *__restrict__ orow;
+    size_t opitch;
+    __device__ __forceinline__ void rows4(float v0, float v1, float v2, float v3)
+    {
+        orow[0] = v0;
+        orow[opitch] = v1;
+        orow[2 * opitch] = v2;
+        orow[3 * opitch] = v3;
+        orow += 4 * opitch;
+    }
+    __device__ __forceinline__ void row1(float v)
+    {
+        *orow = v;
+        orow += opitch;
+    }
+    __device__ __forceinline__ void empty_tile(int rows)
+    {
+        for (int r = 0; r < rows; ++r) orow[r * opitch] = qnanf();
+    }
+};
+
+// All complete groups of U rows of an interior tile; advances r.
+template <int ORDER, int DEG, class Sink>
 __device__ __forceinline__ void interior_rows(const f32x2 (&X2)[4], const f32x2 (&Y2)[4], uint32_t pitch4,
-                                              uint32_t K, int rows, int &r, float *__restrict__ &orow,
-                                              size_t opitch)
+                                              uint32_t K, int rows, int &r, Sink &sink)
 {
-    constexpr int U = (ORDER == DFR_BICUBIC) ? 2 : 4;           // rows in flight per thread
     f32x2 d = pk2(-(float)kCentre, 1.0f - (float)kCentre);
     const f32x2 step = splat2(2.0f);
+    for (; r + 4 <= rows; r += 4) {
+        const f32x2 va = interior_pair<ORDER, DEG>(X2, Y2, d, pitch4, K);
+        d = add2(d, step);
+        const f32x2 vb = interior_pair<ORDER, DEG>(X2, Y2, d, pitch4, K);
+        d = add2(d, step);
+        float v0, v1, v2, v3;
+        unpk2(va, v0, v1);
+        unpk2(vb, v2, v3);
+        sink.rows4(v0, v1, v2, v3);
+    }
+}
+
+// One 32x32 tile by one warp (lane = output column): EMPTY -> NaN, EXACT -> fp64 map per
+// pixel, FAST -> polynomial coordinates + gathers from the staged box (STAGE) or the image.
+// (ox, oy) is the source pixel of the staged box's element (0, 0); box_smem its shared address.
+struct TileHead {
+    int flag, ix0, iy0, bx0, by0, bx1, by1, deg;
+};
+
+template <int ORDER, bool STAGE, class Sink>
+__device__ __forceinline__ void warp_tile(const TiledParams &P, const TargetDev &tgt, int e, int ttx, int tty,
+                                          int lane, const TileHead &H, float (&X)[4], float (&Y)[4],
+                                          uint32_t box_smem, int ox, int oy, Sink &sink)
+{
+    const int flag = H.flag, ix0 = H.ix0, iy0 = H.iy0, bx0 = H.bx0, by0 = H.by0, bx1 = H.bx1, by1 = H.by1,
+              deg = H.deg;
+    const int tx0 = ttx * TS, ty0 = tty * TS;
+    const int col = tx0 + lane;
+    if (!Sink::kAllLanes && col >= P.onx) return;      // ragged right edge (no block-level sync below)
+    const int rows = min(TS, P.ony - ty0);
+    const float *__restrict__ img = P.src + (size_t)e * P.sny * P.snx;
+
+    if (flag == TILE_EMPTY) {
+        sink.empty_tile(rows);
+        return;
+    }
+    if (flag == TILE_EXACT) {
+        for (int r = 0; r < rows; ++r)
+            sink.row1(exact_pixel<ORDER>(img, P.sny, P.snx, tgt, P.srcdev[e], col, ty0 + r));
+        return;
+    }
+
+    // ---- per-axis fast-gather constants (a FAST tile in a STAGE kernel always has a box)
+    int Alx, Ahx, Aly, Ahy;
+    if (STAGE) {
+        axis_range<ORDER>(P.snx, ox, P.BW, Alx, Ahx);
+        axis_range<ORDER>(P.sny, oy, P.BH, Aly, Ahy);
+    } else {
+        axis_range<ORDER>(P.snx, -(1 << 28), 1 << 30, Alx, Ahx);
+        axis_range<ORDER>(P.sny, -(1 << 28), 1 << 30, Aly, Ahy);
+    }
+    const unsigned cntx = (unsigned)max(Ahx - Alx + 1, 0), cnty = (unsigned)max(Ahy - Aly + 1, 0);
+    const int Cx = kMagicBits - ix0 + Alx, Cy = kMagicBits - iy0 + Aly;
+    // gather array: element (k = 0) = first tap of base index (Alx, Aly)
+    const int tlo = (ORDER == DFR_BICUBIC) ? 1 : 0;
+    GatherSrc<STAGE> G;
+    if (STAGE) {
+        G.pitch = P.BW;
+        G.sbase = box_smem + 4u * (unsigned)((Aly - tlo - oy) * P.BW + (Alx - tlo - ox));
+        G.gbase = nullptr;
+    } else {
+        G.pitch = P.snx;
+        G.sbase = 0;
+        G.gbase = img + ((long long)(Aly - tlo) * P.snx + (Alx - tlo));
+    }
+
+    if (deg < 3) { X[3] = 0.0f; Y[3] = 0.0f; }                  // same polynomial on every path
+    if (deg < 2) { X[2] = 0.0f; Y[2] = 0.0f; }
+    constexpr int U = 4;                      // rows in flight per thread
+    float dj = -(float)kCentre;
+    int r = 0;
+    if (STAGE) {
+        // INTERIOR tile: the record's rigorous index range lies inside [Al, Ah] on both axes
+        // (image interior AND staged box), so no pixel needs a range test or the rim rule.
+        const int top = (ORDER == DFR_NEAREST) ? 1 : 0;          // rint(x) <= floor(x) + 1
+        const bool interior = bx0 >= Alx && bx1 + top <= Ahx && by0 >= Aly && by1 + top <= Ahy;
+        if (interior) {
+            f32x2 X2[4], Y2[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) { X2[q] = splat2(X[q]); Y2[q] = splat2(Y[q]); }
+            const uint32_t pitch4 = 4u * (unsigned)G.pitch;
+            const uint32_t K = G.sbase - pitch4 * (unsigned)Cy - 4u * (unsigned)Cx;
+            if (deg == 1) interior_rows<ORDER, 1>(X2, Y2, pitch4, K, rows, r, sink);
+            else if (deg == 2) interior_rows<ORDER, 2>(X2, Y2, pitch4, K, rows, r, sink);
+            else interior_rows<ORDER, 3>(X2, Y2, pitch4, K, rows, r, sink);
+            dj += (float)r;
+        }
+    }
     for (; r + U <= rows; r += U) {
-        f32x2 v[U / 2];
+        float xl[U], yl[U], val[U];
+        bool ok[U];
 #pragma unroll
-        for (int k = 0; k < U / 2; ++k) {
-            v[k] = interior_pair<ORDER, DEG>(X2, Y2, d, pitch4, K);
-            d = add2(d, step);
+        for (int k = 0; k < U; ++k) {
+            const float d = dj + (float)k;
+            xl[k] = fmaf(fmaf(fmaf(X[3], d, X[2]), d, X[1]), d, X[0]);
+            yl[k] = fmaf(fmaf(fmaf(Y[3], d, Y[2]), d, Y[1]), d, Y[0]);
+            val[k] = fast_pixel<ORDER, STAGE>(G, xl[k], yl[k], Cx, Cy, cntx, cnty, ok[k]);
         }
+        bool all_ok = true;
 #pragma unroll
-        for (int k = 0; k < U / 2; ++k) {
-            float lo, hi;
-            unpk2(v[k], lo, hi);
-            orow[(2 * k) * opitch] = lo;
-            orow[(2 * k + 1) * opitch] = hi;
+        for (int k = 0; k < U; ++k) all_ok = all_ok && ok[k];
+        if (!all_ok) {                        // rare: image rim, outside the staged box, NaN
+#pragma unroll
+            for (int k = 0; k < U; ++k)
+                if (!ok[k]) val[k] = slow_poly_pixel<ORDER>(img, P.sny, P.snx, ix0, iy0, xl[k], yl[k]);
         }
-        orow += U * opitch;
+        sink.rows4(val[0], val[1], val[2], val[3]);
+        dj += (float)U;
+    }
+    for (; r < rows; ++r) {                   // ragged bottom edge
+        const float xs = fmaf(fmaf(fmaf(X[3], dj, X[2]), dj, X[1]), dj, X[0]);
+        const float ys = fmaf(fmaf(fmaf(Y[3], dj, Y[2]), dj, Y[1]), dj, Y[0]);
+        bool ok1;
+        float v = fast_pixel<ORDER, STAGE>(G, xs, ys, Cx, Cy, cntx, cnty, ok1);
+        if (!ok1) v = slow_poly_pixel<ORDER>(img, P.sny, P.snx, ix0, iy0, xs, ys);
+        sink.row1(v);
+        dj += 1.0f;
     }
 }
 
@@ -720,104 +846,12 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
         }
     }
     if (!active) return;
-
-    const int tx0 = ttx * TS, ty0 = tty * TS;
-    const int col = tx0 + lane;
-    if (col >= P.onx) return;           // ragged right edge (no block-level sync below)
-    const int rows = min(TS, P.ony - ty0);
-    float *__restrict__ orow = P.out + ((size_t)e * P.ony + ty0) * P.onx + col;
-    const float *__restrict__ img = P.src + (size_t)e * P.sny * P.snx;
-    const size_t opitch = (size_t)P.onx;
-
-    if (flag == TILE_EMPTY) {
-        for (int r = 0; r < rows; ++r) orow[r * opitch] = qnanf();
-        return;
-    }
-    if (flag == TILE_EXACT) {
-        for (int r = 0; r < rows; ++r)
-            orow[r * opitch] = exact_pixel<ORDER>(img, P.sny, P.snx, tgt, P.srcdev[e], col, ty0 + r);
-        return;
-    }
-
-    // ---- per-axis fast-gather constants (a FAST tile in a STAGE kernel always has a box)
-    int Alx, Ahx, Aly, Ahy;
-    if (STAGE) {
-        axis_range<ORDER>(P.snx, ox, P.BW, Alx, Ahx);
-        axis_range<ORDER>(P.sny, oy, P.BH, Aly, Ahy);
-    } else {
-        axis_range<ORDER>(P.snx, -(1 << 28), 1 << 30, Alx, Ahx);
-        axis_range<ORDER>(P.sny, -(1 << 28), 1 << 30, Aly, Ahy);
-    }
-    const unsigned cntx = (unsigned)max(Ahx - Alx + 1, 0), cnty = (unsigned)max(Ahy - Aly + 1, 0);
-    const int Cx = kMagicBits - ix0 + Alx, Cy = kMagicBits - iy0 + Aly;
-    // gather array: element (k = 0) = first tap of base index (Alx, Aly)
-    const int tlo = (ORDER == DFR_BICUBIC) ? 1 : 0;
-    GatherSrc<STAGE> G;
-    if (STAGE) {
-        G.pitch = P.BW;
-        G.sbase = smem_u32(box) + 4u * (unsigned)((Aly - tlo - oy) * P.BW + (Alx - tlo - ox));
-        G.gbase = nullptr;
-    } else {
-        G.pitch = P.snx;
-        G.sbase = 0;
-        G.gbase = img + ((long long)(Aly - tlo) * P.snx + (Alx - tlo));
-    }
-
-    if (deg < 3) { X[3] = 0.0f; Y[3] = 0.0f; }                  // same polynomial on every path
-    if (deg < 2) { X[2] = 0.0f; Y[2] = 0.0f; }
-    constexpr int U = 4;                      // rows in flight per thread
-    float dj = -(float)kCentre;
-    int r = 0;
-    if (STAGE) {
-        // INTERIOR tile: the record's rigorous index range lies inside [Al, Ah] on both axes
-        // (image interior AND staged box), so no pixel needs a range test or the rim rule.
-        const int top = (ORDER == DFR_NEAREST) ? 1 : 0;          // rint(x) <= floor(x) + 1
-        const bool interior = bx0 >= Alx && bx1 + top <= Ahx && by0 >= Aly && by1 + top <= Ahy;
-        if (interior) {
-            f32x2 X2[4], Y2[4];
-#pragma unroll
-            for (int q = 0; q < 4; ++q) { X2[q] = splat2(X[q]); Y2[q] = splat2(Y[q]); }
-            const uint32_t pitch4 = 4u * (unsigned)G.pitch;
-            const uint32_t K = G.sbase - pitch4 * (unsigned)Cy - 4u * (unsigned)Cx;
-            if (deg == 1) interior_rows<ORDER, 1>(X2, Y2, pitch4, K, rows, r, orow, opitch);
-            else if (deg == 2) interior_rows<ORDER, 2>(X2, Y2, pitch4, K, rows, r, orow, opitch);
-            else interior_rows<ORDER, 3>(X2, Y2, pitch4, K, rows, r, orow, opitch);
-            dj += (float)r;
-        }
-    }
-    for (; r + U <= rows; r += U) {
-        float xl[U], yl[U], val[U];
-        bool ok[U];
-#pragma unroll
-        for (int k = 0; k < U; ++k) {
-            const float d = dj + (float)k;
-            xl[k] = fmaf(fmaf(fmaf(X[3], d, X[2]), d, X[1]), d, X[0]);
-            yl[k] = fmaf(fmaf(fmaf(Y[3], d, Y[2]), d, Y[1]), d, Y[0]);
-            val[k] = fast_pixel<ORDER, STAGE>(G, xl[k], yl[k], Cx, Cy, cntx, cnty, ok[k]);
-        }
-        bool all_ok = true;
-#pragma unroll
-        for (int k = 0; k < U; ++k) all_ok = all_ok && ok[k];
-        if (!all_ok) {                        // rare: image rim, outside the staged box, NaN
-#pragma unroll
-            for (int k = 0; k < U; ++k)
-                if (!ok[k]) val[k] = slow_poly_pixel<ORDER>(img, P.sny, P.snx, ix0, iy0, xl[k], yl[k]);
-        }
-#pragma unroll
-        for (int k = 0; k < U; ++k) orow[k * opitch] = val[k];
-        orow += U * opitch;
-        dj += (float)U;
-    }
-    for (; r < rows; ++r) {                   // ragged bottom edge
-        const float xs = fmaf(fmaf(fmaf(X[3], dj, X[2]), dj, X[1]), dj, X[0]);
-        const float ys = fmaf(fmaf(fmaf(Y[3], dj, Y[2]), dj, Y[1]), dj, Y[0]);
-        bool ok1;
-        float v = fast_pixel<ORDER, STAGE>(G, xs, ys, Cx, Cy, cntx, cnty, ok1);
-        if (!ok1) v = slow_poly_pixel<ORDER>(img, P.sny, P.snx, ix0, iy0, xs, ys);
-        *orow = v;
-        orow += opitch;
-        dj += 1.0f;
-    }
+    TileHead H;
+    H.flag = flag; H.ix0 = ix0; H.iy0 = iy0; H.bx0 = bx0; H.by0 = by0; H.bx1 = bx1; H.by1 = by1; H.deg = deg;
+    StoreSink sink;
+    sink.orow = P.out + ((size_t)e * P.ony + (size_t)tty * TS) * P.onx + (ttx * TS + lane);
+    sink.opitch = (size_t)P.onx;
+    warp_tile<ORDER, STAGE>(P, tgt, e, ttx, tty, lane, H, X, Y, smem_u32(box), ox, oy, sink);
 }
 
 // coordinates the tiled path uses (dfr_src_coords): same records, same polynomial code
