@@ -121,6 +121,33 @@ int dfr_reproject_host(const float *src_host, int32_t n, int32_t src_ny, int32_t
                        int32_t out_ny, int32_t out_nx, int32_t order,
                        float *out_host, int32_t batch);
 
+/* ---- fused reproject-and-stack --------- */
+
+/* The paper's stated purpose of reprojection is that images "can be combined to
+ * produce a single, deeper image". This entry point does both in
+ * one kernel, so the n per-exposure frames never reach HBM:
+ *   sum [j][i] (+)= sum over e of weights[e] * v_e(i, j)
+ *   wsum[j][i] (+)= sum over the same e of weights[e]
+ * where v_e is what dfr_reproject would store for exposure e, and exposure e
+ * contributes to a pixel only where v_e is not NaN (inside its footprint and no
+ * NaN under the taps). Accumulation is float32, in exposure order.
+ *   src_batch, src_wcs, tgt_wcs, out_ny/nx, order : as dfr_reproject
+ *   weights    : HOST float32[n], or NULL for 1.0 each (must be finite)
+ *   sum, wsum  : DEVICE float32 [out_ny][out_nx] each; must not overlap src_batch
+ *                or each other
+ *   accumulate : 0 = both arrays are overwritten; 1 = the batch is added to their
+ *                current contents (co-adding a stream of batches)
+ * The mean image is sum / wsum (dfr_stack_finalize). Errors as dfr_reproject. */
+int dfr_reproject_stack(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+                        const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                        int32_t out_ny, int32_t out_nx, int32_t order,
+                        const float *weights, float *sum, float *wsum, int32_t accumulate,
+                        void *stream);
+
+/* mean[k] = sum[k] / wsum[k], NaN where wsum[k] == 0. DEVICE float32[npix] each;
+ * mean may be the same array as sum. */
+int dfr_stack_finalize(const float *sum, const float *wsum, int64_t npix, float *mean, void *stream);
+
 /* ---- coordinate entry points, for testing (§3.2.1 / §3.2.2) ---- */
 
 /* Pixel -> sky with WCS *w (HOST). x, y, ra_deg, dec_deg: DEVICE double[npts].
@@ -148,7 +175,7 @@ int dfr_src_coords(int32_t n, int32_t src_ny, int32_t src_nx,
 /* CD_ij = CDELT_i * PC_ij (FITS Paper I). HOST only. */
 int dfr_wcs_set_pc_cdelt(dfr_wcs *w, const double pc[4], const double cdelt[2]);
 
-/* Counters of the last dfr_reproject / dfr_reproject_ex call on this thread (HOST):
+/* Counters of the last dfr_reproject* call on this thread (HOST):
  * stats[0] = tiles on the fast path, [1] = tiles on the exact path,
  * [2] = tiles entirely outside the footprint, [3] = kernels launched. */
 int dfr_last_stats(int64_t stats[4]);

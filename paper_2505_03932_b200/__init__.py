@@ -19,7 +19,8 @@ NEAREST, BILINEAR, BICUBIC = 0, 1, 3
 PATH_AUTO, PATH_EXACT, PATH_TILED = 0, 1, 2
 _ORDER_NAMES = {"nearest": 0, "nearest-neighbor": 0, "bilinear": 1, "bicubic": 3}
 
-EXPORTS = ["dfr_reproject", "dfr_reproject_ex", "dfr_reproject_host", "dfr_pix2world",
+EXPORTS = ["dfr_reproject", "dfr_reproject_ex", "dfr_reproject_host", "dfr_reproject_stack",
+           "dfr_stack_finalize", "dfr_pix2world",
            "dfr_world2pix", "dfr_src_coords", "dfr_wcs_set_pc_cdelt", "dfr_last_stats",
            "dfr_profile_enable", "dfr_profile_last",
            "dfr_strerror", "dfr_last_error", "dfr_version"]
@@ -56,6 +57,9 @@ def lib():
         L.dfr_reproject.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, vp]
         L.dfr_reproject_ex.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, vp, i32]
         L.dfr_reproject_host.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, i32]
+        L.dfr_reproject_stack.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32,
+                                          C.POINTER(C.c_float), fp, fp, i32, vp]
+        L.dfr_stack_finalize.argtypes = [fp, fp, i64, fp, vp]
         L.dfr_pix2world.argtypes = [wp, dp, dp, i64, dp, dp, vp]
         L.dfr_world2pix.argtypes = [wp, dp, dp, i64, dp, dp, vp]
         L.dfr_src_coords.argtypes = [i32, i32, i32, wp, wp, i32, i32, i32, dp, dp, vp, i32]
@@ -171,6 +175,56 @@ def dfr_reproject_host(src_host, src_wcs, tgt_wcs, shape_out=None, order=BILINEA
     _check(lib().dfr_reproject_host(src_t.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx,
                                     _order(order), out_t.data_ptr(), int(batch)))
     return out_host
+
+
+def dfr_reproject_stack(src_batch, src_wcs, tgt_wcs, shape_out=None, order=BILINEAR, weights=None,
+                        sum=None, wsum=None, accumulate=False, stream=None):
+    """dfr_reproject_stack (include/dfr.h): fused reprojection + co-addition. Returns the
+    CUDA float32 (sum, wsum) [out_ny][out_nx]; pass them back with accumulate=True to add
+    further batches."""
+    import torch
+    if src_batch.dim() == 2:
+        src_batch = src_batch[None]
+    _need_cuda(src_batch, torch.float32, "src_batch")
+    n, sny, snx = src_batch.shape
+    ony, onx = (sny, snx) if shape_out is None else (int(shape_out[0]), int(shape_out[1]))
+    ws = pack_wcs_array(src_wcs)
+    if len(ws) != n:
+        raise ValueError("one source WCS per exposure")
+    tw = pack_wcs(tgt_wcs)
+    if sum is None:
+        sum = torch.empty((ony, onx), dtype=torch.float32, device=src_batch.device)
+    if wsum is None:
+        wsum = torch.empty((ony, onx), dtype=torch.float32, device=src_batch.device)
+    for t, name in ((sum, "sum"), (wsum, "wsum")):
+        _need_cuda(t, torch.float32, name)
+        if tuple(t.shape) != (ony, onx):
+            raise ValueError(f"{name} has the wrong shape")
+    wp = None
+    if weights is not None:
+        w = np.ascontiguousarray(weights, dtype=np.float32)
+        if w.size != n:
+            raise ValueError("one weight per exposure")
+        wp = w.ctypes.data_as(C.POINTER(C.c_float))
+    with torch.cuda.device(src_batch.device):
+        _check(lib().dfr_reproject_stack(src_batch.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx,
+                                         _order(order), wp, sum.data_ptr(), wsum.data_ptr(),
+                                         1 if accumulate else 0, _stream_ptr(stream)))
+    return sum, wsum
+
+
+def dfr_stack_finalize(sum, wsum, mean=None, stream=None):
+    """dfr_stack_finalize: mean = sum / wsum, NaN where wsum == 0."""
+    import torch
+    _need_cuda(sum, torch.float32, "sum")
+    _need_cuda(wsum, torch.float32, "wsum")
+    if mean is None:
+        mean = torch.empty_like(sum)
+    _need_cuda(mean, torch.float32, "mean")
+    with torch.cuda.device(sum.device):
+        _check(lib().dfr_stack_finalize(sum.data_ptr(), wsum.data_ptr(), sum.numel(), mean.data_ptr(),
+                                        _stream_ptr(stream)))
+    return mean
 
 
 def dfr_pix2world(wcs, x, y, stream=None):

@@ -1,6 +1,7 @@
 // dfr_api.cu — the C ABI of include/dfr.h: argument validation, host
 // pre-composition, stream-ordered scratch, kernel launches. No compute happens
 // on the host beyond the O(n) per-exposure constant folding of dfr_host.cu.
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <mutex>
@@ -200,6 +201,69 @@ int dfr_src_coords(int32_t n, int32_t src_ny, int32_t src_nx,
     cudaFreeAsync(dsrc, st);
     if (err != cudaSuccess) return cuda_fail(err, "src_coords launch");
     return DFR_OK;
+}
+
+int dfr_reproject_stack(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+                        const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                        int32_t out_ny, int32_t out_nx, int32_t order,
+                        const float *weights, float *sum, float *wsum, int32_t accumulate,
+                        void *stream)
+{
+    if (!src_batch || !sum || !wsum) { set_error("NULL image pointer"); return DFR_ERR_NULL; }
+    int rc = check_common(n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order);
+    if (rc != DFR_OK) return rc;
+    const char *s0 = (const char *)src_batch, *s1 = s0 + sizeof(float) * (size_t)n * src_ny * src_nx;
+    const size_t ob = sizeof(float) * (size_t)out_ny * out_nx;
+    const char *a0 = (const char *)sum, *b0 = (const char *)wsum;
+    if ((a0 < s1 && s0 < a0 + ob) || (b0 < s1 && s0 < b0 + ob) || (a0 < b0 + ob && b0 < a0 + ob)) {
+        set_error("sum / wsum overlap src_batch or each other");
+        return DFR_ERR_ALIAS;
+    }
+    std::vector<float> hw((size_t)n, 1.0f);
+    if (weights)
+        for (int32_t e = 0; e < n; ++e) {
+            if (!std::isfinite(weights[e])) { set_error("weights[%d] is not finite", e); return DFR_ERR_NONFINITE_WCS; }
+            hw[e] = weights[e];
+        }
+    std::call_once(g_pool_once, tune_pool);
+    cudaStream_t st = (cudaStream_t)stream;
+    g_last.pending = false;
+    TargetDev tgt;
+    make_target(tgt_wcs, &tgt);
+    std::vector<SourceDev> hsrc;
+    SourceDev *dsrc = nullptr;
+    rc = upload_sources(n, src_wcs, tgt_wcs, st, hsrc, &dsrc);
+    if (rc != DFR_OK) return rc;
+    float *dw = nullptr;
+    int32_t *dcnt = nullptr;
+    TiledStats ts = {0, 0, 0, 0};
+    cudaError_t err = ensure_last();
+    if (err == cudaSuccess) err = cudaMallocAsync((void **)&dw, sizeof(float) * (size_t)n, st);
+    // pageable source: the runtime stages the bytes before returning, so `hw` may die
+    if (err == cudaSuccess) err = cudaMemcpyAsync(dw, hw.data(), sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, st);
+    if (err == cudaSuccess) err = cudaMallocAsync((void **)&dcnt, 4 * sizeof(int32_t), st);
+    if (err == cudaSuccess)
+        err = launch_tiled_stack(src_batch, n, src_ny, src_nx, tgt, dsrc, hsrc.data(), out_ny, out_nx, order,
+                                 dw, sum, wsum, accumulate != 0, st, dcnt, &ts, &g_last.prof);
+    if (err == cudaSuccess)
+        err = cudaMemcpyAsync(g_last.pinned, dcnt, 3 * sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+    if (err == cudaSuccess) err = cudaEventRecord(g_last.done, st);
+    if (dcnt) cudaFreeAsync(dcnt, st);
+    if (dw) cudaFreeAsync(dw, st);
+    cudaFreeAsync(dsrc, st);
+    g_last.kernels = ts.kernels;
+    g_last.tiled = true;
+    g_last.pending = (err == cudaSuccess);
+    if (err != cudaSuccess) return cuda_fail(err, "reproject_stack launch");
+    return DFR_OK;
+}
+
+int dfr_stack_finalize(const float *sum, const float *wsum, int64_t npix, float *mean, void *stream)
+{
+    if (npix < 0) { set_error("npix < 0"); return DFR_ERR_SHAPE; }
+    if (npix > 0 && (!sum || !wsum || !mean)) { set_error("NULL pointer"); return DFR_ERR_NULL; }
+    cudaError_t err = launch_stack_finalize(sum, wsum, (long long)npix, mean, (cudaStream_t)stream);
+    return err == cudaSuccess ? DFR_OK : cuda_fail(err, "stack_finalize launch");
 }
 
 static int sky_common(const dfr_wcs *w, const void *a, const void *b, const void *c, const void *d,

@@ -368,6 +368,7 @@ struct TiledParams {
     int n, e0, sny, snx, ony, onx;                 // e0: first exposure of this launch
     int tiles_x, tiles_y, ctas_x, ctas_y;
     int BW, BH;                                    // staged box (STAGE) in source pixels
+    int stage_bytes;                               // stack kernel: bytes per box stage
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
@@ -618,6 +619,18 @@ __device__ __forceinline__ f32x2 interior_pair(const f32x2 (&X)[4], const f32x2 
     return acc;
 }
 
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t done = 0;
+    while (!done) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    }
+}
+
 // Where the values of a tile go. A sink receives the rows of a tile in increasing order:
 // rows4(v) = the next four rows, row1(v) = the next single row (ragged bottom edge).
 // StoreSink: the per-exposure output of dfr_reproject (one coalesced 128-byte row per warp).
@@ -625,6 +638,7 @@ struct StoreSink {
     static constexpr bool kAllLanes = false;       // lanes beyond the right edge may leave early
     float *__restrict__ orow;
     size_t opitch;
+    __device__ __forceinline__ void prefetch4() {}
     __device__ __forceinline__ void rows4(float v0, float v1, float v2, float v3)
     {
         orow[0] = v0;
@@ -652,6 +666,7 @@ __device__ __forceinline__ void interior_rows(const f32x2 (&X2)[4], const f32x2 
     f32x2 d = pk2(-(float)kCentre, 1.0f - (float)kCentre);
     const f32x2 step = splat2(2.0f);
     for (; r + 4 <= rows; r += 4) {
+        sink.prefetch4();
         const f32x2 va = interior_pair<ORDER, DEG>(X2, Y2, d, pitch4, K);
         d = add2(d, step);
         const f32x2 vb = interior_pair<ORDER, DEG>(X2, Y2, d, pitch4, K);
@@ -740,6 +755,7 @@ __device__ __forceinline__ void warp_tile(const TiledParams &P, const TargetDev 
         }
     }
     for (; r + U <= rows; r += U) {
+        sink.prefetch4();
         float xl[U], yl[U], val[U];
         bool ok[U];
 #pragma unroll
@@ -852,6 +868,209 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
     sink.orow = P.out + ((size_t)e * P.ony + (size_t)tty * TS) * P.onx + (ttx * TS + lane);
     sink.opitch = (size_t)P.onx;
     warp_tile<ORDER, STAGE>(P, tgt, e, ttx, tty, lane, H, X, Y, smem_u32(box), ox, oy, sink);
+}
+
+// ---------------------------------------------------------------------------------
+// fused reproject-and-stack (dfr_reproject_stack)
+//
+// One CTA per 64x64 output tile loops over the exposures; the per-pixel accumulators
+//   sum += w_e v_e,  wsum += w_e   (only where v_e is not NaN)
+// of each warp's 32x32 tile (2 x 32 rows per lane) live in TENSOR MEMORY: 64 TMEM columns
+// per CTA, lane = output column, column = row (sum) / 32 + row (wsum), read and written
+// four rows at a time with tcgen05.ld / tcgen05.st (32x32b.x4). They never occupy
+// registers for longer than four pixels, there is no per-exposure output in HBM, and the
+// row loop stays a loop. The source boxes arrive through a two-stage TMA ring: while
+// exposure e is accumulated out of stage e & 1, the box of e + 1 is in flight.
+// ---------------------------------------------------------------------------------
+struct StackSink {
+    static constexpr bool kAllLanes = true;        // tcgen05.ld/st are warp-wide: nobody leaves
+    uint32_t taddr;                                // TMEM address of this warp's row 0 (sum)
+    float w;                                       // weight of the current exposure
+    int r;                                         // next row
+    float s0, s1, s2, s3, c0, c1, c2, c3;          // accumulators of rows r .. r + 3 in flight
+    __device__ __forceinline__ void prefetch4()
+    {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                     : "=f"(s0), "=f"(s1), "=f"(s2), "=f"(s3) : "r"(taddr + (uint32_t)r));
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                     : "=f"(c0), "=f"(c1), "=f"(c2), "=f"(c3) : "r"(taddr + (uint32_t)(TS + r)));
+    }
+    __device__ __forceinline__ void add(float &s, float &c, float v) const
+    {
+        const bool ok = v == v;                    // NaN: outside the footprint, or NaN taps
+        s = ok ? fmaf(w, v, s) : s;
+        c = ok ? c + w : c;
+    }
+    __device__ __forceinline__ void rows4(float v0, float v1, float v2, float v3)
+    {
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        add(s0, c0, v0); add(s1, c1, v1); add(s2, c2, v2); add(s3, c3, v3);
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
+                     ::"r"(taddr + (uint32_t)r), "f"(s0), "f"(s1), "f"(s2), "f"(s3) : "memory");
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
+                     ::"r"(taddr + (uint32_t)(TS + r)), "f"(c0), "f"(c1), "f"(c2), "f"(c3) : "memory");
+        r += 4;
+    }
+    __device__ __forceinline__ void row1(float v)
+    {
+        float s, c;
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=f"(s) : "r"(taddr + (uint32_t)r));
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=f"(c) : "r"(taddr + (uint32_t)(TS + r)));
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        add(s, c, v);
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(taddr + (uint32_t)r), "f"(s) : "memory");
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(taddr + (uint32_t)(TS + r)), "f"(c) : "memory");
+        r += 1;
+    }
+    __device__ __forceinline__ void empty_tile(int) {}           // an empty tile adds nothing
+};
+
+constexpr int kStackCols = 2 * TS;                 // TMEM columns per CTA (power of two >= 32)
+
+struct StackParams {
+    const float *weights;                          // DEVICE [n]
+    float *sum, *wsum;                             // DEVICE [ony][onx]
+    int accumulate;                                // 0: overwrite, 1: add to the current contents
+};
+
+template <int ORDER, bool STAGE>
+__global__ void __launch_bounds__(32 * CTA_T * CTA_T)
+tiled_stack_kernel(const __grid_constant__ TiledParams P, const __grid_constant__ TargetDev tgt,
+                   const __grid_constant__ CUtensorMap tmap, const __grid_constant__ StackParams S)
+{
+    extern __shared__ __align__(128) unsigned char stages[];       // 2 boxes (STAGE)
+    __shared__ __align__(8) unsigned long long full[2];
+    __shared__ int4 head[2];                                       // has_box, ox, oy
+    __shared__ uint32_t tmem_base;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int ttx = blockIdx.x * CTA_T + (warp % CTA_T), tty = blockIdx.y * CTA_T + (warp / CTA_T);
+    const bool active = ttx < P.tiles_x && tty < P.tiles_y;
+    const int ntile = P.tiles_x * P.tiles_y, ctas = P.ctas_x * P.ctas_y;
+    const int tile = active ? tty * P.tiles_x + ttx : 0;
+    const int cta = blockIdx.y * P.ctas_x + blockIdx.x;
+    const uint32_t box_bytes = (uint32_t)(P.BW * P.BH * sizeof(float));
+
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                     ::"r"(smem_u32(&tmem_base)), "n"(kStackCols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    if (STAGE && threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&full[0])));
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&full[1])));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+
+    StackSink sink;
+    sink.taddr = tmem_base + ((uint32_t)(warp * 32) << 16);
+    sink.w = 0.0f;
+    sink.r = 0;
+    for (int g = 0; g < kStackCols; g += 4)                        // zero sum and wsum
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %1, %1, %1};"
+                     ::"r"(sink.taddr + (uint32_t)g), "f"(0.0f) : "memory");
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+
+    // thread 0: stage head + expect_tx + TMA box load of exposure e into stage s
+    auto issue = [&](int e, int s, int2 cb) {
+        const int hb = cb.x != kNoBox;
+        // TMA wants a 16-byte aligned start along x (measured on B200): round down to 4 floats
+        const int ox = (cb.x - (Taps<ORDER>::lo + 1)) & ~3, oy = cb.y - (Taps<ORDER>::lo + 1);
+        head[s] = make_int4(hb, ox, oy, 0);
+        const uint32_t bar = smem_u32(&full[s]);
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(hb ? box_bytes : 0u) : "memory");
+        if (hb)
+            asm volatile(
+                "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                ::"r"(smem_u32(stages + (size_t)s * P.stage_bytes)), "l"(&tmap), "r"(ox), "r"(oy), "r"(e), "r"(bar) : "memory");
+    };
+    if (STAGE && threadIdx.x == 0) {
+        issue(0, 0, __ldg(P.cta_box + cta));
+        if (P.n > 1) issue(1, 1, __ldg(P.cta_box + (size_t)ctas + cta));
+    }
+
+    for (int e = 0; e < P.n; ++e) {
+        const int s = e & 1;
+        int2 cb2 = make_int2(kNoBox, kNoBox);
+        if (STAGE && threadIdx.x == 0 && e + 2 < P.n) cb2 = __ldg(P.cta_box + (size_t)(e + 2) * ctas + cta);
+        // this exposure's record (requested before the box is waited for)
+        const TileRec *rec = P.recs + ((size_t)e * ntile + tile);
+        const int4 h0 = __ldg(reinterpret_cast<const int4 *>(&rec->ix0));       // ix0 iy0 bx0 by0
+        const int4 h1 = __ldg(reinterpret_cast<const int4 *>(&rec->bx1));       // bx1 by1 flag deg
+        TileHead H;
+        H.ix0 = h0.x; H.iy0 = h0.y; H.bx0 = h0.z; H.by0 = h0.w; H.bx1 = h1.x; H.by1 = h1.y; H.flag = h1.z; H.deg = h1.w;
+        float X[4], Y[4];
+        {
+            const float di = (float)lane - (float)kCentre;
+            const float4 *c4 = reinterpret_cast<const float4 *>(rec->cx);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float4 a = __ldg(c4 + q), b = __ldg(c4 + 4 + q);
+                X[q] = fmaf(fmaf(fmaf(a.w, di, a.z), di, a.y), di, a.x);
+                Y[q] = fmaf(fmaf(fmaf(b.w, di, b.z), di, b.y), di, b.x);
+            }
+        }
+        sink.w = __ldg(S.weights + e);
+        sink.r = 0;
+        int ox = 0, oy = 0;
+        if (STAGE) {
+            mbar_wait(smem_u32(&full[s]), (uint32_t)(e >> 1) & 1u);
+            const int4 hd = head[s];
+            ox = hd.y; oy = hd.z;
+        }
+        if (active)
+            warp_tile<ORDER, STAGE>(P, tgt, e, ttx, tty, lane, H, X, Y,
+                                    smem_u32(stages + (size_t)s * P.stage_bytes), ox, oy, sink);
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        if (STAGE) {
+            __syncthreads();                            // every warp is done with stage s
+            if (threadIdx.x == 0 && e + 2 < P.n) issue(e + 2, s, cb2);
+        }
+    }
+
+    // ---- epilogue: accumulators -> sum, wsum (one coalesced 128-byte row per warp and row)
+    if (active) {
+        const int col = ttx * TS + lane, ty0 = tty * TS;
+        const int rows = min(TS, P.ony - ty0);
+        for (int r = 0; r < TS; r += 4) {
+            float a[4], c[4];
+            asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                         : "=f"(a[0]), "=f"(a[1]), "=f"(a[2]), "=f"(a[3]) : "r"(sink.taddr + (uint32_t)r));
+            asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                         : "=f"(c[0]), "=f"(c[1]), "=f"(c[2]), "=f"(c[3]) : "r"(sink.taddr + (uint32_t)(TS + r)));
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (r + k < rows && col < P.onx) {
+                    const size_t o = (size_t)(ty0 + r + k) * P.onx + col;
+                    if (S.accumulate) {
+                        S.sum[o] += a[k];
+                        S.wsum[o] += c[k];
+                    } else {
+                        S.sum[o] = a[k];
+                        S.wsum[o] = c[k];
+                    }
+                }
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 0)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kStackCols) : "memory");
+}
+
+__global__ void stack_finalize_kernel(const float *__restrict__ sum, const float *__restrict__ wsum,
+                                      long long npix, float *__restrict__ mean)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < npix) {
+        const float w = wsum[i];
+        mean[i] = (w != 0.0f) ? sum[i] / w : qnanf();
+    }
 }
 
 // coordinates the tiled path uses (dfr_src_coords): same records, same polynomial code
@@ -1026,25 +1245,25 @@ static void free_scratch(Scratch &sc, cudaStream_t st)
     if (sc.cta_box) cudaFreeAsync(sc.cta_box, st);
 }
 
-cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
-                                   const TargetDev &tgt, const SourceDev *srcdev,
-                                   const SourceDev *srchost,
-                                   int ony, int onx, int order, float *out, cudaStream_t st,
-                                   int32_t *dev_counters, TiledStats *stats, ProfileEvents *prof)
-{
+// Setup kernels + staging decision shared by the per-exposure and the stacking launchers.
+struct Prepared {
     TiledParams P;
-    std::memset(&P, 0, sizeof P);
-    P.src = src;
-    P.out = out;
     Scratch sc;
-    if (prof && prof->enabled) cudaEventRecord(prof->setup_begin, st);
-    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, srchost, ony, onx, st, dev_counters, sc, P);
-    if (err != cudaSuccess) { free_scratch(sc, st); return err; }
-
-    // ---- staging decision: box size from a host probe; TMA needs 16-byte rows
-    bool stage = false;
     CUtensorMap tmap;
-    std::memset(&tmap, 0, sizeof tmap);
+    bool stage = false;
+    size_t box_bytes = 0;
+};
+
+static cudaError_t prepare_tiled(const float *src, int n, int sny, int snx, const TargetDev &tgt,
+                                 const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx,
+                                 int order, cudaStream_t st, int32_t *dev_counters, Prepared &R)
+{
+    std::memset(&R.P, 0, sizeof R.P);
+    std::memset(&R.tmap, 0, sizeof R.tmap);
+    R.P.src = src;
+    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, srchost, ony, onx, st, dev_counters, R.sc, R.P);
+    if (err != cudaSuccess) return err;
+    // ---- staging decision: box size from a host probe; TMA needs 16-byte rows
     double ex, ey;
     const int tlo = (order == DFR_BICUBIC) ? 1 : 0, thi = (order == DFR_BICUBIC) ? 2 : 1;
     EncodeTiledFn enc = get_encode();
@@ -1059,25 +1278,89 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
             const cuuint64_t strides[2] = {(cuuint64_t)snx * 4, (cuuint64_t)snx * sny * 4};
             const cuuint32_t boxd[3] = {(cuuint32_t)bw, (cuuint32_t)bh, 1};
             const cuuint32_t estr[3] = {1, 1, 1};
-            CUresult r = enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)src, dims, strides, boxd, estr,
+            CUresult r = enc(&R.tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)src, dims, strides, boxd, estr,
                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-            if (r == CUDA_SUCCESS) { stage = true; P.BW = bw; P.BH = bh; }
+            if (r == CUDA_SUCCESS) { R.stage = true; R.P.BW = bw; R.P.BH = bh; }
         }
     }
-    const size_t smem = stage ? (size_t)P.BW * P.BH * sizeof(float) : 0;
+    R.box_bytes = R.stage ? (size_t)R.P.BW * R.P.BH * sizeof(float) : 0;
+    return cudaSuccess;
+}
+
+cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
+                                   const TargetDev &tgt, const SourceDev *srcdev,
+                                   const SourceDev *srchost,
+                                   int ony, int onx, int order, float *out, cudaStream_t st,
+                                   int32_t *dev_counters, TiledStats *stats, ProfileEvents *prof)
+{
+    Prepared R;
+    if (prof && prof->enabled) cudaEventRecord(prof->setup_begin, st);
+    cudaError_t err = prepare_tiled(src, n, sny, snx, tgt, srcdev, srchost, ony, onx, order, st, dev_counters, R);
+    if (err != cudaSuccess) { free_scratch(R.sc, st); return err; }
+    R.P.out = out;
     if (prof && prof->enabled) cudaEventRecord(prof->main_begin, st);
 #define DFR_LAUNCH(O)                                                                     \
-    err = stage ? launch_main<O, true>(P, tgt, tmap, smem, st) : launch_main<O, false>(P, tgt, tmap, 0, st)
+    err = R.stage ? launch_main<O, true>(R.P, tgt, R.tmap, R.box_bytes, st) : launch_main<O, false>(R.P, tgt, R.tmap, 0, st)
     if (order == DFR_NEAREST) DFR_LAUNCH(DFR_NEAREST);
     else if (order == DFR_BILINEAR) DFR_LAUNCH(DFR_BILINEAR);
     else DFR_LAUNCH(DFR_BICUBIC);
 #undef DFR_LAUNCH
     if (prof && prof->enabled) cudaEventRecord(prof->main_end, st);
-    free_scratch(sc, st);
+    free_scratch(R.sc, st);
     stats->kernels = 3;
     stats->tiles_fast = stats->tiles_exact = stats->tiles_empty = -1;   // filled from dev_counters by the caller
     return err;
+}
+
+template <int ORDER, bool STAGE>
+static cudaError_t launch_stack(TiledParams P, const TargetDev &tgt, const CUtensorMap &tmap, size_t box_bytes,
+                                const StackParams &S, cudaStream_t st)
+{
+    auto kern = tiled_stack_kernel<ORDER, STAGE>;
+    P.stage_bytes = (int)((box_bytes + 127) & ~(size_t)127);
+    const size_t smem = STAGE ? 2 * (size_t)P.stage_bytes : 0;
+    if (STAGE) {
+        cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (err != cudaSuccess) return err;
+    }
+    if (P.ctas_y > 65535) return cudaErrorInvalidConfiguration;
+    P.e0 = 0;
+    const dim3 grid((unsigned)P.ctas_x, (unsigned)P.ctas_y, 1);
+    kern<<<grid, 32 * CTA_T * CTA_T, smem, st>>>(P, tgt, tmap, S);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_tiled_stack(const float *src, int n, int sny, int snx, const TargetDev &tgt,
+                               const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx, int order,
+                               const float *dev_weights, float *sum, float *wsum, int accumulate,
+                               cudaStream_t st, int32_t *dev_counters, TiledStats *stats, ProfileEvents *prof)
+{
+    Prepared R;
+    if (prof && prof->enabled) cudaEventRecord(prof->setup_begin, st);
+    cudaError_t err = prepare_tiled(src, n, sny, snx, tgt, srcdev, srchost, ony, onx, order, st, dev_counters, R);
+    if (err != cudaSuccess) { free_scratch(R.sc, st); return err; }
+    StackParams S;
+    S.weights = dev_weights; S.sum = sum; S.wsum = wsum; S.accumulate = accumulate;
+    if (prof && prof->enabled) cudaEventRecord(prof->main_begin, st);
+#define DFR_LAUNCH(O)                                                                     \
+    err = R.stage ? launch_stack<O, true>(R.P, tgt, R.tmap, R.box_bytes, S, st) : launch_stack<O, false>(R.P, tgt, R.tmap, 0, S, st)
+    if (order == DFR_NEAREST) DFR_LAUNCH(DFR_NEAREST);
+    else if (order == DFR_BILINEAR) DFR_LAUNCH(DFR_BILINEAR);
+    else DFR_LAUNCH(DFR_BICUBIC);
+#undef DFR_LAUNCH
+    if (prof && prof->enabled) cudaEventRecord(prof->main_end, st);
+    free_scratch(R.sc, st);
+    stats->kernels = 3;
+    stats->tiles_fast = stats->tiles_exact = stats->tiles_empty = -1;
+    return err;
+}
+
+cudaError_t launch_stack_finalize(const float *sum, const float *wsum, long long npix, float *mean, cudaStream_t st)
+{
+    if (npix <= 0) return cudaSuccess;
+    stack_finalize_kernel<<<(unsigned)((npix + 255) / 256), 256, 0, st>>>(sum, wsum, npix, mean);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_tiled_coords(int n, int sny, int snx, const TargetDev &tgt,

@@ -1,0 +1,149 @@
+"""-m gpu: dfr_reproject_stack (fused reproject-and-stack) against the
+oracle's orc_stack on the same seeded inputs, through the C ABI.
+
+Tolerances: every exposure's value is within VALUE_TOL x DR of the oracle's,
+so |sum_gpu - sum_orc| <= VALUE_TOL x DR x sum_e |w_e| (+ float32 accumulation, which is far
+below it); wsum must be identical; pixels where ANY exposure's oracle coordinate lies
+within EDGE_BAND of its footprint edge are compared only for consistency (wsum may differ
+by that exposure's weight there)."""
+import numpy as np
+import pytest
+
+import dfr_synth as S
+import oracle
+from tests import parity as PR
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2505_03932_b200 as pkg
+    pkg.lib()
+    return pkg
+
+
+def check_stack(P, w, order, weights=None, tol_scale=1.0):
+    n = len(w.src_wcs)
+    sny, snx = w.images.shape[1:]
+    src = torch.from_numpy(w.images).cuda()
+    s, ws = P.dfr_reproject_stack(src, w.src_wcs, w.tgt_wcs, w.shape_out, order, weights=weights)
+    torch.cuda.synchronize()
+    s, ws = s.cpu().numpy(), ws.cpu().numpy()
+    so, wo = oracle.stack(w.images, w.src_wcs, w.tgt_wcs, w.shape_out, order, weights)
+    band = np.zeros(w.shape_out, dtype=bool)
+    tie = np.zeros(w.shape_out, dtype=bool)
+    for e in range(n):
+        xo, yo = oracle.src_coords(w.tgt_wcs, w.src_wcs[e], *w.shape_out)
+        band |= PR.edge_band(xo, yo, sny, snx)
+        if order == 0:
+            tie |= ((np.abs(xo - np.floor(xo) - 0.5) < PR.TIE_BAND) | (np.abs(yo - np.floor(yo) - 0.5) < PR.TIE_BAND))
+    assert not np.isnan(s).any() and not np.isnan(ws).any()
+    assert np.array_equal(ws[~band], wo[~band]), "weight sums differ away from footprint edges"
+    wabs = np.abs(np.ones(n) if weights is None else np.asarray(weights, dtype=np.float64)).sum()
+    dr = max(PR.dyn_range(im) for im in w.images)
+    ok = ~band & ~tie
+    err = np.abs(s[ok].astype(np.float64) - so[ok])
+    lim = tol_scale * PR.VALUE_TOL * dr * wabs
+    assert err.max() <= lim, f"stack parity: max {err.max():.3e} > {lim:.3e}"
+    return {"max": float(err.max()), "lim": lim, "depth_max": float(wo.max()), "depth0_frac": float((wo == 0).mean()),
+            "band_px": int(band.sum())}
+
+
+@pytest.mark.parametrize("order", [0, 1, 3])
+def test_stack_small_batch_all_orders(P, order):
+    """Ragged shapes, rotated + SIP exposures overlapping partially, random weights."""
+    rng = np.random.default_rng(61)
+    sny, snx, ony, onx = 140, 212, 150, 177
+    n = 5
+    imgs = np.stack([S.make_image(sny, snx, 30, rng) for _ in range(n)])
+    srcs = [S.add_sip(S.make_wcs(snx, sny, 150.0 + 0.004 * rng.uniform(-1, 1), 2.0 + 0.004 * rng.uniform(-1, 1),
+                                 rng.uniform(-20, 20), S.PIXSCALE), 3, snx / 2.0, rng, amp=1e-4) for _ in range(n)]
+    tgt = S.add_sip(S.make_wcs(onx, ony, 150.001, 2.0005, 4.0, S.PIXSCALE * 1.03), 3, onx / 2.0, rng, amp=1e-4)
+    w = S.Workload("stack-ragged", imgs, srcs, tgt, (ony, onx), (order,))
+    wts = rng.integers(4, 17, n) / 8.0          # multiples of 1/8: every partial sum is exact in float32
+    st = check_stack(P, w, order, wts)
+    assert st["depth_max"] > 3.0 and st["depth0_frac"] < 0.5
+    print("stack ragged", order, st)
+
+
+def test_stack_single_exposure_equals_reproject(P):
+    w = S.config0()
+    src = torch.from_numpy(w.images).cuda()
+    out = P.dfr_reproject(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1)[0]
+    s, ws = P.dfr_reproject_stack(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1)
+    m = torch.isnan(out)
+    assert torch.equal(ws, (~m).float())
+    assert torch.equal(s[~m], out[~m]) and bool((s[m] == 0).all())        # bit exact: w = 1
+    mean = P.dfr_stack_finalize(s, ws)
+    assert torch.equal(torch.isnan(mean), m) and torch.equal(mean[~m], out[~m])
+
+
+def test_stack_accumulate_over_batches_and_nan_pixels(P):
+    """Two calls with accumulate=True equal one call over all exposures up to float32
+    re-association (the second batch is summed before it is added); a NaN source pixel is
+    skipped by its exposure only."""
+    w = S.config2(batch=6, n=512, nstars=300)
+    w.images[2, 100:110, 200:230] = np.nan
+    src = torch.from_numpy(w.images).cuda()
+    s_all, w_all = P.dfr_reproject_stack(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1)
+    s, ws = P.dfr_reproject_stack(src[:4], w.src_wcs[:4], w.tgt_wcs, w.shape_out, 1)
+    P.dfr_reproject_stack(src[4:], w.src_wcs[4:], w.tgt_wcs, w.shape_out, 1, sum=s, wsum=ws, accumulate=True)
+    assert torch.equal(ws, w_all) and torch.allclose(s, s_all, rtol=5e-7, atol=0)
+    st = check_stack(P, w, 1)
+    so, wo = oracle.stack(w.images, w.src_wcs, w.tgt_wcs, w.shape_out, 1)
+    assert (wo == 5.0).sum() > 100 and not np.isnan(so).any()
+    print("stack nan/accumulate", st)
+
+
+def test_stack_config2_full_size(P):
+    """configs[2] (32 x 2048^2 -> 2048^2) in the launch configuration bench.py --stack
+    times: wsum everywhere, sum on 60 000 sampled pixels computed one by one by the oracle."""
+    w = S.config2()
+    src = torch.from_numpy(w.images).cuda()
+    s, ws = P.dfr_reproject_stack(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1)
+    torch.cuda.synchronize()
+    st = P.dfr_last_stats()
+    s, ws = s.cpu().numpy(), ws.cpu().numpy()
+    sny, snx = w.images.shape[1:]
+    rng = np.random.default_rng(333)
+    ii = rng.integers(0, 2048, 60000).astype(np.float64)
+    jj = rng.integers(0, 2048, 60000).astype(np.float64)
+    ra, dec = oracle.pix2world(w.tgt_wcs, ii, jj)
+    so, wo, band = np.zeros(ii.size), np.zeros(ii.size), np.zeros(ii.size, dtype=bool)
+    for e in range(32):
+        xo, yo = oracle.world2pix(w.src_wcs[e], ra, dec)
+        v = oracle.interp(w.images[e], xo, yo, 1)
+        ok = ~np.isnan(v)
+        so += np.where(ok, v, 0.0)
+        wo += ok
+        band |= PR.edge_band(xo, yo, sny, snx)
+    gs, gw = s[jj.astype(int), ii.astype(int)], ws[jj.astype(int), ii.astype(int)]
+    assert np.array_equal(gw[~band], wo[~band].astype(np.float32))
+    dr = max(PR.dyn_range(im) for im in w.images)
+    err = np.abs(gs[~band] - so[~band])
+    assert err.max() <= PR.VALUE_TOL * dr * 32
+    assert ws.max() == 32.0 and 20.0 < ws.mean() < 32.0
+    print("C2 stack", st, "max err", err.max(), "limit", PR.VALUE_TOL * dr * 32, "mean depth", ws.mean())
+
+
+def test_stack_unaligned_pitch_and_exact_tiles(P):
+    """nx % 4 != 0 (no TMA staging) and a map that defeats the polynomial fit (EXACT tiles)."""
+    rng = np.random.default_rng(71)
+    imgs = np.stack([S.make_image(301, 403, 60, rng) for _ in range(3)])
+    srcs = [S.make_wcs(403, 301, 150.0 + 1e-3 * k, 2.0, 3.0 * k, S.PIXSCALE) for k in range(3)]
+    tgt = S.make_wcs(390, 310, 150.001, 2.0005, -2.0, S.PIXSCALE)
+    w = S.Workload("odd", imgs, srcs, tgt, (310, 390), (1,))
+    check_stack(P, w, 1)
+    assert P.dfr_last_stats()["tiles_fast"] > 0
+    imgs = np.stack([S.make_image(512, 512, 100, rng) for _ in range(2)])
+    srcs = [S.make_wcs(512, 512, 150.0, 2.0, 0.0, S.PIXSCALE), S.make_wcs(512, 512, 150.001, 2.0, 5.0, S.PIXSCALE)]
+    tgt = S.make_wcs(512, 512, 150.0005, 2.0003, 0.7, S.PIXSCALE)
+    tgt.a_order = tgt.b_order = 4
+    tgt.a[4][0] = 1e-8
+    w = S.Workload("quartic", imgs, srcs, tgt, (512, 512), (1,))
+    check_stack(P, w, 1)
+    assert P.dfr_last_stats()["tiles_exact"] > 0
