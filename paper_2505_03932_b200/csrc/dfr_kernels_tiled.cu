@@ -27,6 +27,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 
@@ -368,7 +369,7 @@ struct TiledParams {
     int n, e0, sny, snx, ony, onx;                 // e0: first exposure of this launch
     int tiles_x, tiles_y, ctas_x, ctas_y;
     int BW, BH;                                    // staged box (STAGE) in source pixels
-    int stage_bytes;                               // stack kernel: bytes per box stage
+    int stage_bytes, rec_off;                      // stack kernel: bytes per stage, offset of its records
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
@@ -930,35 +931,58 @@ constexpr int kStackCols = 2 * TS;                 // TMEM columns per CTA (powe
 struct StackParams {
     const float *weights;                          // DEVICE [n]
     float *sum, *wsum;                             // DEVICE [ony][onx]
-    int accumulate;                                // 0: overwrite, 1: add to the current contents
+    int add;                                       // 0: plain stores (one chunk, overwrite); 1: atomic adds
+    int nchunk;                                    // exposure chunks = gridDim.z
 };
 
+constexpr int kStackConsumers = CTA_T * CTA_T;                  // compute warps per CTA
+constexpr int kStackThreads = 32 * (kStackConsumers + 1);       // + one producer warp
+constexpr int kRecBytes = kStackConsumers * (int)sizeof(TileRec);
+
+// the producer's wait: back off between polls so the spin does not take issue slots
+__device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity)
+{
+    for (;;) {
+        uint32_t done;
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+        if (done) break;
+        __nanosleep(100);
+    }
+}
+
+// stage = [ box BW x BH floats | the CTA tile's 4 TileRec | head ]; STAGE = false: records only
 template <int ORDER, bool STAGE>
-__global__ void __launch_bounds__(32 * CTA_T * CTA_T)
+__global__ void __launch_bounds__(kStackThreads)
 tiled_stack_kernel(const __grid_constant__ TiledParams P, const __grid_constant__ TargetDev tgt,
                    const __grid_constant__ CUtensorMap tmap, const __grid_constant__ StackParams S)
 {
-    extern __shared__ __align__(128) unsigned char stages[];       // 2 boxes (STAGE)
-    __shared__ __align__(8) unsigned long long full[2];
+    extern __shared__ __align__(128) unsigned char stages[];
+    __shared__ __align__(8) unsigned long long full[2], empty[2];
     __shared__ int4 head[2];                                       // has_box, ox, oy
     __shared__ uint32_t tmem_base;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int ttx = blockIdx.x * CTA_T + (warp % CTA_T), tty = blockIdx.y * CTA_T + (warp / CTA_T);
-    const bool active = ttx < P.tiles_x && tty < P.tiles_y;
     const int ntile = P.tiles_x * P.tiles_y, ctas = P.ctas_x * P.ctas_y;
-    const int tile = active ? tty * P.tiles_x + ttx : 0;
     const int cta = blockIdx.y * P.ctas_x + blockIdx.x;
-    const uint32_t box_bytes = (uint32_t)(P.BW * P.BH * sizeof(float));
+    // this CTA's chunk of the exposure list (grid.z chunks balance the waves; partial sums
+    // of different chunks meet in global memory through atomic adds)
+    const int e_lo = (int)((long long)blockIdx.z * P.n / S.nchunk);
+    const int e_hi = (int)((long long)(blockIdx.z + 1) * P.n / S.nchunk);
 
     if (warp == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
                      ::"r"(smem_u32(&tmem_base)), "n"(kStackCols) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
-    if (STAGE && threadIdx.x == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&full[0])));
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&full[1])));
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < 2; ++s) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&full[s])));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(&empty[s])), "r"(kStackConsumers));
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
@@ -966,95 +990,104 @@ tiled_stack_kernel(const __grid_constant__ TiledParams P, const __grid_constant_
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 
-    StackSink sink;
-    sink.taddr = tmem_base + ((uint32_t)(warp * 32) << 16);
-    sink.w = 0.0f;
-    sink.r = 0;
-    for (int g = 0; g < kStackCols; g += 4)                        // zero sum and wsum
-        asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %1, %1, %1};"
-                     ::"r"(sink.taddr + (uint32_t)g), "f"(0.0f) : "memory");
-    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-
-    // thread 0: stage head + expect_tx + TMA box load of exposure e into stage s
-    auto issue = [&](int e, int s, int2 cb) {
-        const int hb = cb.x != kNoBox;
-        // TMA wants a 16-byte aligned start along x (measured on B200): round down to 4 floats
-        const int ox = (cb.x - (Taps<ORDER>::lo + 1)) & ~3, oy = cb.y - (Taps<ORDER>::lo + 1);
-        head[s] = make_int4(hb, ox, oy, 0);
-        const uint32_t bar = smem_u32(&full[s]);
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(hb ? box_bytes : 0u) : "memory");
-        if (hb)
-            asm volatile(
-                "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-                ::"r"(smem_u32(stages + (size_t)s * P.stage_bytes)), "l"(&tmap), "r"(ox), "r"(oy), "r"(e), "r"(bar) : "memory");
-    };
-    if (STAGE && threadIdx.x == 0) {
-        issue(0, 0, __ldg(P.cta_box + cta));
-        if (P.n > 1) issue(1, 1, __ldg(P.cta_box + (size_t)ctas + cta));
-    }
-
-    for (int e = 0; e < P.n; ++e) {
-        const int s = e & 1;
-        int2 cb2 = make_int2(kNoBox, kNoBox);
-        if (STAGE && threadIdx.x == 0 && e + 2 < P.n) cb2 = __ldg(P.cta_box + (size_t)(e + 2) * ctas + cta);
-        // this exposure's record (requested before the box is waited for)
-        const TileRec *rec = P.recs + ((size_t)e * ntile + tile);
-        const int4 h0 = __ldg(reinterpret_cast<const int4 *>(&rec->ix0));       // ix0 iy0 bx0 by0
-        const int4 h1 = __ldg(reinterpret_cast<const int4 *>(&rec->bx1));       // bx1 by1 flag deg
-        TileHead H;
-        H.ix0 = h0.x; H.iy0 = h0.y; H.bx0 = h0.z; H.by0 = h0.w; H.bx1 = h1.x; H.by1 = h1.y; H.flag = h1.z; H.deg = h1.w;
-        float X[4], Y[4];
-        {
-            const float di = (float)lane - (float)kCentre;
-            const float4 *c4 = reinterpret_cast<const float4 *>(rec->cx);
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const float4 a = __ldg(c4 + q), b = __ldg(c4 + 4 + q);
-                X[q] = fmaf(fmaf(fmaf(a.w, di, a.z), di, a.y), di, a.x);
-                Y[q] = fmaf(fmaf(fmaf(b.w, di, b.z), di, b.y), di, b.x);
+    if (warp == kStackConsumers) {
+        // ------------------------------ producer (one lane) ------------------------------
+        if (lane == 0) {
+            const uint32_t box_bytes = (uint32_t)(P.BW * P.BH * sizeof(float));
+            // the CTA tile's records: up to two runs (tile rows) of up to two records
+            const int tx0 = blockIdx.x * CTA_T, ty0 = blockIdx.y * CTA_T;
+            const uint32_t run = (uint32_t)min(CTA_T, P.tiles_x - tx0) * (uint32_t)sizeof(TileRec);
+            const int nrun = min(CTA_T, P.tiles_y - ty0);
+            for (int e = e_lo; e < e_hi; ++e) {
+                const int k = e - e_lo, s = k & 1;
+                int2 cb = make_int2(kNoBox, kNoBox);
+                if (STAGE) cb = __ldg(P.cta_box + (size_t)e * ctas + cta);
+                if (k >= 2) mbar_wait_sleep(smem_u32(&empty[s]), ((uint32_t)(k >> 1) & 1u) ^ 1u);
+                const int hb = STAGE && cb.x != kNoBox;
+                // TMA wants a 16-byte aligned start along x (measured on B200): round down to 4 floats
+                const int ox = (cb.x - (Taps<ORDER>::lo + 1)) & ~3, oy = cb.y - (Taps<ORDER>::lo + 1);
+                head[s] = make_int4(hb, ox, oy, 0);
+                unsigned char *st = stages + (size_t)s * P.stage_bytes;
+                const uint32_t bar = smem_u32(&full[s]);
+                const uint32_t bytes = (hb ? box_bytes : 0u) + run * (uint32_t)nrun;
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+                for (int q = 0; q < nrun; ++q)
+                    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                                 ::"r"(smem_u32(st + P.rec_off + q * CTA_T * (int)sizeof(TileRec))),
+                                   "l"(P.recs + ((size_t)e * ntile + (size_t)(ty0 + q) * P.tiles_x + tx0)), "r"(run), "r"(bar)
+                                 : "memory");
+                if (hb)
+                    asm volatile(
+                        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                        ::"r"(smem_u32(st)), "l"(&tmap), "r"(ox), "r"(oy), "r"(e), "r"(bar) : "memory");
             }
         }
-        sink.w = __ldg(S.weights + e);
+    } else {
+        // ------------------------------ consumers ------------------------------
+        const int ttx = blockIdx.x * CTA_T + (warp % CTA_T), tty = blockIdx.y * CTA_T + (warp / CTA_T);
+        const bool active = ttx < P.tiles_x && tty < P.tiles_y;
+        StackSink sink;
+        sink.taddr = tmem_base + ((uint32_t)(warp * 32) << 16);
+        sink.w = 0.0f;
         sink.r = 0;
-        int ox = 0, oy = 0;
-        if (STAGE) {
-            mbar_wait(smem_u32(&full[s]), (uint32_t)(e >> 1) & 1u);
-            const int4 hd = head[s];
-            ox = hd.y; oy = hd.z;
-        }
-        if (active)
-            warp_tile<ORDER, STAGE>(P, tgt, e, ttx, tty, lane, H, X, Y,
-                                    smem_u32(stages + (size_t)s * P.stage_bytes), ox, oy, sink);
+        for (int g = 0; g < kStackCols; g += 4)                    // zero sum and wsum
+            asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %1, %1, %1};"
+                         ::"r"(sink.taddr + (uint32_t)g), "f"(0.0f) : "memory");
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-        if (STAGE) {
-            __syncthreads();                            // every warp is done with stage s
-            if (threadIdx.x == 0 && e + 2 < P.n) issue(e + 2, s, cb2);
-        }
-    }
 
-    // ---- epilogue: accumulators -> sum, wsum (one coalesced 128-byte row per warp and row)
-    if (active) {
-        const int col = ttx * TS + lane, ty0 = tty * TS;
-        const int rows = min(TS, P.ony - ty0);
-        for (int r = 0; r < TS; r += 4) {
-            float a[4], c[4];
-            asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
-                         : "=f"(a[0]), "=f"(a[1]), "=f"(a[2]), "=f"(a[3]) : "r"(sink.taddr + (uint32_t)r));
-            asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
-                         : "=f"(c[0]), "=f"(c[1]), "=f"(c[2]), "=f"(c[3]) : "r"(sink.taddr + (uint32_t)(TS + r)));
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        for (int e = e_lo; e < e_hi; ++e) {
+            const int k = e - e_lo, s = k & 1;
+            sink.w = __ldg(S.weights + e);
+            sink.r = 0;
+            mbar_wait(smem_u32(&full[s]), (uint32_t)(k >> 1) & 1u);
+            if (active) {
+                const unsigned char *st = stages + (size_t)s * P.stage_bytes;
+                const TileRec *rec = reinterpret_cast<const TileRec *>(st + P.rec_off) + warp;
+                const int4 h0 = *reinterpret_cast<const int4 *>(&rec->ix0);    // ix0 iy0 bx0 by0
+                const int4 h1 = *reinterpret_cast<const int4 *>(&rec->bx1);    // bx1 by1 flag deg
+                TileHead H;
+                H.ix0 = h0.x; H.iy0 = h0.y; H.bx0 = h0.z; H.by0 = h0.w; H.bx1 = h1.x; H.by1 = h1.y; H.flag = h1.z; H.deg = h1.w;
+                float X[4], Y[4];
+                const float di = (float)lane - (float)kCentre;
+                const float4 *c4 = reinterpret_cast<const float4 *>(rec->cx);
 #pragma unroll
-            for (int k = 0; k < 4; ++k)
-                if (r + k < rows && col < P.onx) {
-                    const size_t o = (size_t)(ty0 + r + k) * P.onx + col;
-                    if (S.accumulate) {
-                        S.sum[o] += a[k];
-                        S.wsum[o] += c[k];
-                    } else {
-                        S.sum[o] = a[k];
-                        S.wsum[o] = c[k];
-                    }
+                for (int q = 0; q < 4; ++q) {
+                    const float4 a = c4[q], b = c4[4 + q];
+                    X[q] = fmaf(fmaf(fmaf(a.w, di, a.z), di, a.y), di, a.x);
+                    Y[q] = fmaf(fmaf(fmaf(b.w, di, b.z), di, b.y), di, b.x);
                 }
+                const int4 hd = head[s];
+                warp_tile<ORDER, STAGE>(P, tgt, e, ttx, tty, lane, H, X, Y, smem_u32(st), hd.y, hd.z, sink);
+            }
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            __syncwarp();                                   // every lane is done with stage s
+            if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&empty[s])) : "memory");
+        }
+
+        // ---- epilogue: accumulators -> sum, wsum (one coalesced 128-byte row per warp and row)
+        if (active) {
+            const int col = ttx * TS + lane, ty0 = tty * TS;
+            const int rows = min(TS, P.ony - ty0);
+            for (int r = 0; r < TS; r += 4) {
+                float a[4], c[4];
+                asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                             : "=f"(a[0]), "=f"(a[1]), "=f"(a[2]), "=f"(a[3]) : "r"(sink.taddr + (uint32_t)r));
+                asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                             : "=f"(c[0]), "=f"(c[1]), "=f"(c[2]), "=f"(c[3]) : "r"(sink.taddr + (uint32_t)(TS + r)));
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (r + k < rows && col < P.onx) {
+                        const size_t o = (size_t)(ty0 + r + k) * P.onx + col;
+                        if (S.add) {
+                            atomicAdd(S.sum + o, a[k]);
+                            atomicAdd(S.wsum + o, c[k]);
+                        } else {
+                            S.sum[o] = a[k];
+                            S.wsum[o] = c[k];
+                        }
+                    }
+            }
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -1318,16 +1351,49 @@ static cudaError_t launch_stack(TiledParams P, const TargetDev &tgt, const CUten
                                 const StackParams &S, cudaStream_t st)
 {
     auto kern = tiled_stack_kernel<ORDER, STAGE>;
-    P.stage_bytes = (int)((box_bytes + 127) & ~(size_t)127);
-    const size_t smem = STAGE ? 2 * (size_t)P.stage_bytes : 0;
-    if (STAGE) {
+    P.rec_off = (int)((box_bytes + 127) & ~(size_t)127);
+    P.stage_bytes = (int)((P.rec_off + kRecBytes + 127) & ~(size_t)127);
+    const size_t smem = 2 * (size_t)P.stage_bytes;
+    {
         cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (err != cudaSuccess) return err;
     }
     if (P.ctas_y > 65535) return cudaErrorInvalidConfiguration;
     P.e0 = 0;
-    const dim3 grid((unsigned)P.ctas_x, (unsigned)P.ctas_y, 1);
-    kern<<<grid, 32 * CTA_T * CTA_T, smem, st>>>(P, tgt, tmap, S);
+    // Exposure chunks: every CTA runs for (exposures in its chunk) x (one tile's time), so the
+    // grid is cut along the exposure list until its waves fill the machine evenly.
+    int dev = 0, sms = 0, per_sm = 0;
+    cudaError_t err = cudaGetDevice(&dev);
+    if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    // resident CTAs per SM from the kernel's own resources (the occupancy API returned 1 for
+    // this kernel on B200 / CUDA 12.9): shared memory, registers, TMEM columns
+    cudaFuncAttributes fa;
+    int smem_sm = 0, regs_sm = 0;
+    if (err == cudaSuccess) err = cudaFuncGetAttributes(&fa, kern);
+    if (err == cudaSuccess) err = cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
+    if (err == cudaSuccess) err = cudaDeviceGetAttribute(&regs_sm, cudaDevAttrMaxRegistersPerMultiprocessor, dev);
+    if (err != cudaSuccess) return err;
+    const int threads = kStackThreads;
+    per_sm = std::min(512 / kStackCols, 32);
+    per_sm = std::min<long long>(per_sm, smem_sm / (long long)(smem + fa.sharedSizeBytes + 1024));
+    per_sm = std::min(per_sm, regs_sm / std::max(1, ((fa.numRegs + 7) & ~7) * threads));
+    const double slots = (double)sms * std::max(per_sm, 1), tiles = (double)P.ctas_x * P.ctas_y;
+    int best = 1;
+    double best_eff = 0.0;
+    for (int z = 1; z <= std::min(P.n, 8); ++z) {
+        const double waves = tiles * z / slots, eff = waves / std::ceil(waves);
+        if (eff > best_eff + 0.02) { best_eff = eff; best = z; }
+    }
+    StackParams S2 = S;
+    S2.nchunk = best;
+    if (best > 1 && !S.add) {                       // partial sums meet by atomic adds: start from zero
+        const size_t bytes = sizeof(float) * (size_t)P.ony * P.onx;
+        if ((err = cudaMemsetAsync(S.sum, 0, bytes, st)) != cudaSuccess) return err;
+        if ((err = cudaMemsetAsync(S.wsum, 0, bytes, st)) != cudaSuccess) return err;
+        S2.add = 1;
+    }
+    const dim3 grid((unsigned)P.ctas_x, (unsigned)P.ctas_y, (unsigned)best);
+    kern<<<grid, kStackThreads, smem, st>>>(P, tgt, tmap, S2);
     return cudaGetLastError();
 }
 
@@ -1341,7 +1407,7 @@ cudaError_t launch_tiled_stack(const float *src, int n, int sny, int snx, const 
     cudaError_t err = prepare_tiled(src, n, sny, snx, tgt, srcdev, srchost, ony, onx, order, st, dev_counters, R);
     if (err != cudaSuccess) { free_scratch(R.sc, st); return err; }
     StackParams S;
-    S.weights = dev_weights; S.sum = sum; S.wsum = wsum; S.accumulate = accumulate;
+    S.weights = dev_weights; S.sum = sum; S.wsum = wsum; S.add = accumulate; S.nchunk = 1;
     if (prof && prof->enabled) cudaEventRecord(prof->main_begin, st);
 #define DFR_LAUNCH(O)                                                                     \
     err = R.stage ? launch_stack<O, true>(R.P, tgt, R.tmap, R.box_bytes, S, st) : launch_stack<O, false>(R.P, tgt, R.tmap, 0, S, st)
