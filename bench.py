@@ -144,6 +144,70 @@ def run_reference(args):
     return 0
 
 
+def run_stack(args):
+    """--mode stack: dfr_reproject_stack on configs[2] (32 exposures -> one sum + one weight
+    frame). Same timing discipline as the headline; one JSON line with its own metric."""
+    import torch
+    import paper_2505_03932_b200 as P
+    P.lib()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    w = S.config2(batch=BATCH)
+    src = torch.from_numpy(w.images).cuda()
+    ws_arr, tw = P.pack_wcs_array(w.src_wcs), P.pack_wcs(w.tgt_wcs)
+    ssum = torch.empty((NPIX, NPIX), dtype=torch.float32, device="cuda")
+    wsum = torch.empty_like(ssum)
+
+    def step():
+        P.dfr_reproject_stack(src, ws_arr, tw, (NPIX, NPIX), P.BILINEAR, sum=ssum, wsum=wsum)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    time.sleep(0.3)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    torch.cuda.synchronize()
+    ev[0].record()
+    for k in range(args.steps):
+        step()
+        ev[k + 1].record()
+    torch.cuda.synchronize()
+    total_ms = ev[0].elapsed_time(ev[-1])
+    per_step = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
+    time.sleep(0.2)
+    sampler.stop()
+    P.dfr_profile_enable(True)
+    ms = []
+    for _ in range(min(args.steps, 10)):
+        step()
+        ms.append(P.dfr_profile_last())
+    P.dfr_profile_enable(False)
+    main_ms = statistics.mean(m[1] for m in ms)
+    stats = P.dfr_last_stats()
+    in_mpix = BATCH * NPIX * NPIX / 1e6
+    hbm, which, _ = peaks()
+    alg = 4.0 * BATCH * NPIX * NPIX + 8.0 * NPIX * NPIX       # sources read once + sum and wsum written
+    achieved = alg / (main_ms * 1e-3) / 1e9
+    line = {"metric": "input exposure Mpix/s reprojected and stacked (32 x 2048^2 TAN-SIP3 bilinear -> one 2048^2 sum + weight)",
+            "value": in_mpix * args.steps / (total_ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "configs[2] through dfr_reproject_stack", "depth_mean": float(wsum.mean().item()),
+                       "l2": "inputs per step are 537 MB > 126 MB L2 (no flush needed)", "tiles": stats},
+            "ms_per_step_median": statistics.median(per_step),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm,
+                         "traffic": None, "peak_source": which, "kernel": "tiled_stack_kernel", "kernel_ms": main_ms,
+                         "setup_kernels_ms": statistics.mean(m[0] for m in ms), "algorithmic_bytes_per_launch": alg,
+                         "note": "issue-bound, not HBM-bound: see DESIGN.md §6.5"},
+            "cpu_baseline": None, "e2e": None, "gpu_launches": int(stats["kernels"]) * args.steps,
+            "clocks": sampler.summary()}
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -153,7 +217,12 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--path", default="auto", choices=["auto", "exact"])
+    ap.add_argument("--mode", default="reproject", choices=["reproject", "stack"],
+                    help="stack: the fused reproject-and-stack entry point (SURVEY.md §8(f) f1) on the same "
+                         "workload; not the headline metric")
     args = ap.parse_args()
+    if args.mode == "stack" and args.impl == "ours":
+        return run_stack(args)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)

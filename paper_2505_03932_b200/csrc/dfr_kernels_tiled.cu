@@ -939,18 +939,18 @@ constexpr int kStackConsumers = CTA_T * CTA_T;                  // compute warps
 constexpr int kStackThreads = 32 * (kStackConsumers + 1);       // + one producer warp
 constexpr int kRecBytes = kStackConsumers * (int)sizeof(TileRec);
 
-// the producer's wait: back off between polls so the spin does not take issue slots
+// the producer's wait: let the hardware suspend the thread (time hint) instead of spinning,
+// so the wait takes no issue slots from the compute warps
 __device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity)
 {
     for (;;) {
         uint32_t done;
         asm volatile(
             "{\n\t.reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
             "selp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+            : "=r"(done) : "r"(bar), "r"(parity), "r"(20000u) : "memory");
         if (done) break;
-        __nanosleep(100);
     }
 }
 
