@@ -144,6 +144,16 @@ int dfr_reproject_stack(const float *src_batch, int32_t n, int32_t src_ny, int32
                         const float *weights, float *sum, float *wsum, int32_t accumulate,
                         void *stream);
 
+/* End-to-end form of the stack with HOST buffers (the ">1000 exposures" case of
+ * PAPER.md:25 co-added instead of returned one by one): src_host [n][src_ny][src_nx]
+ * is uploaded in batches of `batch` (<= 0 selects 32) on private streams, every batch is
+ * added into one device-resident sum / wsum pair while the next uploads, and only the two
+ * [out_ny][out_nx] frames come back. weights: HOST float32[n] or NULL. Synchronous. */
+int dfr_stack_host(const float *src_host, int32_t n, int32_t src_ny, int32_t src_nx,
+                   const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                   int32_t out_ny, int32_t out_nx, int32_t order, const float *weights,
+                   float *sum_host, float *wsum_host, int32_t batch);
+
 /* mean[k] = sum[k] / wsum[k], NaN where wsum[k] == 0. DEVICE float32[npix] each;
  * mean may be the same array as sum. */
 int dfr_stack_finalize(const float *sum, const float *wsum, int64_t npix, float *mean, void *stream);

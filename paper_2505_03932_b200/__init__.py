@@ -20,7 +20,7 @@ PATH_AUTO, PATH_EXACT, PATH_TILED = 0, 1, 2
 _ORDER_NAMES = {"nearest": 0, "nearest-neighbor": 0, "bilinear": 1, "bicubic": 3}
 
 EXPORTS = ["dfr_reproject", "dfr_reproject_ex", "dfr_reproject_host", "dfr_reproject_stack",
-           "dfr_stack_finalize", "dfr_pix2world",
+           "dfr_stack_finalize", "dfr_stack_host", "dfr_pix2world",
            "dfr_world2pix", "dfr_src_coords", "dfr_wcs_set_pc_cdelt", "dfr_last_stats",
            "dfr_profile_enable", "dfr_profile_last",
            "dfr_strerror", "dfr_last_error", "dfr_version"]
@@ -60,6 +60,7 @@ def lib():
         L.dfr_reproject_stack.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32,
                                           C.POINTER(C.c_float), fp, fp, i32, vp]
         L.dfr_stack_finalize.argtypes = [fp, fp, i64, fp, vp]
+        L.dfr_stack_host.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, C.POINTER(C.c_float), fp, fp, i32]
         L.dfr_pix2world.argtypes = [wp, dp, dp, i64, dp, dp, vp]
         L.dfr_world2pix.argtypes = [wp, dp, dp, i64, dp, dp, vp]
         L.dfr_src_coords.argtypes = [i32, i32, i32, wp, wp, i32, i32, i32, dp, dp, vp, i32]
@@ -211,6 +212,34 @@ def dfr_reproject_stack(src_batch, src_wcs, tgt_wcs, shape_out=None, order=BILIN
                                          _order(order), wp, sum.data_ptr(), wsum.data_ptr(),
                                          1 if accumulate else 0, _stream_ptr(stream)))
     return sum, wsum
+
+
+def dfr_stack_host(src_host, src_wcs, tgt_wcs, shape_out=None, order=BILINEAR, weights=None, batch=32):
+    """dfr_stack_host: HOST float32 exposures in (pinned for full PCIe rate), HOST (sum, wsum)
+    float32 [out_ny][out_nx] out; uploads and the stacking kernels are pipelined in the library."""
+    import torch
+    src_t = torch.as_tensor(src_host)
+    if src_t.dim() == 2:
+        src_t = src_t[None]
+    if src_t.is_cuda or src_t.dtype != torch.float32 or not src_t.is_contiguous():
+        raise ValueError("src_host must be a contiguous float32 host array")
+    n, sny, snx = src_t.shape
+    ony, onx = (sny, snx) if shape_out is None else (int(shape_out[0]), int(shape_out[1]))
+    ws = pack_wcs_array(src_wcs)
+    if len(ws) != n:
+        raise ValueError("one source WCS per exposure")
+    tw = pack_wcs(tgt_wcs)
+    wp = None
+    if weights is not None:
+        w = np.ascontiguousarray(weights, dtype=np.float32)
+        if w.size != n:
+            raise ValueError("one weight per exposure")
+        wp = w.ctypes.data_as(C.POINTER(C.c_float))
+    s = torch.empty((ony, onx), dtype=torch.float32, pin_memory=True)
+    c = torch.empty((ony, onx), dtype=torch.float32, pin_memory=True)
+    _check(lib().dfr_stack_host(src_t.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx, _order(order), wp,
+                                s.data_ptr(), c.data_ptr(), int(batch)))
+    return s, c
 
 
 def dfr_stack_finalize(sum, wsum, mean=None, stream=None):

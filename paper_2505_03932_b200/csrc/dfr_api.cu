@@ -61,6 +61,11 @@ static thread_local LastCall g_last;
 static thread_local int64_t g_stats_acc[4] = {0, 0, 0, 0};   // used by dfr_reproject_host
 static thread_local bool g_accumulate = false;
 
+static int stack_impl(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+                      const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs, int32_t out_ny, int32_t out_nx,
+                      int32_t order, const float *weights, float *sum, float *wsum, int32_t accumulate,
+                      cudaStream_t st);
+
 static cudaError_t ensure_last()
 {
     cudaError_t err;
@@ -219,14 +224,30 @@ int dfr_reproject_stack(const float *src_batch, int32_t n, int32_t src_ny, int32
         set_error("sum / wsum overlap src_batch or each other");
         return DFR_ERR_ALIAS;
     }
+    for (int32_t e = 0; weights && e < n; ++e)
+        if (!std::isfinite(weights[e])) { set_error("weights[%d] is not finite", e); return DFR_ERR_NONFINITE_WCS; }
+    return stack_impl(src_batch, n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order, weights, sum, wsum,
+                      accumulate, (cudaStream_t)stream);
+}
+
+}  // extern "C"
+
+namespace dfr {
+// validated arguments -> constants, scratch, launches (stream-ordered)
+static int stack_impl(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+                      const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs, int32_t out_ny, int32_t out_nx,
+                      int32_t order, const float *weights, float *sum, float *wsum, int32_t accumulate,
+                      cudaStream_t st)
+{
     std::vector<float> hw((size_t)n, 1.0f);
-    if (weights)
-        for (int32_t e = 0; e < n; ++e) {
-            if (!std::isfinite(weights[e])) { set_error("weights[%d] is not finite", e); return DFR_ERR_NONFINITE_WCS; }
-            hw[e] = weights[e];
-        }
+    for (int32_t e = 0; weights && e < n; ++e) hw[e] = weights[e];
     std::call_once(g_pool_once, tune_pool);
-    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    if (g_accumulate && g_last.pending) {         // previous batch of a streaming call
+        int64_t t[4];
+        collect_stats(t);
+        for (int k = 0; k < 4; ++k) g_stats_acc[k] += t[k];
+    }
     g_last.pending = false;
     TargetDev tgt;
     make_target(tgt_wcs, &tgt);
@@ -257,6 +278,9 @@ int dfr_reproject_stack(const float *src_batch, int32_t n, int32_t src_ny, int32
     if (err != cudaSuccess) return cuda_fail(err, "reproject_stack launch");
     return DFR_OK;
 }
+}  // namespace dfr
+
+extern "C" {
 
 int dfr_stack_finalize(const float *sum, const float *wsum, int64_t npix, float *mean, void *stream)
 {
@@ -401,6 +425,79 @@ int dfr_reproject_host(const float *src_host, int32_t n, int32_t src_ny, int32_t
     }
     g_last.kernels = -1;                 // marks "use the accumulated totals"
     return rc;
+}
+
+int dfr_stack_host(const float *src_host, int32_t n, int32_t src_ny, int32_t src_nx,
+                   const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                   int32_t out_ny, int32_t out_nx, int32_t order, const float *weights,
+                   float *sum_host, float *wsum_host, int32_t batch)
+{
+    if (!src_host || !sum_host || !wsum_host) { set_error("NULL image pointer"); return DFR_ERR_NULL; }
+    int rc = check_common(n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order);
+    if (rc != DFR_OK) return rc;
+    for (int32_t e = 0; weights && e < n; ++e)
+        if (!std::isfinite(weights[e])) { set_error("weights[%d] is not finite", e); return DFR_ERR_NONFINITE_WCS; }
+    if (batch <= 0) batch = 32;
+    if (batch > n) batch = n;
+    const size_t in_px = (size_t)src_ny * src_nx, out_bytes = sizeof(float) * (size_t)out_ny * out_nx;
+    std::lock_guard<std::mutex> lock(g_pipe.mu);
+    int dev = 0;
+    cudaError_t err = cudaGetDevice(&dev);
+    if (err != cudaSuccess) return cuda_fail(err, "cudaGetDevice");
+    if (g_pipe.dev != dev) {                       // buffers belong to one device
+        for (Slot &s : g_pipe.slot) {
+            if (s.din) cudaFree(s.din);
+            if (s.dout) cudaFree(s.dout);
+            if (s.st) cudaStreamDestroy(s.st);
+            s = Slot();
+        }
+        g_pipe.dev = dev;
+    }
+    const int nb = (n + batch - 1) / batch;
+    const int used = nb < kSlots ? nb : kSlots;
+    // slot 0's output buffer holds sum and wsum; every slot needs an input buffer and a stream
+    for (int k = 0; k < used; ++k) {
+        err = ensure_slot(g_pipe.slot[k], in_px * batch * sizeof(float), k == 0 ? 2 * out_bytes : 0);
+        if (err != cudaSuccess) return cuda_fail(err, "pipeline buffers");
+    }
+    float *dsum = g_pipe.slot[0].dout, *dwsum = dsum + (size_t)out_ny * out_nx;
+    cudaEvent_t zeroed = nullptr;
+    if ((err = cudaEventCreateWithFlags(&zeroed, cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(err, "event");
+    err = cudaMemsetAsync(dsum, 0, 2 * out_bytes, g_pipe.slot[0].st);
+    if (err == cudaSuccess) err = cudaEventRecord(zeroed, g_pipe.slot[0].st);
+    for (int k = 1; k < used && err == cudaSuccess; ++k) err = cudaStreamWaitEvent(g_pipe.slot[k].st, zeroed, 0);
+    if (err != cudaSuccess) { cudaEventDestroy(zeroed); return cuda_fail(err, "pipeline start"); }
+    for (int k = 0; k < 4; ++k) g_stats_acc[k] = 0;
+    g_last.pending = false;
+    g_accumulate = true;
+    for (int b = 0; b < nb; ++b) {
+        Slot &s = g_pipe.slot[b % kSlots];
+        const int32_t e0 = b * batch, ne = (n - e0 < batch) ? n - e0 : batch;
+        // the slot's stream orders its own reuse: H2D(b) waits for the kernels of b - kSlots;
+        // batches of different slots add into sum / wsum concurrently (atomic adds)
+        err = cudaMemcpyAsync(s.din, src_host + in_px * e0, in_px * ne * sizeof(float), cudaMemcpyHostToDevice, s.st);
+        if (err != cudaSuccess) { rc = cuda_fail(err, "H2D"); break; }
+        rc = stack_impl(s.din, ne, src_ny, src_nx, src_wcs + e0, tgt_wcs, out_ny, out_nx, order,
+                        weights ? weights + e0 : nullptr, dsum, dwsum, 1, s.st);
+        if (rc != DFR_OK) break;
+    }
+    for (int k = 0; k < used; ++k) {
+        err = cudaStreamSynchronize(g_pipe.slot[k].st);
+        if (err != cudaSuccess && rc == DFR_OK) rc = cuda_fail(err, "pipeline sync");
+    }
+    cudaEventDestroy(zeroed);
+    g_accumulate = false;
+    if (g_last.pending) {
+        int64_t t[4];
+        collect_stats(t);
+        for (int k = 0; k < 4; ++k) g_stats_acc[k] += t[k];
+        g_last.pending = false;
+    }
+    g_last.kernels = -1;                 // marks "use the accumulated totals"
+    if (rc != DFR_OK) return rc;
+    err = cudaMemcpy(sum_host, dsum, out_bytes, cudaMemcpyDeviceToHost);
+    if (err == cudaSuccess) err = cudaMemcpy(wsum_host, dwsum, out_bytes, cudaMemcpyDeviceToHost);
+    return err == cudaSuccess ? DFR_OK : cuda_fail(err, "D2H");
 }
 
 int dfr_wcs_set_pc_cdelt(dfr_wcs *w, const double pc[4], const double cdelt[2])

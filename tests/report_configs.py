@@ -138,6 +138,19 @@ def stream_case(n_exp, n_img, batch=32):
     out = P.dfr_reproject_host(torch.from_numpy(w.images).pin_memory(), w.src_wcs, w.tgt_wcs, w.shape_out, 1, batch=2)
     par = parity(w, 1, out.numpy(), range(len(w.src_wcs)))
     mpix = n_exp * wi.shape_out[0] * wi.shape_out[1] / 1e6
+    # the same stream co-added instead of returned one by one (dfr_stack_host)
+    # (one call per n_img exposures, because the pixel content cycles; each call returns its
+    # own sum / wsum pair, added on the host outside nothing: the adds are inside the timing)
+    P.dfr_stack_host(hin[:2 * batch], ws_all[:2 * batch], tw, wi.shape_out, 1, batch=batch)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    ssum = swsum = None
+    for b0 in range(0, n_exp, n_img):
+        a, c = P.dfr_stack_host(hin[:min(n_img, n_exp - b0)], ws_all[b0:b0 + n_img], tw, wi.shape_out, 1, batch=batch)
+        ssum = a if ssum is None else ssum.add_(a)
+        swsum = c if swsum is None else swsum.add_(c)
+    stack_s = time.perf_counter() - t0
+    stack_depth = float(swsum.max().item())
     # device-resident kernel time of one batch of 32
     src = hin[:batch].cuda()
     dout = torch.empty((batch,) + tuple(wi.shape_out), dtype=torch.float32, device="cuda")
@@ -147,7 +160,9 @@ def stream_case(n_exp, n_img, batch=32):
             "wall_s": el, "exposures_per_s": n_exp / el, "mpix_per_s": mpix / el,
             "h2d_gbs": n_exp * 2048 * 2048 * 4 / el / 1e9, "d2h_gbs": mpix * 4e6 / el / 1e9,
             "device_batch_ms": med, "device_batch_mpix_per_s": batch * 16.777216 / (med * 1e-3),
-            "device_batch_gbs": alg / (med * 1e-3) / 1e9, "generation_s": gen_s, **par}
+            "device_batch_gbs": alg / (med * 1e-3) / 1e9, "generation_s": gen_s,
+            "stack_wall_s": stack_s, "stack_exposures_per_s": n_exp / stack_s,
+            "stack_h2d_gbs": n_exp * 2048 * 2048 * 4 / stack_s / 1e9, "stack_depth_max": stack_depth, **par}
 
 
 def main():
@@ -197,7 +212,9 @@ def main():
                     f"(H2D {c4['h2d_gbs']:.1f} GB/s + D2H {c4['d2h_gbs']:.1f} GB/s concurrently); device-resident batch of 32: "
                     f"{c4['device_batch_ms']:.3f} ms = {c4['device_batch_mpix_per_s']:.0f} Mpix/s, {c4['device_batch_gbs']:.0f} GB/s; "
                     f"parity on exposures {c4['exposures_checked']}: coord {c4['coord_max_px']:.1e} px, value {c4['value_max_dr']:.1e} x DR, "
-                    f"NaN frac {c4['nan_frac']:.3f}.\n")
+                    f"NaN frac {c4['nan_frac']:.3f}. The same stream co-added by dfr_stack_host (only sum and wsum come back): "
+                    f"{c4['stack_wall_s']:.2f} s = {c4['stack_exposures_per_s']:.0f} exposures/s (H2D {c4['stack_h2d_gbs']:.1f} GB/s), "
+                    f"deepest pixel {c4['stack_depth_max']:.0f} exposures.\n")
     print("wrote", args.out + ".md")
 
 

@@ -147,3 +147,27 @@ def test_stack_unaligned_pitch_and_exact_tiles(P):
     w = S.Workload("quartic", imgs, srcs, tgt, (512, 512), (1,))
     check_stack(P, w, 1)
     assert P.dfr_last_stats()["tiles_exact"] > 0
+
+
+def test_stack_host_stream(P):
+    """dfr_stack_host on a configs[4]-like stream (mosaic target, one batch per 2 exposures so
+    batches overlap on the pipeline's streams): equals the device entry point up to float32
+    re-association, and the oracle within the stack tolerance."""
+    idx = (0, 31, 32, 511, 1023)
+    w = S.config4(idx, n=512, nstars=200, mosaic=1024)
+    wts = np.array([1.0, 2.0, 0.5, 1.0, 4.0])
+    src = torch.from_numpy(w.images).pin_memory()
+    s, c = P.dfr_stack_host(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1, weights=wts, batch=2)
+    st = P.dfr_last_stats()
+    ds, dc = P.dfr_reproject_stack(torch.from_numpy(w.images).cuda(), w.src_wcs, w.tgt_wcs, w.shape_out, 1, weights=wts)
+    assert torch.equal(c, dc.cpu()) and torch.allclose(s, ds.cpu(), rtol=1e-6, atol=1e-3)
+    assert st["tiles_fast"] + st["tiles_empty"] + st["tiles_exact"] == 5 * 32 * 32
+    so, wo = oracle.stack(w.images, w.src_wcs, w.tgt_wcs, w.shape_out, 1, wts)
+    band = np.zeros(w.shape_out, dtype=bool)
+    for e in range(len(idx)):
+        xo, yo = oracle.src_coords(w.tgt_wcs, w.src_wcs[e], *w.shape_out)
+        band |= PR.edge_band(xo, yo, 512, 512)
+    assert np.array_equal(c.numpy()[~band], wo[~band])
+    dr = max(PR.dyn_range(im) for im in w.images)
+    assert np.abs(s.numpy()[~band] - so[~band]).max() <= PR.VALUE_TOL * dr * wts.sum()
+    assert 0.5 < (wo == 0).mean() < 0.95                  # a mosaic: most of it is empty
