@@ -185,6 +185,17 @@ int dfr_src_coords(int32_t n, int32_t src_ny, int32_t src_nx,
 /* CD_ij = CDELT_i * PC_ij (FITS Paper I). HOST only. */
 int dfr_wcs_set_pc_cdelt(dfr_wcs *w, const double pc[4], const double cdelt[2]);
 
+/* Inverse SIP polynomials for a WCS that lacks them (PAPER.md:51 assumes SIP_INV_A /
+ * SIP_INV_B exist). HOST only. Fits AP, BP of the given order
+ * (1..9, full triangle 0 <= p+q <= order) by least squares so that
+ *   u ~= U + AP(U, V),  v ~= V + BP(U, V)   with (U, V) = (u + A(u,v), v + B(u,v))
+ * on a 64 x 64 uniform grid of pixel centres over [0, nx-1] x [0, ny-1] (Householder QR,
+ * columns scaled to [-1, 1]). Overwrites w->ap, w->bp (entries outside the triangle are
+ * zeroed) and sets w->ap_order = w->bp_order = order. *max_resid_px (optional) receives
+ * the largest |u - (U + AP)|, |v - (V + BP)| over the grid: raise the order if it is too
+ * large for the application. The forward side of *w must be valid. */
+int dfr_wcs_fit_inverse_sip(dfr_wcs *w, int32_t order, int32_t nx, int32_t ny, double *max_resid_px);
+
 /* Counters of the last dfr_reproject* call on this thread (HOST):
  * stats[0] = tiles on the fast path, [1] = tiles on the exact path,
  * [2] = tiles entirely outside the footprint, [3] = kernels launched. */

@@ -21,7 +21,7 @@ _ORDER_NAMES = {"nearest": 0, "nearest-neighbor": 0, "bilinear": 1, "bicubic": 3
 
 EXPORTS = ["dfr_reproject", "dfr_reproject_ex", "dfr_reproject_host", "dfr_reproject_stack",
            "dfr_stack_finalize", "dfr_stack_host", "dfr_pix2world",
-           "dfr_world2pix", "dfr_src_coords", "dfr_wcs_set_pc_cdelt", "dfr_last_stats",
+           "dfr_world2pix", "dfr_src_coords", "dfr_wcs_set_pc_cdelt", "dfr_wcs_fit_inverse_sip", "dfr_last_stats",
            "dfr_profile_enable", "dfr_profile_last",
            "dfr_strerror", "dfr_last_error", "dfr_version"]
 
@@ -65,6 +65,7 @@ def lib():
         L.dfr_world2pix.argtypes = [wp, dp, dp, i64, dp, dp, vp]
         L.dfr_src_coords.argtypes = [i32, i32, i32, wp, wp, i32, i32, i32, dp, dp, vp, i32]
         L.dfr_wcs_set_pc_cdelt.argtypes = [wp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.dfr_wcs_fit_inverse_sip.argtypes = [wp, i32, i32, i32, C.POINTER(C.c_double)]
         L.dfr_last_stats.argtypes = [C.POINTER(C.c_int64)]
         L.dfr_profile_enable.argtypes = [C.c_int]
         L.dfr_profile_last.argtypes = [C.POINTER(C.c_float)]
@@ -305,6 +306,14 @@ def dfr_wcs_set_pc_cdelt(wcs: DfrWCS, pc, cdelt):
     cd_a = (C.c_double * 2)(*[float(v) for v in cdelt])
     _check(lib().dfr_wcs_set_pc_cdelt(C.byref(wcs), pc_a, cd_a))
     return wcs
+
+
+def dfr_wcs_fit_inverse_sip(wcs: DfrWCS, order: int, nx: int, ny: int) -> float:
+    """dfr_wcs_fit_inverse_sip: fits AP/BP into `wcs` (a packed DfrWCS, modified in place);
+    returns the largest round-trip residual on the fit grid, in pixels."""
+    res = C.c_double(0.0)
+    _check(lib().dfr_wcs_fit_inverse_sip(C.byref(wcs), int(order), int(nx), int(ny), C.byref(res)))
+    return float(res.value)
 
 
 def dfr_last_stats():

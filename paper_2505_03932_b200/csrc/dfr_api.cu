@@ -510,6 +510,21 @@ int dfr_wcs_set_pc_cdelt(dfr_wcs *w, const double pc[4], const double cdelt[2])
     return DFR_OK;
 }
 
+int dfr_wcs_fit_inverse_sip(dfr_wcs *w, int32_t order, int32_t nx, int32_t ny, double *max_resid_px)
+{
+    if (!w) { set_error("NULL pointer"); return DFR_ERR_NULL; }
+    if (order < 1 || order > DFR_SIP_MAX_ORDER) {
+        set_error("inverse SIP order %d outside [1, %d]", order, DFR_SIP_MAX_ORDER);
+        return DFR_ERR_SIP_ORDER;
+    }
+    if (nx < 1 || ny < 1) { set_error("bad image shape %dx%d", ny, nx); return DFR_ERR_SHAPE; }
+    dfr_wcs probe = *w;
+    probe.ap_order = probe.bp_order = 0;          // only the forward side has to be valid
+    const int rc = validate_wcs(&probe);
+    if (rc != DFR_OK) return rc;
+    return fit_inverse_sip(w, order, nx, ny, max_resid_px);
+}
+
 int dfr_last_stats(int64_t stats[4])
 {
     if (!stats) return DFR_ERR_NULL;

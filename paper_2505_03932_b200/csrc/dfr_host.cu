@@ -15,6 +15,7 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <vector>
 
 #include "dfr_internal.h"
 
@@ -160,6 +161,106 @@ void make_sky(const dfr_wcs *w, SkyDev *out)
     pack_poly(w->b, w->b_order, &out->b);
     pack_poly(w->ap, w->ap_order, &out->ap);
     pack_poly(w->bp, w->bp_order, &out->bp);
+}
+
+// ---- inverse SIP fit ---------------------------------------
+// Least squares by Householder QR (the scaled-monomial Gram matrix of order 9 is far too
+// ill-conditioned for normal equations). A is m x n column-major, overwritten; b1, b2 are
+// the two right-hand sides, overwritten; the solutions come back in x1, x2.
+static void qr_solve2(std::vector<double> &A, int m, int n, std::vector<double> &b1,
+                      std::vector<double> &b2, std::vector<double> &x1, std::vector<double> &x2)
+{
+    for (int k = 0; k < n; ++k) {
+        double *col = &A[(size_t)k * m];
+        double norm = 0.0;
+        for (int i = k; i < m; ++i) norm += col[i] * col[i];
+        norm = std::sqrt(norm);
+        if (norm == 0.0) continue;
+        const double alpha = col[k] > 0.0 ? -norm : norm;
+        col[k] -= alpha;                              // v = x - alpha e_k, stored in place
+        double vnorm2 = 0.0;
+        for (int i = k; i < m; ++i) vnorm2 += col[i] * col[i];
+        if (vnorm2 > 0.0) {
+            auto reflect = [&](double *y) {
+                double dot = 0.0;
+                for (int i = k; i < m; ++i) dot += col[i] * y[i];
+                const double f = 2.0 * dot / vnorm2;
+                for (int i = k; i < m; ++i) y[i] -= f * col[i];
+            };
+            for (int j = k + 1; j < n; ++j) reflect(&A[(size_t)j * m]);
+            reflect(b1.data());
+            reflect(b2.data());
+        }
+        col[k] = alpha;                               // R_kk (the rest of v is no longer needed)
+    }
+    x1.assign((size_t)n, 0.0);
+    x2.assign((size_t)n, 0.0);
+    for (int k = n - 1; k >= 0; --k) {
+        double s1 = b1[k], s2 = b2[k];
+        for (int j = k + 1; j < n; ++j) {
+            s1 -= A[(size_t)j * m + k] * x1[j];
+            s2 -= A[(size_t)j * m + k] * x2[j];
+        }
+        const double r = A[(size_t)k * m + k];
+        x1[k] = r != 0.0 ? s1 / r : 0.0;
+        x2[k] = r != 0.0 ? s2 / r : 0.0;
+    }
+}
+
+static double sip_sum(const double *c, int order, double u, double v)
+{
+    double r = 0.0;
+    for (int p = order; p >= 0; --p) {
+        double inner = 0.0;
+        for (int q = order - p; q >= 0; --q) inner = inner * v + c[p * DFR_SIP_DIM + q];
+        r = r * u + inner;
+    }
+    return r;
+}
+
+int fit_inverse_sip(dfr_wcs *w, int order, int nx, int ny, double *max_resid)
+{
+    constexpr int G = 64;
+    const int m = G * G, n = (order + 1) * (order + 2) / 2;
+    std::vector<double> U((size_t)m), V((size_t)m), du((size_t)m), dv((size_t)m);
+    double hx = 0.0, hy = 0.0;
+    for (int j = 0; j < G; ++j)
+        for (int i = 0; i < G; ++i) {
+            const double x = (nx - 1.0) * i / (G - 1.0), y = (ny - 1.0) * j / (G - 1.0);
+            const double u = x - (w->crpix[0] - 1.0), v = y - (w->crpix[1] - 1.0);
+            const int k = j * G + i;
+            U[k] = u + (w->a_order > 0 ? sip_sum(w->a, w->a_order, u, v) : 0.0);
+            V[k] = v + (w->b_order > 0 ? sip_sum(w->b, w->b_order, u, v) : 0.0);
+            du[k] = u - U[k];
+            dv[k] = v - V[k];
+            hx = std::fmax(hx, std::fabs(U[k]));
+            hy = std::fmax(hy, std::fabs(V[k]));
+        }
+    if (!(hx > 0.0)) hx = 1.0;
+    if (!(hy > 0.0)) hy = 1.0;
+    std::vector<double> A((size_t)m * n), x1, x2, b1 = du, b2 = dv;
+    int col = 0;
+    for (int p = 0; p <= order; ++p)
+        for (int q = 0; p + q <= order; ++q, ++col)
+            for (int k = 0; k < m; ++k) A[(size_t)col * m + k] = std::pow(U[k] / hx, p) * std::pow(V[k] / hy, q);
+    qr_solve2(A, m, n, b1, b2, x1, x2);
+    std::memset(w->ap, 0, sizeof w->ap);
+    std::memset(w->bp, 0, sizeof w->bp);
+    col = 0;
+    for (int p = 0; p <= order; ++p)
+        for (int q = 0; p + q <= order; ++q, ++col) {
+            const double s = std::pow(hx, p) * std::pow(hy, q);
+            w->ap[p * DFR_SIP_DIM + q] = x1[col] / s;
+            w->bp[p * DFR_SIP_DIM + q] = x2[col] / s;
+        }
+    w->ap_order = w->bp_order = order;
+    double res = 0.0;
+    for (int k = 0; k < m; ++k) {
+        res = std::fmax(res, std::fabs(sip_sum(w->ap, order, U[k], V[k]) - du[k]));
+        res = std::fmax(res, std::fabs(sip_sum(w->bp, order, U[k], V[k]) - dv[k]));
+    }
+    if (max_resid) *max_resid = res;
+    return DFR_OK;
 }
 
 }  // namespace dfr

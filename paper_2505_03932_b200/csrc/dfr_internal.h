@@ -49,6 +49,7 @@ void pack_poly(const double *c10x10, int order, Poly *out);
 void make_target(const dfr_wcs *t, TargetDev *out);
 void make_source(const dfr_wcs *t, const dfr_wcs *s, SourceDev *out);
 void make_sky(const dfr_wcs *w, SkyDev *out);
+int  fit_inverse_sip(dfr_wcs *w, int order, int nx, int ny, double *max_resid);
 void set_error(const char *fmt, ...);
 int  cuda_fail(cudaError_t e, const char *what);            // records text, returns DFR_ERR_CUDA
 
