@@ -335,3 +335,9 @@ def dfr_profile_last():
 
 def dfr_version() -> int:
     return int(lib().dfr_version())
+
+
+def calculate_reprojection(*args, **kwargs):
+    """see paper_2505_03932_b200.api.calculate_reprojection."""
+    from .api import calculate_reprojection as f
+    return f(*args, **kwargs)
