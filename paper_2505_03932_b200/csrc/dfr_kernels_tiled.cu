@@ -74,6 +74,28 @@ static FitConsts make_fit_consts()
     return f;
 }
 
+// Programmatic dependent launch (PDL): a kernel launched with launch_pdl() may start while
+// its predecessor in the stream is still running; it must call pdl_wait() before touching
+// anything the predecessor writes. pdl_trigger() in the predecessor allows that early start.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <class... KArgs, class... Args>
+static cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args &&...args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 constexpr double kHalf = 0.5 * TS;            // 16: pixel offset of s = 1
 constexpr double kCentre = 0.5 * (TS - 1);    // 15.5: tile centre relative to its first pixel
 constexpr int kNoBox = 0x7fffffff;            // cta_box entry of a CTA tile without FAST tiles
@@ -86,6 +108,7 @@ target_nodes_kernel(const __grid_constant__ TargetDev tgt, const __grid_constant
                     int ctas_x, int ctas, double2 *__restrict__ uv)
 {
     // sample points of the 64x64 CTA tiles (the parent fit of tile_setup_kernel)
+    pdl_trigger();                                  // the setup kernel may stage its constants meanwhile
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= ctas * NPTS) return;
     const int c = idx / NPTS, k = idx - c * NPTS;
@@ -295,7 +318,9 @@ tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ 
             sm[k] = v;
         }
     }
+    pdl_trigger();                                  // the main kernel's launch may overlap this one
     __syncthreads();
+    pdl_wait();                                     // the node table is complete
     const int c = blockIdx.x * kSetupThreads + threadIdx.x;
     int nflag[3] = {0, 0, 0};
     if (c < ctas) {
@@ -806,6 +831,7 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
     const int ntile = P.tiles_x * P.tiles_y;
     const TileRec *rec = P.recs + ((size_t)e * ntile + (active ? tty * P.tiles_x + ttx : 0));
 
+    pdl_wait();                         // the setup kernel's records and box origins are complete
     // ---- stage the CTA tile's source box first: its origin was reduced by the setup kernel
     // (cta_box), so the TMA load does not wait for the tile records, which load meanwhile.
     int ox = 0, oy = 0;                 // origin of the staged box in source pixels
@@ -989,6 +1015,7 @@ tiled_stack_kernel(const __grid_constant__ TiledParams P, const __grid_constant_
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    pdl_wait();                         // the setup kernel's records and box origins are complete
 
     if (warp == kStackConsumers) {
         // ------------------------------ producer (one lane) ------------------------------
@@ -1221,8 +1248,7 @@ static cudaError_t launch_main(const TiledParams &P, const TargetDev &tgt, const
     for (int e0 = 0; e0 < P.n; e0 += 65535) {
         Q.e0 = e0;
         const dim3 grid((unsigned)P.ctas_x, (unsigned)P.ctas_y, (unsigned)std::min(P.n - e0, 65535));
-        kern<<<grid, 32 * CTA_T * CTA_T, smem, st>>>(Q, tgt, tmap);
-        const cudaError_t err = cudaGetLastError();
+        const cudaError_t err = launch_pdl(kern, grid, dim3(32 * CTA_T * CTA_T), smem, st, Q, tgt, tmap);
         if (err != cudaSuccess) return err;
     }
     return cudaSuccess;
@@ -1262,11 +1288,11 @@ static cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, cons
     const unsigned bx = (unsigned)((ctas + kSetupThreads - 1) / kSetupThreads);
     for (int e0 = 0; e0 < n; e0 += 65535) {
         const dim3 grid(bx, (unsigned)std::min(n - e0, 65535));
-        if (maxo == 0) tile_setup_kernel<0><<<grid, 128, 0, st>>>(sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
-        else if (maxo <= 3) tile_setup_kernel<3><<<grid, 128, 0, st>>>(sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
-        else if (maxo <= 5) tile_setup_kernel<5><<<grid, 128, 0, st>>>(sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
-        else tile_setup_kernel<9><<<grid, 128, 0, st>>>(sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
-        if ((err = cudaGetLastError()) != cudaSuccess) return err;
+        if (maxo == 0) err = launch_pdl(tile_setup_kernel<0>, grid, dim3(128), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
+        else if (maxo <= 3) err = launch_pdl(tile_setup_kernel<3>, grid, dim3(128), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
+        else if (maxo <= 5) err = launch_pdl(tile_setup_kernel<5>, grid, dim3(128), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
+        else err = launch_pdl(tile_setup_kernel<9>, grid, dim3(128), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
+        if (err != cudaSuccess) return err;
     }
     return cudaSuccess;
 }
@@ -1393,8 +1419,7 @@ static cudaError_t launch_stack(TiledParams P, const TargetDev &tgt, const CUten
         S2.add = 1;
     }
     const dim3 grid((unsigned)P.ctas_x, (unsigned)P.ctas_y, (unsigned)best);
-    kern<<<grid, kStackThreads, smem, st>>>(P, tgt, tmap, S2);
-    return cudaGetLastError();
+    return launch_pdl(kern, grid, dim3(kStackThreads), smem, st, P, tgt, tmap, S2);
 }
 
 cudaError_t launch_tiled_stack(const float *src, int n, int sny, int snx, const TargetDev &tgt,
