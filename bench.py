@@ -306,16 +306,16 @@ def main():
     if args.e2e_steps > 0:
         hsrc = torch.from_numpy(w.images).pin_memory()
         hout = torch.empty((BATCH, NPIX, NPIX), dtype=torch.float32).pin_memory()
-        P.dfr_reproject_host(hsrc, ws_arr, tw, (NPIX, NPIX), P.BILINEAR, out_host=hout, batch=8)
+        P.dfr_reproject_host(hsrc, ws_arr, tw, (NPIX, NPIX), P.BILINEAR, out_host=hout, batch=4)
         barrier()
         t0 = time.perf_counter()
         for _ in range(args.e2e_steps):
-            P.dfr_reproject_host(hsrc, ws_arr, tw, (NPIX, NPIX), P.BILINEAR, out_host=hout, batch=8)
+            P.dfr_reproject_host(hsrc, ws_arr, tw, (NPIX, NPIX), P.BILINEAR, out_host=hout, batch=4)
         torch.cuda.synchronize()
         el = max_over_ranks(time.perf_counter() - t0, device="cuda")
         e2e = {"value": out_mpix * world * args.e2e_steps / el, "unit": UNIT,
                "h2d_bytes_per_step": int(w.images.nbytes), "d2h_bytes_per_step": int(hout.numel() * 4),
-               "steps": args.e2e_steps, "api": "dfr_reproject_host(batch=8), pinned host buffers"}
+               "steps": args.e2e_steps, "api": "dfr_reproject_host(batch=4), pinned host buffers"}
         same = bool(torch.equal(torch.nan_to_num(hout[:2], nan=-1.0), torch.nan_to_num(out[:2].cpu(), nan=-1.0)))
         e2e["matches_device_path"] = same
 
