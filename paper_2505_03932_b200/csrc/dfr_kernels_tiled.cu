@@ -817,7 +817,7 @@ __device__ __forceinline__ void warp_tile(const TiledParams &P, const TargetDev 
 // main kernel: one CTA per 64x64 output tile per exposure, one warp per 32x32 tile
 // ---------------------------------------------------------------------------------
 template <int ORDER, bool STAGE>
-__global__ void __launch_bounds__(32 * CTA_T * CTA_T)
+__global__ void __launch_bounds__(32 * CTA_T * CTA_T, 8)
 tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_constant__ TargetDev tgt,
                        const __grid_constant__ CUtensorMap tmap)
 {
