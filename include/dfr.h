@@ -130,7 +130,9 @@ int dfr_reproject_host(const float *src_host, int32_t n, int32_t src_ny, int32_t
  *   wsum[j][i] (+)= sum over the same e of weights[e]
  * where v_e is what dfr_reproject would store for exposure e, and exposure e
  * contributes to a pixel only where v_e is not NaN (inside its footprint and no
- * NaN under the taps). Accumulation is float32, in exposure order.
+ * NaN under the taps). Accumulation is float32. Large batches are split into exposure
+ * chunks whose partial sums are combined with atomic adds, so the last bits of `sum` may
+ * differ from run to run; `wsum` is exact whenever the weights' partial sums are.
  *   src_batch, src_wcs, tgt_wcs, out_ny/nx, order : as dfr_reproject
  *   weights    : HOST float32[n], or NULL for 1.0 each (must be finite)
  *   sum, wsum  : DEVICE float32 [out_ny][out_nx] each; must not overlap src_batch

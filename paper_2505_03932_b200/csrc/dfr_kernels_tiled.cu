@@ -402,12 +402,6 @@ __device__ __forceinline__ uint32_t smem_u32(const void *p)
     return (uint32_t)__cvta_generic_to_shared(p);
 }
 
-// Per-axis constants of the fast gather: valid floor/rint index range and address bias.
-struct AxisFast {
-    int C;              // k = float_as_int(T) - C  is the index relative to `lo`
-    unsigned cnt;       // valid <=> (unsigned)k < cnt
-};
-
 // index range [A_lo, A_hi] of the base tap for which every tap is inside the image AND
 // inside the staged box [o, o + B)
 template <int ORDER>

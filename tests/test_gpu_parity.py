@@ -289,3 +289,48 @@ def test_two_level_setup_fallback(P):
         else:
             assert st["tiles_exact"] == 0 and st["tiles_fast"] > 200
             assert d < 5e-6                   # 1.3e-5 if the parent cubic had been accepted
+
+
+def test_random_geometries_tiled_vs_exact(P):
+    """Robustness of the unchecked interior loop: 36 seeded random geometries (scale ratio
+    0.6-1.7, any rotation, offsets that leave part of the target uncovered, SIP on both
+    sides, ragged shapes) x 3 orders. The tiled path must agree with the exact per-pixel
+    path to the value tolerance wherever both are valid, differ in validity only on the
+    footprint edge, and the stack must equal the NaN-aware sum of the exact reprojections."""
+    rng = np.random.default_rng(2024)
+    worst = 0.0
+    for case in range(36):
+        sny, snx = (int(v) for v in rng.integers(90, 420, 2))
+        snx = snx // 4 * 4 if case % 3 else snx                    # both staged and unstaged sources
+        ony, onx = (int(v) for v in rng.integers(70, 400, 2))
+        n = int(rng.integers(1, 4))
+        imgs = np.stack([S.make_image(sny, snx, 30, rng) for _ in range(n)])
+        scale = S.PIXSCALE * rng.uniform(0.6, 1.7)
+        srcs = []
+        for _ in range(n):
+            w = S.make_wcs(snx, sny, 150.0 + rng.uniform(-0.02, 0.02), 2.0 + rng.uniform(-0.02, 0.02),
+                           rng.uniform(0, 360), S.PIXSCALE)
+            srcs.append(S.add_sip(w, int(rng.integers(2, 6)), snx / 2.0, rng, amp=10 ** rng.uniform(-6, -3.5)))
+        tgt = S.make_wcs(onx, ony, 150.0, 2.0, rng.uniform(0, 360), scale)
+        if case % 2:
+            S.add_sip(tgt, 3, onx / 2.0, rng, amp=1e-4)
+        src = torch.from_numpy(imgs).cuda()
+        dr = max(PR.dyn_range(im) for im in imgs)
+        for order in (0, 1, 3):
+            fast = P.dfr_reproject(src, srcs, tgt, (ony, onx), order, path=P.PATH_AUTO)
+            st = P.dfr_last_stats()
+            exact = P.dfr_reproject(src, srcs, tgt, (ony, onx), order, path=P.PATH_EXACT)
+            mf, mx = torch.isnan(fast), torch.isnan(exact)
+            assert int((mf != mx).sum()) <= 4 * (ony + onx) * n, (case, order)   # only along footprint edges
+            both = ~mf & ~mx
+            if order > 0 and bool(both.any()):
+                d = float((fast[both] - exact[both]).abs().max())
+                worst = max(worst, d / dr)
+                assert d <= PR.VALUE_TOL * dr, (case, order, d, st)
+            if order == 1:
+                s, ws = P.dfr_reproject_stack(src, srcs, tgt, (ony, onx), order)
+                ok = ~(mf != mx).any(0)
+                ref = torch.nan_to_num(exact, nan=0.0).sum(0)
+                assert torch.equal(ws[ok], (~mx).sum(0).float()[ok]), (case, "wsum")
+                assert float((s[ok] - ref[ok]).abs().max()) <= PR.VALUE_TOL * dr * n, (case, "sum")
+    print("random geometries: worst tiled-vs-exact value difference", worst, "x DR")
