@@ -171,3 +171,25 @@ def test_stack_host_stream(P):
     dr = max(PR.dyn_range(im) for im in w.images)
     assert np.abs(s.numpy()[~band] - so[~band]).max() <= PR.VALUE_TOL * dr * wts.sum()
     assert 0.5 < (wo == 0).mean() < 0.95                  # a mosaic: most of it is empty
+
+
+def test_stack_many_exposures_few_tiles(P):
+    """40 exposures onto a 3 x 3-tile target: the grid is cut into the maximum number of
+    exposure chunks, including chunks of unequal length; signed weights."""
+    rng = np.random.default_rng(81)
+    n, sn, on = 40, 128, 160
+    imgs = np.stack([S.make_image(sn, sn, 8, rng) for _ in range(n)])
+    srcs = [S.make_wcs(sn, sn, 150.0 + 0.01 * rng.uniform(-1, 1), 2.0 + 0.01 * rng.uniform(-1, 1),
+                       rng.uniform(0, 360), S.PIXSCALE) for _ in range(n)]
+    tgt = S.make_wcs(on, on, 150.0, 2.0, 10.0, S.PIXSCALE * 1.2)
+    w = S.Workload("many", imgs, srcs, tgt, (on, on), (1,))
+    wts = rng.integers(-8, 17, n) / 4.0
+    st = check_stack(P, w, 1, wts)
+    # accumulate=True on top of existing contents with several chunks
+    src = torch.from_numpy(imgs).cuda()
+    s0 = torch.full((on, on), 3.0, device="cuda")
+    w0 = torch.full((on, on), 1.0, device="cuda")
+    s, c = P.dfr_reproject_stack(src, srcs, tgt, (on, on), 1, weights=wts)
+    P.dfr_reproject_stack(src, srcs, tgt, (on, on), 1, weights=wts, sum=s0, wsum=w0, accumulate=True)
+    assert torch.equal(w0, c + 1.0) and torch.allclose(s0, s + 3.0, rtol=1e-6, atol=1e-3)
+    print("stack many", st)
