@@ -50,7 +50,8 @@ static int check_common(int32_t n, int32_t sny, int32_t snx, const dfr_wcs *sw, 
 // Per-thread record of the last call: tile counters land in pinned host memory through an
 // async copy; dfr_last_stats waits for it. Also the optional timing events (dfr_profile_*).
 struct LastCall {
-    int32_t *pinned = nullptr;          // 3 counters: fast, exact, empty
+    int32_t *pinned = nullptr;          // 3 counters: fast, exact, empty (mapped host memory,
+    int32_t *pinned_dev = nullptr;      // written by the setup kernel through this device pointer)
     cudaEvent_t done = nullptr;
     bool pending = false;
     int64_t kernels = 0;
@@ -69,7 +70,10 @@ static int stack_impl(const float *src_batch, int32_t n, int32_t src_ny, int32_t
 static cudaError_t ensure_last()
 {
     cudaError_t err;
-    if (!g_last.pinned && (err = cudaMallocHost((void **)&g_last.pinned, 4 * sizeof(int32_t))) != cudaSuccess) return err;
+    if (!g_last.pinned) {
+        if ((err = cudaHostAlloc((void **)&g_last.pinned, 4 * sizeof(int32_t), cudaHostAllocMapped)) != cudaSuccess) return err;
+        if ((err = cudaHostGetDevicePointer((void **)&g_last.pinned_dev, g_last.pinned, 0)) != cudaSuccess) return err;
+    }
     if (!g_last.done && (err = cudaEventCreateWithFlags(&g_last.done, cudaEventDisableTiming)) != cudaSuccess) return err;
     return cudaSuccess;
 }
@@ -130,16 +134,11 @@ static int reproject_impl(const float *src, int32_t n, int32_t sny, int32_t snx,
         g_last.kernels = 1;
         g_last.tiled = false;
     } else {
-        int32_t *dcnt = nullptr;
         err = ensure_last();
-        if (err == cudaSuccess) err = cudaMallocAsync((void **)&dcnt, 4 * sizeof(int32_t), st);
         if (err == cudaSuccess)
             err = launch_tiled_reproject(src, n, sny, snx, tgt, dsrc, hsrc.data(), ony, onx, order, out, st,
-                                         dcnt, &ts, &g_last.prof);
-        if (err == cudaSuccess)
-            err = cudaMemcpyAsync(g_last.pinned, dcnt, 3 * sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+                                         g_last.pinned_dev, &ts, &g_last.prof);
         if (err == cudaSuccess) err = cudaEventRecord(g_last.done, st);
-        if (dcnt) cudaFreeAsync(dcnt, st);
         g_last.kernels = ts.kernels;
         g_last.tiled = true;
         g_last.pending = (err == cudaSuccess);
@@ -256,20 +255,15 @@ static int stack_impl(const float *src_batch, int32_t n, int32_t src_ny, int32_t
     rc = upload_sources(n, src_wcs, tgt_wcs, st, hsrc, &dsrc);
     if (rc != DFR_OK) return rc;
     float *dw = nullptr;
-    int32_t *dcnt = nullptr;
     TiledStats ts = {0, 0, 0, 0};
     cudaError_t err = ensure_last();
     if (err == cudaSuccess) err = cudaMallocAsync((void **)&dw, sizeof(float) * (size_t)n, st);
     // pageable source: the runtime stages the bytes before returning, so `hw` may die
     if (err == cudaSuccess) err = cudaMemcpyAsync(dw, hw.data(), sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, st);
-    if (err == cudaSuccess) err = cudaMallocAsync((void **)&dcnt, 4 * sizeof(int32_t), st);
     if (err == cudaSuccess)
         err = launch_tiled_stack(src_batch, n, src_ny, src_nx, tgt, dsrc, hsrc.data(), out_ny, out_nx, order,
-                                 dw, sum, wsum, accumulate != 0, st, dcnt, &ts, &g_last.prof);
-    if (err == cudaSuccess)
-        err = cudaMemcpyAsync(g_last.pinned, dcnt, 3 * sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+                                 dw, sum, wsum, accumulate != 0, st, g_last.pinned_dev, &ts, &g_last.prof);
     if (err == cudaSuccess) err = cudaEventRecord(g_last.done, st);
-    if (dcnt) cudaFreeAsync(dcnt, st);
     if (dw) cudaFreeAsync(dw, st);
     cudaFreeAsync(dsrc, st);
     g_last.kernels = ts.kernels;

@@ -105,8 +105,10 @@ constexpr int kNoBox = 0x7fffffff;            // cta_box entry of a CTA tile wit
 // ---------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128)
 target_nodes_kernel(const __grid_constant__ TargetDev tgt, const __grid_constant__ FitConsts fc,
-                    int ctas_x, int ctas, double2 *__restrict__ uv)
+                    int ctas_x, int ctas, double2 *__restrict__ uv, int32_t *__restrict__ counters)
 {
+    // tile counters + ticket of the setup kernel start from zero (no memset in the stream)
+    if (blockIdx.x == 0 && threadIdx.x < 4) counters[threadIdx.x] = 0;
     // sample points of the 64x64 CTA tiles (the parent fit of tile_setup_kernel)
     pdl_trigger();                                  // the setup kernel may stage its constants meanwhile
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
@@ -295,7 +297,8 @@ __global__ void __launch_bounds__(kSetupThreads)
 tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ srcdev,
                   const __grid_constant__ TargetDev tgt, const __grid_constant__ FitConsts fc, int e0,
                   int tiles_x, int tiles_y, int ctas_x, int ctas, int sny, int snx,
-                  TileRec *__restrict__ recs, int2 *__restrict__ cta_box, int32_t *__restrict__ counters)
+                  TileRec *__restrict__ recs, int2 *__restrict__ cta_box, int32_t *__restrict__ counters,
+                  int total_blocks, int32_t *__restrict__ host_stats)
 {
     __shared__ double sm[11 + 2 * tri(N)];
     const int e = e0 + blockIdx.y;
@@ -365,11 +368,20 @@ tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ 
         // origin of the CTA tile's staged box = min over its FAST tiles (kNoBox: none)
         cta_box[(size_t)e * ctas + c] = make_int2(box_x, box_y);
     }
-    if (counters) {
+    // tile statistics: per-warp sums -> device counters; the last block of the last launch
+    // (ticket) writes the totals straight into the caller's mapped host memory, so
+    // dfr_last_stats needs neither a memset nor a copy in the stream
 #pragma unroll
-        for (int f = 0; f < 3; ++f) {
-            const int w = __reduce_add_sync(0xffffffffu, nflag[f]);
-            if ((threadIdx.x & 31) == 0 && w) atomicAdd(&counters[f], w);
+    for (int f = 0; f < 3; ++f) {
+        const int w = __reduce_add_sync(0xffffffffu, nflag[f]);
+        if ((threadIdx.x & 31) == 0 && w) atomicAdd(&counters[f], w);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0 && host_stats) {
+        __threadfence();
+        if (atomicAdd(&counters[3], 1) == total_blocks - 1) {
+            __threadfence();
+            for (int f = 0; f < 3; ++f) host_stats[f] = *(volatile int32_t *)&counters[f];
         }
     }
 }
@@ -1252,11 +1264,12 @@ struct Scratch {
     double2 *uv = nullptr;
     TileRec *recs = nullptr;
     int2 *cta_box = nullptr;
+    int32_t *counters = nullptr;                    // fast, exact, empty, ticket
 };
 
 static cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const SourceDev *srcdev,
                              const SourceDev *srchost, int ony, int onx, cudaStream_t st,
-                             int32_t *counters, Scratch &sc, TiledParams &P)
+                             int32_t *host_stats, Scratch &sc, TiledParams &P)
 {
     static const FitConsts fc = make_fit_consts();
     P.n = n; P.sny = sny; P.snx = snx; P.ony = ony; P.onx = onx;
@@ -1273,19 +1286,21 @@ static cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, cons
     P.recs = sc.recs;
     if ((err = cudaMallocAsync((void **)&sc.cta_box, sizeof(int2) * (size_t)ctas * n, st)) != cudaSuccess) return err;
     P.cta_box = sc.cta_box;
-    if (counters && (err = cudaMemsetAsync(counters, 0, 3 * sizeof(int32_t), st)) != cudaSuccess) return err;
-    target_nodes_kernel<<<(ctas * NPTS + 127) / 128, 128, 0, st>>>(tgt, fc, P.ctas_x, ctas, sc.uv);
+    if ((err = cudaMallocAsync((void **)&sc.counters, 4 * sizeof(int32_t), st)) != cudaSuccess) return err;
+    target_nodes_kernel<<<(ctas * NPTS + 127) / 128, 128, 0, st>>>(tgt, fc, P.ctas_x, ctas, sc.uv, sc.counters);
     if ((err = cudaGetLastError()) != cudaSuccess) return err;
     // SIP order class of the batch: inverse polynomials are zero-padded up to N
     int maxo = 0;
     for (int e = 0; e < n; ++e) maxo = std::max(maxo, std::max(srchost[e].ap.order, srchost[e].bp.order));
     const unsigned bx = (unsigned)((ctas + kSetupThreads - 1) / kSetupThreads);
+    const long long total_blocks = (long long)bx * n;
+    if (total_blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     for (int e0 = 0; e0 < n; e0 += 65535) {
         const dim3 grid(bx, (unsigned)std::min(n - e0, 65535));
-        if (maxo == 0) err = launch_pdl(tile_setup_kernel<0>, grid, dim3(128), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
-        else if (maxo <= 3) err = launch_pdl(tile_setup_kernel<3>, grid, dim3(128), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
-        else if (maxo <= 5) err = launch_pdl(tile_setup_kernel<5>, grid, dim3(128), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
-        else err = launch_pdl(tile_setup_kernel<9>, grid, dim3(128), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, counters);
+        if (maxo == 0) err = launch_pdl(tile_setup_kernel<0>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats);
+        else if (maxo <= 3) err = launch_pdl(tile_setup_kernel<3>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats);
+        else if (maxo <= 5) err = launch_pdl(tile_setup_kernel<5>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats);
+        else err = launch_pdl(tile_setup_kernel<9>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats);
         if (err != cudaSuccess) return err;
     }
     return cudaSuccess;
@@ -1296,6 +1311,7 @@ static void free_scratch(Scratch &sc, cudaStream_t st)
     if (sc.uv) cudaFreeAsync(sc.uv, st);
     if (sc.recs) cudaFreeAsync(sc.recs, st);
     if (sc.cta_box) cudaFreeAsync(sc.cta_box, st);
+    if (sc.counters) cudaFreeAsync(sc.counters, st);
 }
 
 // Setup kernels + staging decision shared by the per-exposure and the stacking launchers.
@@ -1309,12 +1325,12 @@ struct Prepared {
 
 static cudaError_t prepare_tiled(const float *src, int n, int sny, int snx, const TargetDev &tgt,
                                  const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx,
-                                 int order, cudaStream_t st, int32_t *dev_counters, Prepared &R)
+                                 int order, cudaStream_t st, int32_t *host_stats, Prepared &R)
 {
     std::memset(&R.P, 0, sizeof R.P);
     std::memset(&R.tmap, 0, sizeof R.tmap);
     R.P.src = src;
-    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, srchost, ony, onx, st, dev_counters, R.sc, R.P);
+    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, srchost, ony, onx, st, host_stats, R.sc, R.P);
     if (err != cudaSuccess) return err;
     // ---- staging decision: box size from a host probe; TMA needs 16-byte rows
     double ex, ey;
@@ -1345,11 +1361,11 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
                                    const TargetDev &tgt, const SourceDev *srcdev,
                                    const SourceDev *srchost,
                                    int ony, int onx, int order, float *out, cudaStream_t st,
-                                   int32_t *dev_counters, TiledStats *stats, ProfileEvents *prof)
+                                   int32_t *host_stats, TiledStats *stats, ProfileEvents *prof)
 {
     Prepared R;
     if (prof && prof->enabled) cudaEventRecord(prof->setup_begin, st);
-    cudaError_t err = prepare_tiled(src, n, sny, snx, tgt, srcdev, srchost, ony, onx, order, st, dev_counters, R);
+    cudaError_t err = prepare_tiled(src, n, sny, snx, tgt, srcdev, srchost, ony, onx, order, st, host_stats, R);
     if (err != cudaSuccess) { free_scratch(R.sc, st); return err; }
     R.P.out = out;
     if (prof && prof->enabled) cudaEventRecord(prof->main_begin, st);
@@ -1362,7 +1378,7 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
     if (prof && prof->enabled) cudaEventRecord(prof->main_end, st);
     free_scratch(R.sc, st);
     stats->kernels = 3;
-    stats->tiles_fast = stats->tiles_exact = stats->tiles_empty = -1;   // filled from dev_counters by the caller
+    stats->tiles_fast = stats->tiles_exact = stats->tiles_empty = -1;   // filled from host_stats by the caller
     return err;
 }
 
@@ -1419,11 +1435,11 @@ static cudaError_t launch_stack(TiledParams P, const TargetDev &tgt, const CUten
 cudaError_t launch_tiled_stack(const float *src, int n, int sny, int snx, const TargetDev &tgt,
                                const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx, int order,
                                const float *dev_weights, float *sum, float *wsum, int accumulate,
-                               cudaStream_t st, int32_t *dev_counters, TiledStats *stats, ProfileEvents *prof)
+                               cudaStream_t st, int32_t *host_stats, TiledStats *stats, ProfileEvents *prof)
 {
     Prepared R;
     if (prof && prof->enabled) cudaEventRecord(prof->setup_begin, st);
-    cudaError_t err = prepare_tiled(src, n, sny, snx, tgt, srcdev, srchost, ony, onx, order, st, dev_counters, R);
+    cudaError_t err = prepare_tiled(src, n, sny, snx, tgt, srcdev, srchost, ony, onx, order, st, host_stats, R);
     if (err != cudaSuccess) { free_scratch(R.sc, st); return err; }
     StackParams S;
     S.weights = dev_weights; S.sum = sum; S.wsum = wsum; S.add = accumulate; S.nchunk = 1;
