@@ -61,6 +61,30 @@ struct LastCall {
 static thread_local LastCall g_last;
 static thread_local int64_t g_stats_acc[4] = {0, 0, 0, 0};   // used by dfr_reproject_host
 static thread_local bool g_accumulate = false;
+static thread_local int32_t *g_stream_totals = nullptr;      // DEVICE int[3]: tile totals of a streaming call
+
+// Streaming calls (dfr_reproject_host, dfr_stack_host): the batches add their tile counters
+// into one device array (no host wait between batches); harvested once at the end.
+static cudaError_t stream_stats_begin()
+{
+    cudaError_t err;
+    if (!g_stream_totals && (err = cudaMalloc((void **)&g_stream_totals, 4 * sizeof(int32_t))) != cudaSuccess) return err;
+    if ((err = cudaMemset(g_stream_totals, 0, 4 * sizeof(int32_t))) != cudaSuccess) return err;
+    for (int k = 0; k < 4; ++k) g_stats_acc[k] = 0;
+    g_last.pending = false;
+    g_accumulate = true;
+    return cudaSuccess;
+}
+
+static void stream_stats_end()
+{
+    g_accumulate = false;
+    int32_t t[3] = {0, 0, 0};
+    if (cudaMemcpy(t, g_stream_totals, sizeof t, cudaMemcpyDeviceToHost) == cudaSuccess)
+        for (int k = 0; k < 3; ++k) g_stats_acc[k] = t[k];
+    g_last.pending = false;
+    g_last.kernels = -1;                 // marks "use the accumulated totals"
+}
 
 static int stack_impl(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
                       const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs, int32_t out_ny, int32_t out_nx,
@@ -113,11 +137,6 @@ static int reproject_impl(const float *src, int32_t n, int32_t sny, int32_t snx,
                           int32_t order, float *out, cudaStream_t st, int32_t path)
 {
     std::call_once(g_pool_once, tune_pool);
-    if (g_accumulate && g_last.pending) {         // previous batch of a streaming call
-        int64_t t[4];
-        collect_stats(t);
-        for (int k = 0; k < 4; ++k) g_stats_acc[k] += t[k];
-    }
     g_last.pending = false;
     TargetDev tgt;
     make_target(tw, &tgt);
@@ -137,11 +156,16 @@ static int reproject_impl(const float *src, int32_t n, int32_t sny, int32_t snx,
         err = ensure_last();
         if (err == cudaSuccess)
             err = launch_tiled_reproject(src, n, sny, snx, tgt, dsrc, hsrc.data(), ony, onx, order, out, st,
-                                         g_last.pinned_dev, &ts, &g_last.prof);
-        if (err == cudaSuccess) err = cudaEventRecord(g_last.done, st);
-        g_last.kernels = ts.kernels;
-        g_last.tiled = true;
-        g_last.pending = (err == cudaSuccess);
+                                         g_accumulate ? g_stream_totals : g_last.pinned_dev, g_accumulate ? 1 : 0,
+                                         &ts, &g_last.prof);
+        if (g_accumulate) {
+            g_stats_acc[3] += ts.kernels;
+        } else {
+            if (err == cudaSuccess) err = cudaEventRecord(g_last.done, st);
+            g_last.kernels = ts.kernels;
+            g_last.tiled = true;
+            g_last.pending = (err == cudaSuccess);
+        }
     }
     cudaFreeAsync(dsrc, st);
     if (err != cudaSuccess) return cuda_fail(err, "reproject launch");
@@ -242,11 +266,6 @@ static int stack_impl(const float *src_batch, int32_t n, int32_t src_ny, int32_t
     for (int32_t e = 0; weights && e < n; ++e) hw[e] = weights[e];
     std::call_once(g_pool_once, tune_pool);
     int rc;
-    if (g_accumulate && g_last.pending) {         // previous batch of a streaming call
-        int64_t t[4];
-        collect_stats(t);
-        for (int k = 0; k < 4; ++k) g_stats_acc[k] += t[k];
-    }
     g_last.pending = false;
     TargetDev tgt;
     make_target(tgt_wcs, &tgt);
@@ -262,13 +281,19 @@ static int stack_impl(const float *src_batch, int32_t n, int32_t src_ny, int32_t
     if (err == cudaSuccess) err = cudaMemcpyAsync(dw, hw.data(), sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, st);
     if (err == cudaSuccess)
         err = launch_tiled_stack(src_batch, n, src_ny, src_nx, tgt, dsrc, hsrc.data(), out_ny, out_nx, order,
-                                 dw, sum, wsum, accumulate != 0, st, g_last.pinned_dev, &ts, &g_last.prof);
-    if (err == cudaSuccess) err = cudaEventRecord(g_last.done, st);
+                                 dw, sum, wsum, accumulate != 0, st,
+                                 g_accumulate ? g_stream_totals : g_last.pinned_dev, g_accumulate ? 1 : 0,
+                                 &ts, &g_last.prof);
+    if (!g_accumulate && err == cudaSuccess) err = cudaEventRecord(g_last.done, st);
     if (dw) cudaFreeAsync(dw, st);
     cudaFreeAsync(dsrc, st);
-    g_last.kernels = ts.kernels;
-    g_last.tiled = true;
-    g_last.pending = (err == cudaSuccess);
+    if (g_accumulate) {
+        g_stats_acc[3] += ts.kernels;
+    } else {
+        g_last.kernels = ts.kernels;
+        g_last.tiled = true;
+        g_last.pending = (err == cudaSuccess);
+    }
     if (err != cudaSuccess) return cuda_fail(err, "reproject_stack launch");
     return DFR_OK;
 }
@@ -389,9 +414,7 @@ int dfr_reproject_host(const float *src_host, int32_t n, int32_t src_ny, int32_t
         err = ensure_slot(g_pipe.slot[k], in_px * batch * sizeof(float), out_px * batch * sizeof(float));
         if (err != cudaSuccess) return cuda_fail(err, "pipeline buffers");
     }
-    for (int k = 0; k < 4; ++k) g_stats_acc[k] = 0;
-    g_last.pending = false;
-    g_accumulate = true;
+    if ((err = stream_stats_begin()) != cudaSuccess) return cuda_fail(err, "stream statistics");
     for (int b = 0; b < nb; ++b) {
         Slot &s = g_pipe.slot[b % kSlots];
         const int32_t e0 = b * batch, ne = (n - e0 < batch) ? n - e0 : batch;
@@ -410,14 +433,7 @@ int dfr_reproject_host(const float *src_host, int32_t n, int32_t src_ny, int32_t
         err = cudaStreamSynchronize(g_pipe.slot[k].st);
         if (err != cudaSuccess && rc == DFR_OK) rc = cuda_fail(err, "pipeline sync");
     }
-    g_accumulate = false;
-    if (g_last.pending) {
-        int64_t t[4];
-        collect_stats(t);
-        for (int k = 0; k < 4; ++k) g_stats_acc[k] += t[k];
-        g_last.pending = false;
-    }
-    g_last.kernels = -1;                 // marks "use the accumulated totals"
+    stream_stats_end();
     return rc;
 }
 
@@ -461,9 +477,7 @@ int dfr_stack_host(const float *src_host, int32_t n, int32_t src_ny, int32_t src
     if (err == cudaSuccess) err = cudaEventRecord(zeroed, g_pipe.slot[0].st);
     for (int k = 1; k < used && err == cudaSuccess; ++k) err = cudaStreamWaitEvent(g_pipe.slot[k].st, zeroed, 0);
     if (err != cudaSuccess) { cudaEventDestroy(zeroed); return cuda_fail(err, "pipeline start"); }
-    for (int k = 0; k < 4; ++k) g_stats_acc[k] = 0;
-    g_last.pending = false;
-    g_accumulate = true;
+    if ((err = stream_stats_begin()) != cudaSuccess) return cuda_fail(err, "stream statistics");
     for (int b = 0; b < nb; ++b) {
         Slot &s = g_pipe.slot[b % kSlots];
         const int32_t e0 = b * batch, ne = (n - e0 < batch) ? n - e0 : batch;
@@ -480,14 +494,7 @@ int dfr_stack_host(const float *src_host, int32_t n, int32_t src_ny, int32_t src
         if (err != cudaSuccess && rc == DFR_OK) rc = cuda_fail(err, "pipeline sync");
     }
     cudaEventDestroy(zeroed);
-    g_accumulate = false;
-    if (g_last.pending) {
-        int64_t t[4];
-        collect_stats(t);
-        for (int k = 0; k < 4; ++k) g_stats_acc[k] += t[k];
-        g_last.pending = false;
-    }
-    g_last.kernels = -1;                 // marks "use the accumulated totals"
+    stream_stats_end();
     if (rc != DFR_OK) return rc;
     err = cudaMemcpy(sum_host, dsum, out_bytes, cudaMemcpyDeviceToHost);
     if (err == cudaSuccess) err = cudaMemcpy(wsum_host, dwsum, out_bytes, cudaMemcpyDeviceToHost);

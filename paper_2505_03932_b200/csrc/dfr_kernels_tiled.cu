@@ -298,7 +298,7 @@ tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ 
                   const __grid_constant__ TargetDev tgt, const __grid_constant__ FitConsts fc, int e0,
                   int tiles_x, int tiles_y, int ctas_x, int ctas, int sny, int snx,
                   TileRec *__restrict__ recs, int2 *__restrict__ cta_box, int32_t *__restrict__ counters,
-                  int total_blocks, int32_t *__restrict__ host_stats)
+                  int total_blocks, int32_t *__restrict__ host_stats, int stats_add)
 {
     __shared__ double sm[11 + 2 * tri(N)];
     const int e = e0 + blockIdx.y;
@@ -381,7 +381,11 @@ tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ 
         __threadfence();
         if (atomicAdd(&counters[3], 1) == total_blocks - 1) {
             __threadfence();
-            for (int f = 0; f < 3; ++f) host_stats[f] = *(volatile int32_t *)&counters[f];
+            for (int f = 0; f < 3; ++f) {
+                const int32_t v = *(volatile int32_t *)&counters[f];
+                if (stats_add) atomicAdd(&host_stats[f], v);     // streaming calls: device-side totals
+                else host_stats[f] = v;
+            }
         }
     }
 }
@@ -1269,7 +1273,7 @@ struct Scratch {
 
 static cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const SourceDev *srcdev,
                              const SourceDev *srchost, int ony, int onx, cudaStream_t st,
-                             int32_t *host_stats, Scratch &sc, TiledParams &P)
+                             int32_t *host_stats, int stats_add, Scratch &sc, TiledParams &P)
 {
     static const FitConsts fc = make_fit_consts();
     P.n = n; P.sny = sny; P.snx = snx; P.ony = ony; P.onx = onx;
@@ -1297,10 +1301,10 @@ static cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, cons
     if (total_blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     for (int e0 = 0; e0 < n; e0 += 65535) {
         const dim3 grid(bx, (unsigned)std::min(n - e0, 65535));
-        if (maxo == 0) err = launch_pdl(tile_setup_kernel<0>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats);
-        else if (maxo <= 3) err = launch_pdl(tile_setup_kernel<3>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats);
-        else if (maxo <= 5) err = launch_pdl(tile_setup_kernel<5>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats);
-        else err = launch_pdl(tile_setup_kernel<9>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats);
+        if (maxo == 0) err = launch_pdl(tile_setup_kernel<0>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
+        else if (maxo <= 3) err = launch_pdl(tile_setup_kernel<3>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
+        else if (maxo <= 5) err = launch_pdl(tile_setup_kernel<5>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
+        else err = launch_pdl(tile_setup_kernel<9>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
         if (err != cudaSuccess) return err;
     }
     return cudaSuccess;
@@ -1325,12 +1329,12 @@ struct Prepared {
 
 static cudaError_t prepare_tiled(const float *src, int n, int sny, int snx, const TargetDev &tgt,
                                  const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx,
-                                 int order, cudaStream_t st, int32_t *host_stats, Prepared &R)
+                                 int order, cudaStream_t st, int32_t *host_stats, int stats_add, Prepared &R)
 {
     std::memset(&R.P, 0, sizeof R.P);
     std::memset(&R.tmap, 0, sizeof R.tmap);
     R.P.src = src;
-    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, srchost, ony, onx, st, host_stats, R.sc, R.P);
+    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, srchost, ony, onx, st, host_stats, stats_add, R.sc, R.P);
     if (err != cudaSuccess) return err;
     // ---- staging decision: box size from a host probe; TMA needs 16-byte rows
     double ex, ey;
@@ -1361,11 +1365,11 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
                                    const TargetDev &tgt, const SourceDev *srcdev,
                                    const SourceDev *srchost,
                                    int ony, int onx, int order, float *out, cudaStream_t st,
-                                   int32_t *host_stats, TiledStats *stats, ProfileEvents *prof)
+                                   int32_t *host_stats, int stats_add, TiledStats *stats, ProfileEvents *prof)
 {
     Prepared R;
     if (prof && prof->enabled) cudaEventRecord(prof->setup_begin, st);
-    cudaError_t err = prepare_tiled(src, n, sny, snx, tgt, srcdev, srchost, ony, onx, order, st, host_stats, R);
+    cudaError_t err = prepare_tiled(src, n, sny, snx, tgt, srcdev, srchost, ony, onx, order, st, host_stats, stats_add, R);
     if (err != cudaSuccess) { free_scratch(R.sc, st); return err; }
     R.P.out = out;
     if (prof && prof->enabled) cudaEventRecord(prof->main_begin, st);
@@ -1435,11 +1439,11 @@ static cudaError_t launch_stack(TiledParams P, const TargetDev &tgt, const CUten
 cudaError_t launch_tiled_stack(const float *src, int n, int sny, int snx, const TargetDev &tgt,
                                const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx, int order,
                                const float *dev_weights, float *sum, float *wsum, int accumulate,
-                               cudaStream_t st, int32_t *host_stats, TiledStats *stats, ProfileEvents *prof)
+                               cudaStream_t st, int32_t *host_stats, int stats_add, TiledStats *stats, ProfileEvents *prof)
 {
     Prepared R;
     if (prof && prof->enabled) cudaEventRecord(prof->setup_begin, st);
-    cudaError_t err = prepare_tiled(src, n, sny, snx, tgt, srcdev, srchost, ony, onx, order, st, host_stats, R);
+    cudaError_t err = prepare_tiled(src, n, sny, snx, tgt, srcdev, srchost, ony, onx, order, st, host_stats, stats_add, R);
     if (err != cudaSuccess) { free_scratch(R.sc, st); return err; }
     StackParams S;
     S.weights = dev_weights; S.sum = sum; S.wsum = wsum; S.add = accumulate; S.nchunk = 1;
@@ -1472,7 +1476,7 @@ cudaError_t launch_tiled_coords(int n, int sny, int snx, const TargetDev &tgt,
     TiledParams P;
     std::memset(&P, 0, sizeof P);
     Scratch sc;
-    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, srchost, ony, onx, st, nullptr, sc, P);
+    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, srchost, ony, onx, st, nullptr, 0, sc, P);
     if (err == cudaSuccess) {
         for (int e0 = 0; e0 < n && err == cudaSuccess; e0 += 65535) {
             P.e0 = e0;

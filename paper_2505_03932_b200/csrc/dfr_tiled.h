@@ -39,13 +39,14 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
                                    const TargetDev &tgt, const SourceDev *srcdev,
                                    const SourceDev *srchost,
                                    int ony, int onx, int order, float *out, cudaStream_t st,
-                                   int32_t *host_stats /* device-visible mapped host memory, 3 ints, or NULL */,
+                                   int32_t *host_stats /* 3 ints the setup kernel can write (mapped host or device memory), or NULL */,
+                                   int stats_add /* 0: store the totals, 1: atomically add them (streaming) */,
                                    TiledStats *stats, ProfileEvents *prof);
 // dfr_reproject_stack: sum / wsum accumulated over the n exposures in one kernel.
 cudaError_t launch_tiled_stack(const float *src, int n, int sny, int snx, const TargetDev &tgt,
                                const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx, int order,
                                const float *dev_weights, float *sum, float *wsum, int accumulate,
-                               cudaStream_t st, int32_t *host_stats, TiledStats *stats, ProfileEvents *prof);
+                               cudaStream_t st, int32_t *host_stats, int stats_add, TiledStats *stats, ProfileEvents *prof);
 cudaError_t launch_stack_finalize(const float *sum, const float *wsum, long long npix, float *mean, cudaStream_t st);
 cudaError_t launch_tiled_coords(int n, int sny, int snx, const TargetDev &tgt,
                                 const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx, int order,
