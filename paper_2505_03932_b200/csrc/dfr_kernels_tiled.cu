@@ -66,7 +66,11 @@ static FitConsts make_fit_consts()
             f.pts[4 * b + a][1] = s[b];
         }
     const double h = 0.70710678118654752440;
-    const double chk[9][2] = {{0, 0}, {h, h}, {-h, h}, {h, -h}, {-h, -h}, {1, 1}, {-1, 1}, {1, -1}, {-1, -1}};
+    // check points: extrema of T4 (0, +-1/sqrt2, +-1) where the interpolation error of a cubic
+    // through Chebyshev nodes peaks. The axis points matter: at the centre, on the diagonals
+    // and at the corners |T4(s)| = |T4(t)| with equal signs, so fourth-order errors of
+    // opposite sign in s and t (u^4 - v^4) cancel there; (+-h, 0) and (0, +-h) separate them.
+    const double chk[9][2] = {{0, 0}, {h, 0}, {-h, 0}, {0, h}, {0, -h}, {1, 1}, {-1, 1}, {1, -1}, {-1, -1}};
     for (int k = 0; k < 9; ++k) {
         f.pts[16 + k][0] = chk[k][0];
         f.pts[16 + k][1] = chk[k][1];
@@ -153,7 +157,7 @@ __device__ __forceinline__ void source_xy_sm(const double *__restrict__ sm, doub
 
 // Cubic fit of the pixel map over one square region: 16 Chebyshev nodes -> tensor-product
 // cubic in (s, t) in [-1, 1]^2 (separably: along s within each node row, then along t),
-// then VERIFIED against the exact map at 9 other points (centre, T4 extrema, corners).
+// then VERIFIED against the exact map at 9 other points (centre, T4 extrema on the axes, corners).
 // uvf(k) returns the target-side (U, V) of sample point k. C[4q + p] = coefficient of s^p t^q.
 template <int N, class UVF>
 __device__ __forceinline__ bool fit_cubic(const double *__restrict__ sm, const FitConsts &fc, UVF uvf,

@@ -289,6 +289,17 @@ def test_two_level_setup_fallback(P):
         else:
             assert st["tiles_exact"] == 0 and st["tiles_fast"] > 200
             assert d < 5e-6                   # 1.3e-5 if the parent cubic had been accepted
+    # u^4 - v^4 in ONE coordinate: the two fourth-order errors cancel wherever |s| and |t| are
+    # both 0, 1/sqrt(2) or 1 (centre, diagonal, corners), so the check points must also sample
+    # the axes or the 64x64 fit would be accepted with a 2.6e-5 px error
+    tgt = S.make_wcs(512, 512, 150.0005, 2.0003, 0.7, S.PIXSCALE)
+    tgt.a_order = tgt.b_order = 4
+    tgt.a[4][0], tgt.a[0][4] = 1e-10, -1e-10
+    xf, yf = P.dfr_src_coords([src], tgt, (512, 512), (512, 512), 1, path=P.PATH_AUTO)
+    xe, ye = P.dfr_src_coords([src], tgt, (512, 512), (512, 512), 1, path=P.PATH_EXACT)
+    d = max(torch.nan_to_num(xf - xe).abs().max().item(), torch.nan_to_num(yf - ye).abs().max().item())
+    print("u^4 - v^4: tiled vs exact", d)
+    assert d < 6e-6
 
 
 def test_random_geometries_tiled_vs_exact(P):
