@@ -414,6 +414,7 @@ struct TiledParams {
     int n, e0, sny, snx, ony, onx;                 // e0: first exposure of this launch
     int tiles_x, tiles_y, ctas_x, ctas_y;
     int BW, BH;                                    // staged box (STAGE) in source pixels
+    int prefetch_dist;                             // L2 prefetch distance in CTA tiles (0: off)
     int stage_bytes, rec_off;                      // stack kernel: bytes per stage, offset of its records
 };
 
@@ -868,6 +869,21 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
                 "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
                 ::"r"(dst), "l"(&tmap), "r"(ox), "r"(oy), "r"(e), "r"(bar) : "memory");
         }
+        // L2 prefetch of the box of the CTA tile that will be scheduled about one wave from now
+        // (blocks are issued in linear order), so that its own TMA load finds the lines in L2
+        if (threadIdx.x == 0 && P.prefetch_dist > 0) {
+            const long long ctas = (long long)P.ctas_x * P.ctas_y;
+            const long long lin = ((long long)blockIdx.z * P.ctas_y + blockIdx.y) * P.ctas_x + blockIdx.x + P.prefetch_dist;
+            if (lin < ctas * (long long)gridDim.z) {
+                const int2 cf = __ldg(P.cta_box + (size_t)P.e0 * ctas + lin);
+                if (cf.x != kNoBox) {
+                    const int fx = (cf.x - (Taps<ORDER>::lo + 1)) & ~3, fy = cf.y - (Taps<ORDER>::lo + 1);
+                    const int fe = P.e0 + (int)(lin / ctas);
+                    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];"
+                                 ::"l"(&tmap), "r"(fx), "r"(fy), "r"(fe) : "memory");
+                }
+            }
+        }
     }
 
     int flag = TILE_EMPTY, ix0 = 0, iy0 = 0, bx0 = 0, by0 = 0, bx1 = 0, by1 = 0, deg = 3;
@@ -1259,6 +1275,15 @@ static cudaError_t launch_main(const TiledParams &P, const TargetDev &tgt, const
     }
     if (P.ctas_y > 65535) return cudaErrorInvalidConfiguration;
     TiledParams Q = P;
+    if (STAGE) {
+        int dev = 0, sms = 0, per_sm = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess &&
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 32 * CTA_T * CTA_T, smem) == cudaSuccess)
+            Q.prefetch_dist = sms * per_sm / 2;     // measured on B200, C2: flat optimum between 1/2 and 3/4 of a wave
+        static const char *pd = std::getenv("DFR_PREFETCH");      // A-B timing only
+        if (pd) Q.prefetch_dist = std::atoi(pd);
+    }
     for (int e0 = 0; e0 < P.n; e0 += 65535) {
         Q.e0 = e0;
         const dim3 grid((unsigned)P.ctas_x, (unsigned)P.ctas_y, (unsigned)std::min(P.n - e0, 65535));
