@@ -42,7 +42,7 @@ BATCH, NPIX = 32, 2048
 FALLBACK_HBM_GBS = 6650.0          # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum of one tiled_reproject_kernel launch on this
 # workload, from the `ncu --set full` capture summarised in profiles/ (cannot be measured live)
-NCU_TRAFFIC_BYTES = 537.03e6 + 492.01e6
+NCU_TRAFFIC_BYTES = 536.94e6 + 493.84e6
 NCU_TRAFFIC_SOURCE = "profiles/r01_main_kernel_ncu.md"
 
 
