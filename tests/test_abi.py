@@ -83,6 +83,30 @@ def test_validation_errors_without_gpu(P):
     assert L.dfr_pix2world(C.byref(good), None, fake_src, 5, fake_out, fake_out, None) == -1
 
 
+def test_stack_validation_errors_without_gpu(P):
+    L = P.lib()
+    w = S.make_wcs(8, 8, 1.0, 2.0, 0.0, S.PIXSCALE)
+    good = P.pack_wcs(w)
+    arr = (P.DfrWCS * 2)(good, good)
+    src, a, b = C.c_void_p(0x10000), C.c_void_p(0x90000), C.c_void_p(0xA0000)
+    wts = (C.c_float * 2)(1.0, 2.0)
+
+    def call(src=src, n=2, order=1, weights=wts, s=a, c=b, tw=good):
+        return L.dfr_reproject_stack(src, n, 8, 8, arr, C.byref(tw), 8, 8, order, weights, s, c, 0, None)
+
+    assert call(src=None) == -1 and call(s=None) == -1 and call(c=None) == -1   # DFR_ERR_NULL
+    assert call(n=0) == -2 and call(order=2) == -3
+    assert call(s=C.c_void_p(0x10000 + 16)) == -7 and call(c=a) == -7            # overlap src / each other
+    assert call(weights=(C.c_float * 2)(1.0, float("inf"))) == -6                # non-finite weight
+    assert b"weights[1]" in L.dfr_last_error()
+    # host-buffer form and finalize
+    assert L.dfr_stack_host(None, 2, 8, 8, arr, C.byref(good), 8, 8, 1, None, a, b, 2) == -1
+    assert L.dfr_stack_host(src, 2, 8, 8, arr, C.byref(good), 8, 8, 5, None, a, b, 2) == -3
+    assert L.dfr_stack_finalize(a, b, -1, a, None) == -2
+    assert L.dfr_stack_finalize(None, b, 4, a, None) == -1
+    assert L.dfr_stack_finalize(None, None, 0, None, None) == 0                  # zero pixels is legal
+
+
 def test_pc_cdelt_helper(P):
     s = P.pack_wcs(S.make_wcs(8, 8, 1.0, 2.0, 0.0, S.PIXSCALE))
     P.dfr_wcs_set_pc_cdelt(s, [0.6, -0.8, 0.8, 0.6], [-2.0, 3.0])
