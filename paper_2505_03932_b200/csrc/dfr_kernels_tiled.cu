@@ -1332,6 +1332,7 @@ static cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, cons
         const dim3 grid(bx, (unsigned)std::min(n - e0, 65535));
         if (maxo == 0) err = launch_pdl(tile_setup_kernel<0>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
         else if (maxo <= 3) err = launch_pdl(tile_setup_kernel<3>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
+        else if (maxo <= 4) err = launch_pdl(tile_setup_kernel<4>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
         else if (maxo <= 5) err = launch_pdl(tile_setup_kernel<5>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
         else err = launch_pdl(tile_setup_kernel<9>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
         if (err != cudaSuccess) return err;
