@@ -99,6 +99,7 @@ def _split(hdu):
 
 
 def _gather(source_hdus):
+    """-> (single, [float32 2-D arrays], [DfrWCS])."""
     single = not isinstance(source_hdus, (list, tuple)) or (
         len(source_hdus) == 2 and not isinstance(source_hdus[0], (list, tuple)) and not hasattr(source_hdus[0], "header")
         and hasattr(source_hdus[0], "shape"))
@@ -111,9 +112,15 @@ def _gather(source_hdus):
             raise ValueError("source images must be 2-D")
         arrays.append(a)
         wcs.append(_as_wcs(hdr, a.shape))
-    if len({a.shape for a in arrays}) != 1:
-        raise ValueError("all source images of one call must have the same shape")
-    return single, np.stack(arrays), wcs
+    return single, arrays, wcs
+
+
+def _groups(arrays):
+    """Indices of the sources grouped by image shape (one library call per shape)."""
+    by_shape = {}
+    for k, a in enumerate(arrays):
+        by_shape.setdefault(a.shape, []).append(k)
+    return list(by_shape.values())
 
 
 def calculate_reprojection(source_hdus, target_wcs, shape_out=None, order="bilinear", device="cuda",
@@ -124,10 +131,17 @@ def calculate_reprojection(source_hdus, target_wcs, shape_out=None, order="bilin
     'bilinear', 'bicubic'. Returns [ny][nx] for one source, [n][ny][nx] for a list; pixels
     outside a source's footprint are NaN."""
     import torch
-    single, images, wcs = _gather(source_hdus)
-    shape_out = tuple(images.shape[1:]) if shape_out is None else (int(shape_out[0]), int(shape_out[1]))
+    single, arrays, wcs = _gather(source_hdus)
+    shape_out = tuple(arrays[0].shape) if shape_out is None else (int(shape_out[0]), int(shape_out[1]))
     tgt = _as_wcs(target_wcs, shape_out)
-    out = dfr_reproject(torch.from_numpy(images).to(device), wcs, tgt, shape_out, order)
+    out = torch.empty((len(arrays),) + shape_out, dtype=torch.float32, device=device)
+    for idx in _groups(arrays):                     # sources may differ in shape (PAPER.md:32)
+        src = torch.from_numpy(np.stack([arrays[k] for k in idx])).to(device)
+        res = dfr_reproject(src, [wcs[k] for k in idx], tgt, shape_out, order)
+        if len(idx) == len(arrays):
+            out = res
+        else:
+            out[torch.as_tensor(idx, device=device)] = res
     if single:
         out = out[0]
     return out if return_torch else out.cpu().numpy()
@@ -138,9 +152,15 @@ def calculate_stack(source_hdus, target_wcs, shape_out=None, order="bilinear", w
     """The co-added mean of the sources on the target grid and its weight map (the stated
     purpose of reprojection): (mean, wsum), NaN where no source covers a pixel."""
     import torch
-    _, images, wcs = _gather(source_hdus)
-    shape_out = tuple(images.shape[1:]) if shape_out is None else (int(shape_out[0]), int(shape_out[1]))
+    _, arrays, wcs = _gather(source_hdus)
+    shape_out = tuple(arrays[0].shape) if shape_out is None else (int(shape_out[0]), int(shape_out[1]))
     tgt = _as_wcs(target_wcs, shape_out)
-    s, w = dfr_reproject_stack(torch.from_numpy(images).to(device), wcs, tgt, shape_out, order, weights=weights)
+    weights = None if weights is None else np.asarray(weights, dtype=np.float32)
+    s = w = None
+    for idx in _groups(arrays):                     # one fused call per source shape, accumulated
+        src = torch.from_numpy(np.stack([arrays[k] for k in idx])).to(device)
+        s, w = dfr_reproject_stack(src, [wcs[k] for k in idx], tgt, shape_out, order,
+                                   weights=None if weights is None else weights[idx],
+                                   sum=s, wsum=w, accumulate=s is not None)
     mean = dfr_stack_finalize(s, w)
     return (mean, w) if return_torch else (mean.cpu().numpy(), w.cpu().numpy())

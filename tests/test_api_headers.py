@@ -112,6 +112,18 @@ def test_calculate_reprojection_against_oracle(A):
     xo, yo = oracle.src_coords(tgt, srcs[0], 240, 320)
     ref = oracle.interp(imgs[0], xo.ravel(), yo.ravel(), 1).reshape(240, 320).astype(np.float32)
     PR.check_image(one, ref, xo, yo, imgs[0], 1)
+    # sources of different shapes in one call: grouped by shape inside, order preserved
+    small = imgs[1][:200, :280].copy()
+    ws_small = srcs[1].copy()
+    mixed = A.calculate_reprojection([hdus[0], HDU(small, header_of(ws_small, 280, 200)), hdus[1]],
+                                     header_of(tgt, 300, 260), shape_out=(260, 300))
+    assert mixed.shape == (3, 260, 300)
+    ref_all = A.calculate_reprojection(hdus, header_of(tgt, 300, 260), shape_out=(260, 300))
+    assert np.array_equal(np.nan_to_num(mixed[0], nan=-1), np.nan_to_num(ref_all[0], nan=-1))
+    assert np.array_equal(np.nan_to_num(mixed[2], nan=-1), np.nan_to_num(ref_all[1], nan=-1))
+    xo, yo = oracle.src_coords(tgt, ws_small, 260, 300)
+    ref = oracle.interp(small, xo.ravel(), yo.ravel(), 1).reshape(260, 300).astype(np.float32)
+    PR.check_image(mixed[1], ref, xo, yo, small, 1)
     mean, wsum = A.calculate_stack(hdus, header_of(tgt, 300, 260), shape_out=(260, 300))
     so, wo = oracle.stack(np.stack(imgs), srcs, tgt, (260, 300), 1)
     ok = wo == 2
