@@ -1,0 +1,58 @@
+"""-m gpu: bench.py prints ONE JSON line with the keys the driver's contract names, for the
+headline mode, the stack mode and (CPU only, rank 0) the reference arm."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+BASE_KEYS = {"metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better",
+             "scaling", "vs_baseline", "dtype", "data", "config", "roofline", "cpu_baseline", "e2e", "gpu_launches"}
+
+
+def run(*args, timeout=600):
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), *args], capture_output=True, text=True,
+                         timeout=timeout, cwd=ROOT)
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [l for l in res.stdout.splitlines() if l.strip()]
+    assert len(lines) == 1, lines
+    return json.loads(lines[0])
+
+
+@pytest.mark.gpu
+def test_headline_line():
+    torch = pytest.importorskip("torch")
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    d = run("--steps", "3", "--warmup", "3", "--e2e-steps", "1", "--no-cpu-baseline")
+    assert BASE_KEYS | {"clocks"} <= set(d)
+    assert d["unit"] == "Mpix/s" and d["steps"] == 3 and d["warmup"] >= 3 and d["n_gpus"] == 1
+    assert d["config"]["workload"].startswith("configs[2]") and "model" not in d["config"]
+    r = d["roofline"]
+    assert r["bound"] == "hbm" and 0.3 < r["frac"] < 1.2 and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
+    assert r["traffic"] and 0.8 < r["traffic"] / r["algorithmic_bytes_per_launch"] < 1.2
+    assert d["gpu_launches"] == 3 * d["steps"] and d["value"] > 1e5
+    e = d["e2e"]
+    assert e["h2d_bytes_per_step"] == 32 * 2048 * 2048 * 4 == e["d2h_bytes_per_step"] and e["matches_device_path"]
+    assert 0 < e["value"] < d["value"]
+    assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+
+
+@pytest.mark.gpu
+def test_stack_line():
+    torch = pytest.importorskip("torch")
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    d = run("--mode", "stack", "--steps", "3", "--warmup", "3")
+    assert BASE_KEYS <= set(d) and d["roofline"]["kernel"] == "tiled_stack_kernel"
+    assert 20.0 < d["config"]["depth_mean"] <= 32.0
+
+
+def test_reference_arm_line():
+    """The oracle arm runs on the host cores (no GPU): a bounded sample per step."""
+    d = run("--impl", "reference", "--steps", "1", "--warmup", "0", timeout=900)
+    assert d["impl"] == "reference" and BASE_KEYS - {"roofline"} <= set(d)      # no kernel, no roofline
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
+    assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["value"] == d["value"] and d["gpu_launches"] == 0
