@@ -57,6 +57,8 @@ def lib():
         _lib.orc_src_coords.argtypes = [wp, wp, C.c_int32, C.c_int32, dp, dp]
         _lib.orc_interp.argtypes = [fp, C.c_int32, C.c_int32, dp, dp, C.c_int64, C.c_int32,
                                     C.c_double, dp]
+        _lib.orc_interp_paper.argtypes = [fp, C.c_int32, C.c_int32, dp, dp, C.c_int64, C.c_int32, dp, dp]
+        _lib.orc_interp_paper.restype = C.c_int
         _lib.orc_reproject.argtypes = [fp, C.c_int32, C.c_int32, C.c_int32, wp, wp,
                                        C.c_int32, C.c_int32, C.c_int32, fp]
         _lib.orc_reproject.restype = C.c_int
@@ -126,6 +128,21 @@ def interp(src, x, y, order, a=KEYS_A):
     lib().orc_interp(src.ctypes.data_as(C.POINTER(C.c_float)), src.shape[0], src.shape[1],
                      xp, yp, x.size, int(order), float(a), _d(val)[1])
     return val
+
+
+def interp_paper(src, x, y, order):
+    """orc_interp_paper: (val, footprint) under the paper's literal normalisation (G19)."""
+    src = np.ascontiguousarray(src, dtype=np.float32)
+    assert src.ndim == 2
+    x, xp = _d(x)
+    y, yp = _d(y)
+    val = np.empty(x.shape, dtype=np.float64)
+    foot = np.empty(x.shape, dtype=np.float64)
+    rc = lib().orc_interp_paper(src.ctypes.data_as(C.POINTER(C.c_float)), src.shape[0], src.shape[1],
+                                xp, yp, x.size, int(order), _d(val)[1], _d(foot)[1])
+    if rc != 0:
+        raise ValueError("orc_interp_paper: defined for nearest and bilinear only")
+    return val, foot
 
 
 def reproject(images, src_wcs, tgt_wcs, shape_out, order):

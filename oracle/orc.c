@@ -206,6 +206,38 @@ void orc_interp(const float *src, int32_t ny, int32_t nx, const double *x, const
         val[k] = interp_one(src, ny, nx, x[k], y[k], order, a);
 }
 
+int orc_interp_paper(const float *src, int32_t ny, int32_t nx, const double *x, const double *y,
+                     int64_t n, int32_t order, double *val, double *foot)
+{
+    if (order != ORC_NEAREST && order != ORC_BILINEAR) return -1;
+    for (int64_t k = 0; k < n; ++k) {
+        double num = 0.0, den = 0.0;
+        if (x[k] == x[k] && y[k] == y[k]) {
+            if (order == ORC_NEAREST) {
+                const double rx = rint(x[k]), ry = rint(y[k]);      /* half-even (G8) */
+                if (rx >= 0.0 && rx <= nx - 1.0 && ry >= 0.0 && ry <= ny - 1.0) {
+                    num = (double)src[(size_t)ry * (size_t)nx + (size_t)rx];
+                    den = 1.0;
+                }
+            } else {
+                const double fx0 = floor(x[k]), fy0 = floor(y[k]);
+                const double fx = x[k] - fx0, fy = y[k] - fy0;
+                for (int m = 0; m < 2; ++m)
+                    for (int l = 0; l < 2; ++l) {
+                        const double ix = fx0 + l, iy = fy0 + m;
+                        if (ix < 0.0 || ix > nx - 1.0 || iy < 0.0 || iy > ny - 1.0) continue;   /* zero padding */
+                        const double w = (l ? fx : 1.0 - fx) * (m ? fy : 1.0 - fy);
+                        num += w * (double)src[(size_t)iy * (size_t)nx + (size_t)ix];
+                        den += w;
+                    }
+            }
+        }
+        val[k] = den > 0.0 ? num / den : NAN;
+        if (foot) foot[k] = den;
+    }
+    return 0;
+}
+
 int orc_reproject(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
                   const orc_wcs *src_wcs, const orc_wcs *tgt_wcs,
                   int32_t out_ny, int32_t out_nx, int32_t order, float *out)

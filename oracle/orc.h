@@ -58,6 +58,17 @@ void orc_src_coords(const orc_wcs *tgt, const orc_wcs *src, int32_t out_ny, int3
 void orc_interp(const float *src, int32_t ny, int32_t nx, const double *x, const double *y,
                 int64_t n, int32_t order, double a, double *val);
 
+/* The paper's literal footprint normalisation ("simultaneously projecting an
+ * identity tensor called the footprint. The final reprojected frame is normalized by this
+ * footprint"; reading G19 of DESIGN.md): the image AND an all-ones image
+ * are interpolated with ZERO padding (a tap outside the image contributes nothing to
+ * either), val = interp(image) / interp(ones) where interp(ones) > 0, NaN elsewhere.
+ * Defined for nearest and bilinear (order 0, 1); for bicubic the projected identity
+ * changes sign near the rim, so the ratio is not a footprint: returns -1.
+ * foot (optional) receives interp(ones). Pins: tests/test_oracle_interp.py (F1-F4). */
+int orc_interp_paper(const float *src, int32_t ny, int32_t nx, const double *x, const double *y,
+                     int64_t n, int32_t order, double *val, double *foot);
+
 /* O1-O13, the whole path: out[e][j][i] float32. Returns 0, or -1 on a bad order. */
 int orc_reproject(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
                   const orc_wcs *src_wcs, const orc_wcs *tgt_wcs,

@@ -243,3 +243,68 @@ def test_batch_uses_per_exposure_wcs(small):
     assert np.array_equal(out[0], img)
     assert np.array_equal(out[1][:, :-2], img[::-1][:, 2:])       # x_s = i + 2
     assert np.isnan(out[1][:, -2:]).all()
+
+
+# ------------------------------------------------- F1-F4: the paper's literal normalisation (G19)
+def test_f1_paper_mode_equals_area_rule_inside_and_extends_half_a_pixel():
+    """Bilinear: footprint > 0 exactly on (-1, n) x (-1, n); wherever the area rule is valid
+    the two values agree (this is G6); in the extra half-pixel band the value is the edge
+    replication the area rule would have produced had it been valid."""
+    rng = np.random.default_rng(70)
+    img = rng.normal(100, 20, (9, 13)).astype(np.float32)
+    x = rng.uniform(-2.0, 14.0, 20000)
+    y = rng.uniform(-2.0, 10.0, 20000)
+    val, foot = oracle.interp_paper(img, x, y, 1)
+    inside = (x > -1) & (x < 13) & (y > -1) & (y < 9)
+    assert np.array_equal(foot > 0, inside) and np.array_equal(~np.isnan(val), inside)
+    area = oracle.interp(img, x, y, 1)
+    ok = ~np.isnan(area)
+    assert ok.sum() > 5000 and np.abs(val[ok] - area[ok]).max() < 1e-10
+    band = inside & ~ok
+    xc, yc = np.clip(x[band], 0, 12), np.clip(y[band], 0, 8)
+    assert band.sum() > 500 and np.abs(val[band] - oracle.interp(img, xc, yc, 1)).max() < 1e-10
+
+
+def test_f2_paper_mode_hand_values():
+    img = np.arange(16, dtype=np.float32).reshape(4, 4)
+    x = np.array([-0.75, 3.9, 1.5, -1.0, 4.0, 0.25])
+    y = np.array([2.0, -0.5, 3.999, 1.0, 1.0, 0.5])
+    val, foot = oracle.interp_paper(img, x, y, 1)
+    assert val[0] == 8.0 and abs(foot[0] - 0.25) < 1e-15            # only the tap (0, 2), weight 1/4
+    assert abs(val[1] - 3.0) < 1e-12 and abs(foot[1] - 0.05) < 1e-12  # only (3, 0): 0.1 x 0.5
+    assert abs(val[2] - 13.5) < 1e-12                                # bottom row only: mean of 13, 14
+    assert np.isnan(val[3]) and np.isnan(val[4]) and foot[3] == 0.0  # x = -1 and x = n: nothing in bounds
+    assert abs(val[5] - (0.25 + 0.5 * 4.0)) < 1e-12 and abs(foot[5] - 1.0) < 1e-15
+
+
+def test_f3_paper_mode_is_zero_padded_grid_sample_ratio():
+    """Library routine: torch-CPU float64 grid_sample(padding_mode='zeros', align_corners=True)
+    of the image and of ones; their ratio is the paper's normalised frame."""
+    torch = pytest.importorskip("torch")
+    rng = np.random.default_rng(71)
+    ny, nx = 11, 17
+    img = rng.normal(0, 1, (ny, nx)).astype(np.float32)
+    x = rng.uniform(-1.5, nx + 0.5, 5000)
+    y = rng.uniform(-1.5, ny + 0.5, 5000)
+    g = torch.from_numpy(np.stack([2 * x / (nx - 1) - 1, 2 * y / (ny - 1) - 1], -1))[None, None]
+    for order, mode in ((1, "bilinear"), (0, "nearest")):
+        t = torch.from_numpy(img.astype(np.float64))[None, None]
+        num = torch.nn.functional.grid_sample(t, g, mode=mode, padding_mode="zeros", align_corners=True)[0, 0, 0].numpy()
+        den = torch.nn.functional.grid_sample(torch.ones_like(t), g, mode=mode, padding_mode="zeros", align_corners=True)[0, 0, 0].numpy()
+        val, foot = oracle.interp_paper(img, x, y, order)
+        tie = (np.abs(x - np.floor(x) - 0.5) < 1e-9) | (np.abs(y - np.floor(y) - 0.5) < 1e-9)
+        keep = ~tie if order == 0 else np.ones_like(tie)
+        assert np.abs(foot[keep] - den[keep]).max() < 1e-12
+        pos = keep & (den > 1e-9)
+        assert np.abs(val[pos] - num[pos] / den[pos]).max() < 1e-9
+
+
+def test_f4_paper_mode_rejects_bicubic_and_nearest_matches_area_rule():
+    img = np.arange(30, dtype=np.float32).reshape(5, 6)
+    with pytest.raises(ValueError):
+        oracle.interp_paper(img, np.zeros(1), np.zeros(1), 3)
+    rng = np.random.default_rng(72)
+    x, y = rng.uniform(-1.5, 7.0, 5000), rng.uniform(-1.5, 6.0, 5000)
+    val, _ = oracle.interp_paper(img, x, y, 0)
+    area = oracle.interp(img, x, y, 0)
+    assert np.array_equal(np.isnan(val), np.isnan(area)) and np.array_equal(np.nan_to_num(val), np.nan_to_num(area))
