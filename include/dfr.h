@@ -88,6 +88,17 @@ typedef enum dfr_status {
  *   TILED : as AUTO (kept distinct so tests can assert the fast path ran). */
 enum { DFR_PATH_AUTO = 0, DFR_PATH_EXACT = 1, DFR_PATH_TILED = 2 };
 
+/* Footprint rule of dfr_reproject_edge.
+ *   AREA  : a pixel is valid where its source coordinate lies in the union of the source
+ *           pixel areas, -0.5 <= x < n - 0.5 (what every other entry point uses).
+ *   PAPER : the paper's literal rule: the image and an identity ("footprint")
+ *           image are interpolated with zero padding and divided; for bilinear this is
+ *           valid on the open square -1 < x < n and equals the AREA result wherever both
+ *           are valid (the half-pixel band it adds takes the edge pixel's value). Nearest:
+ *           identical to AREA. Bicubic: not defined (the projected identity changes sign
+ *           near the rim) -> DFR_ERR_ORDER. */
+enum { DFR_EDGE_AREA = 0, DFR_EDGE_PAPER = 1 };
+
 /* ---- the hot path (calculate_reprojection) -------------- */
 
 /* Reproject n source exposures onto one target grid.
@@ -103,6 +114,12 @@ int dfr_reproject(const float *src_batch, int32_t n, int32_t src_ny, int32_t src
                   const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
                   int32_t out_ny, int32_t out_nx, int32_t order,
                   float *out, void *stream);
+
+/* Same, with an explicit footprint rule (DFR_EDGE_*). */
+int dfr_reproject_edge(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+                       const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                       int32_t out_ny, int32_t out_nx, int32_t order, int32_t edge_mode,
+                       float *out, void *stream);
 
 /* Same, with an explicit path (DFR_PATH_*). */
 int dfr_reproject_ex(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,

@@ -17,9 +17,10 @@ _SO = os.path.join(_PKG, "libdfr.so")
 
 NEAREST, BILINEAR, BICUBIC = 0, 1, 3
 PATH_AUTO, PATH_EXACT, PATH_TILED = 0, 1, 2
+EDGE_AREA, EDGE_PAPER = 0, 1
 _ORDER_NAMES = {"nearest": 0, "nearest-neighbor": 0, "bilinear": 1, "bicubic": 3}
 
-EXPORTS = ["dfr_reproject", "dfr_reproject_ex", "dfr_reproject_host", "dfr_reproject_stack",
+EXPORTS = ["dfr_reproject", "dfr_reproject_edge", "dfr_reproject_ex", "dfr_reproject_host", "dfr_reproject_stack",
            "dfr_stack_finalize", "dfr_stack_host", "dfr_pix2world",
            "dfr_world2pix", "dfr_src_coords", "dfr_wcs_set_pc_cdelt", "dfr_wcs_fit_inverse_sip", "dfr_last_stats",
            "dfr_profile_enable", "dfr_profile_last",
@@ -56,6 +57,7 @@ def lib():
         i32, i64 = C.c_int32, C.c_int64
         L.dfr_reproject.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, vp]
         L.dfr_reproject_ex.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, vp, i32]
+        L.dfr_reproject_edge.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, i32, fp, vp]
         L.dfr_reproject_host.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, i32]
         L.dfr_reproject_stack.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32,
                                           C.POINTER(C.c_float), fp, fp, i32, vp]
@@ -129,7 +131,7 @@ def _need_cuda(t, dtype, name):
 
 
 def dfr_reproject(src_batch, src_wcs, tgt_wcs, shape_out=None, order=BILINEAR, out=None,
-                  stream=None, path=PATH_AUTO):
+                  stream=None, path=PATH_AUTO, edge=EDGE_AREA):
     """dfr_reproject / dfr_reproject_ex (include/dfr.h). src_batch: CUDA float32
     [n][ny][nx] (or [ny][nx]); returns the CUDA float32 [n][out_ny][out_nx] output.
     shape_out defaults to the input shape."""
@@ -149,8 +151,14 @@ def dfr_reproject(src_batch, src_wcs, tgt_wcs, shape_out=None, order=BILINEAR, o
     if tuple(out.shape) != (n, ony, onx):
         raise ValueError("out has the wrong shape")
     with torch.cuda.device(src_batch.device):
-        _check(lib().dfr_reproject_ex(src_batch.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx,
-                                      _order(order), out.data_ptr(), _stream_ptr(stream), int(path)))
+        if edge != EDGE_AREA:
+            if path != PATH_AUTO:
+                raise ValueError("an explicit path and an explicit edge rule cannot be combined")
+            _check(lib().dfr_reproject_edge(src_batch.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx,
+                                            _order(order), int(edge), out.data_ptr(), _stream_ptr(stream)))
+        else:
+            _check(lib().dfr_reproject_ex(src_batch.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx,
+                                          _order(order), out.data_ptr(), _stream_ptr(stream), int(path)))
     return out
 
 

@@ -134,7 +134,7 @@ static int upload_sources(int32_t n, const dfr_wcs *sw, const dfr_wcs *tw, cudaS
 
 static int reproject_impl(const float *src, int32_t n, int32_t sny, int32_t snx,
                           const dfr_wcs *sw, const dfr_wcs *tw, int32_t ony, int32_t onx,
-                          int32_t order, float *out, cudaStream_t st, int32_t path)
+                          int32_t order, float *out, cudaStream_t st, int32_t path, int32_t edge = DFR_EDGE_AREA)
 {
     std::call_once(g_pool_once, tune_pool);
     g_last.pending = false;
@@ -148,7 +148,7 @@ static int reproject_impl(const float *src, int32_t n, int32_t sny, int32_t snx,
     TiledStats ts = {0, 0, 0, 0};
     if (path == DFR_PATH_EXACT) {
         if (g_last.prof.enabled) cudaEventRecord(g_last.prof.setup_begin, st), cudaEventRecord(g_last.prof.main_begin, st);
-        err = launch_exact_reproject(src, n, sny, snx, tgt, dsrc, ony, onx, order, out, st);
+        err = launch_exact_reproject(src, n, sny, snx, tgt, dsrc, ony, onx, order, out, st, edge);
         if (g_last.prof.enabled) cudaEventRecord(g_last.prof.main_end, st);
         g_last.kernels = 1;
         g_last.tiled = false;
@@ -157,7 +157,7 @@ static int reproject_impl(const float *src, int32_t n, int32_t sny, int32_t snx,
         if (err == cudaSuccess)
             err = launch_tiled_reproject(src, n, sny, snx, tgt, dsrc, hsrc.data(), ony, onx, order, out, st,
                                          g_accumulate ? g_stream_totals : g_last.pinned_dev, g_accumulate ? 1 : 0,
-                                         &ts, &g_last.prof);
+                                         &ts, &g_last.prof, edge);
         if (g_accumulate) {
             g_stats_acc[3] += ts.kernels;
         } else {
@@ -195,6 +195,31 @@ int dfr_reproject_ex(const float *src_batch, int32_t n, int32_t src_ny, int32_t 
     if (o0 < s1 && s0 < o1) { set_error("out overlaps src_batch"); return DFR_ERR_ALIAS; }
     return reproject_impl(src_batch, n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order,
                           out, (cudaStream_t)stream, path);
+}
+
+int dfr_reproject_edge(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+                       const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                       int32_t out_ny, int32_t out_nx, int32_t order, int32_t edge_mode,
+                       float *out, void *stream)
+{
+    if (!src_batch || !out) { set_error("NULL image pointer"); return DFR_ERR_NULL; }
+    int rc = check_common(n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order);
+    if (rc != DFR_OK) return rc;
+    if (edge_mode != DFR_EDGE_AREA && edge_mode != DFR_EDGE_PAPER) {
+        set_error("unknown edge mode %d", edge_mode);
+        return DFR_ERR_ORDER;
+    }
+    if (edge_mode == DFR_EDGE_PAPER && order == DFR_BICUBIC) {
+        set_error("the paper's footprint normalisation is not defined for bicubic interpolation");
+        return DFR_ERR_ORDER;
+    }
+    const char *s0 = (const char *)src_batch, *s1 = s0 + sizeof(float) * (size_t)n * src_ny * src_nx;
+    const char *o0 = (const char *)out, *o1 = o0 + sizeof(float) * (size_t)n * out_ny * out_nx;
+    if (o0 < s1 && s0 < o1) { set_error("out overlaps src_batch"); return DFR_ERR_ALIAS; }
+    // nearest: the zero-padded identity is 1 exactly on the area footprint
+    const int32_t edge = (order == DFR_NEAREST) ? DFR_EDGE_AREA : edge_mode;
+    return reproject_impl(src_batch, n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order,
+                          out, (cudaStream_t)stream, DFR_PATH_AUTO, edge);
 }
 
 int dfr_reproject(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,

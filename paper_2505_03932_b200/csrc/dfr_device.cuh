@@ -90,9 +90,13 @@ __host__ __device__ __forceinline__ void source_xy(const SourceDev &s, double U,
 
 __device__ __forceinline__ float qnanf() { return __int_as_float(0x7fc00000); }
 
-// a7: footprint = union of source pixel areas, half-open (G6).
-__device__ __forceinline__ bool in_footprint(double x, double y, int ny, int nx)
+// a7: footprint. edge = DFR_EDGE_AREA: union of source pixel areas, half-open (G6);
+// edge = DFR_EDGE_PAPER: where the paper's zero-padded projected identity is positive for
+// bilinear interpolation, the open square (-1, n) x (-1, n) (G19). Taps are
+// edge-replicated under both, which for the second IS the ratio image / identity.
+__device__ __forceinline__ bool in_footprint(double x, double y, int ny, int nx, int edge = DFR_EDGE_AREA)
 {
+    if (edge == DFR_EDGE_PAPER) return (x > -1.0) && (x < (double)nx) && (y > -1.0) && (y < (double)ny);
     return (x >= -0.5) && (x < (double)nx - 0.5) && (y >= -0.5) && (y < (double)ny - 0.5);
 }
 

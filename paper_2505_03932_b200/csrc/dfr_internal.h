@@ -57,7 +57,8 @@ int  cuda_fail(cudaError_t e, const char *what);            // records text, ret
 // exact per-pixel path
 cudaError_t launch_exact_reproject(const float *src, int n, int sny, int snx,
                                    const TargetDev &tgt, const SourceDev *srcdev,
-                                   int ony, int onx, int order, float *out, cudaStream_t st);
+                                   int ony, int onx, int order, float *out, cudaStream_t st,
+                                   int edge = DFR_EDGE_AREA);
 cudaError_t launch_exact_coords(int n, const TargetDev &tgt, const SourceDev *srcdev,
                                 int ony, int onx, double *x, double *y, cudaStream_t st);
 // literal sky kernels

@@ -435,23 +435,23 @@ __device__ __forceinline__ void axis_range(int n, int o, int B, int &A_lo, int &
 
 // Slow pixel of a FAST tile: polynomial coordinate, rim/out-of-box handling by the exact
 // footprint rule and edge-replicated global gathers.
-template <int ORDER>
+template <int ORDER, int EDGE>
 __device__ __noinline__ float slow_poly_pixel(const float *__restrict__ img, int sny, int snx,
                                               int ix0, int iy0, float xl, float yl)
 {
     const double x = (double)ix0 + (double)xl, y = (double)iy0 + (double)yl;
-    if (!in_footprint(x, y, sny, snx)) return qnanf();
+    if (!in_footprint(x, y, sny, snx, EDGE)) return qnanf();
     return sample_global<ORDER>(img, sny, snx, x, y);
 }
 
-template <int ORDER>
+template <int ORDER, int EDGE>
 __device__ __noinline__ float exact_pixel(const float *__restrict__ img, int sny, int snx,
                                           const TargetDev &tgt, const SourceDev &s, int i, int j)
 {
     double U, V, x, y;
     target_uv(tgt, (double)i, (double)j, U, V);
     source_xy(s, U, V, x, y);
-    if (!in_footprint(x, y, sny, snx)) return qnanf();
+    if (!in_footprint(x, y, sny, snx, EDGE)) return qnanf();
     return sample_global<ORDER>(img, sny, snx, x, y);
 }
 
@@ -726,7 +726,7 @@ struct TileHead {
     int flag, ix0, iy0, bx0, by0, bx1, by1, deg;
 };
 
-template <int ORDER, bool STAGE, class Sink>
+template <int ORDER, bool STAGE, int EDGE = DFR_EDGE_AREA, class Sink>
 __device__ __forceinline__ void warp_tile(const TiledParams &P, const TargetDev &tgt, int e, int ttx, int tty,
                                           int lane, const TileHead &H, float (&X)[4], float (&Y)[4],
                                           uint32_t box_smem, int ox, int oy, Sink &sink)
@@ -745,7 +745,7 @@ __device__ __forceinline__ void warp_tile(const TiledParams &P, const TargetDev 
     }
     if (flag == TILE_EXACT) {
         for (int r = 0; r < rows; ++r)
-            sink.row1(exact_pixel<ORDER>(img, P.sny, P.snx, tgt, P.srcdev[e], col, ty0 + r));
+            sink.row1(exact_pixel<ORDER, EDGE>(img, P.sny, P.snx, tgt, P.srcdev[e], col, ty0 + r));
         return;
     }
 
@@ -812,7 +812,7 @@ __device__ __forceinline__ void warp_tile(const TiledParams &P, const TargetDev 
         if (!all_ok) {                        // rare: image rim, outside the staged box, NaN
 #pragma unroll
             for (int k = 0; k < U; ++k)
-                if (!ok[k]) val[k] = slow_poly_pixel<ORDER>(img, P.sny, P.snx, ix0, iy0, xl[k], yl[k]);
+                if (!ok[k]) val[k] = slow_poly_pixel<ORDER, EDGE>(img, P.sny, P.snx, ix0, iy0, xl[k], yl[k]);
         }
         sink.rows4(val[0], val[1], val[2], val[3]);
         dj += (float)U;
@@ -822,7 +822,7 @@ __device__ __forceinline__ void warp_tile(const TiledParams &P, const TargetDev 
         const float ys = fmaf(fmaf(fmaf(Y[3], dj, Y[2]), dj, Y[1]), dj, Y[0]);
         bool ok1;
         float v = fast_pixel<ORDER, STAGE>(G, xs, ys, Cx, Cy, cntx, cnty, ok1);
-        if (!ok1) v = slow_poly_pixel<ORDER>(img, P.sny, P.snx, ix0, iy0, xs, ys);
+        if (!ok1) v = slow_poly_pixel<ORDER, EDGE>(img, P.sny, P.snx, ix0, iy0, xs, ys);
         sink.row1(v);
         dj += 1.0f;
     }
@@ -831,7 +831,9 @@ __device__ __forceinline__ void warp_tile(const TiledParams &P, const TargetDev 
 // ---------------------------------------------------------------------------------
 // main kernel: one CTA per 64x64 output tile per exposure, one warp per 32x32 tile
 // ---------------------------------------------------------------------------------
-template <int ORDER, bool STAGE>
+// EDGE (DFR_EDGE_*) is a template parameter so that the default kernel is compiled exactly as
+// without it (a run-time flag cost 3 % through register allocation alone).
+template <int ORDER, bool STAGE, int EDGE = DFR_EDGE_AREA>
 __global__ void __launch_bounds__(32 * CTA_T * CTA_T, 8)
 tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_constant__ TargetDev tgt,
                        const __grid_constant__ CUtensorMap tmap)
@@ -924,7 +926,7 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
     StoreSink sink;
     sink.orow = P.out + ((size_t)e * P.ony + (size_t)tty * TS) * P.onx + (ttx * TS + lane);
     sink.opitch = (size_t)P.onx;
-    warp_tile<ORDER, STAGE>(P, tgt, e, ttx, tty, lane, H, X, Y, smem_u32(box), ox, oy, sink);
+    warp_tile<ORDER, STAGE, EDGE>(P, tgt, e, ttx, tty, lane, H, X, Y, smem_u32(box), ox, oy, sink);
 }
 
 // ---------------------------------------------------------------------------------
@@ -1264,11 +1266,11 @@ static bool probe_extent(const TargetDev &tgt, const SourceDev *hs, int n, int o
     return any;
 }
 
-template <int ORDER, bool STAGE>
+template <int ORDER, bool STAGE, int EDGE = DFR_EDGE_AREA>
 static cudaError_t launch_main(const TiledParams &P, const TargetDev &tgt, const CUtensorMap &tmap,
                                size_t smem, cudaStream_t st)
 {
-    auto kern = tiled_reproject_kernel<ORDER, STAGE>;
+    auto kern = tiled_reproject_kernel<ORDER, STAGE, EDGE>;
     if (STAGE) {      // per device, cheap: set every time
         cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxBoxBytes);
         if (err != cudaSuccess) return err;
@@ -1395,7 +1397,8 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
                                    const TargetDev &tgt, const SourceDev *srcdev,
                                    const SourceDev *srchost,
                                    int ony, int onx, int order, float *out, cudaStream_t st,
-                                   int32_t *host_stats, int stats_add, TiledStats *stats, ProfileEvents *prof)
+                                   int32_t *host_stats, int stats_add, TiledStats *stats, ProfileEvents *prof,
+                                   int edge)
 {
     Prepared R;
     if (prof && prof->enabled) cudaEventRecord(prof->setup_begin, st);
@@ -1406,13 +1409,16 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
 #define DFR_LAUNCH(O)                                                                     \
     err = R.stage ? launch_main<O, true>(R.P, tgt, R.tmap, R.box_bytes, st) : launch_main<O, false>(R.P, tgt, R.tmap, 0, st)
     if (order == DFR_NEAREST) DFR_LAUNCH(DFR_NEAREST);
+    else if (order == DFR_BILINEAR && edge == DFR_EDGE_PAPER)
+        err = R.stage ? launch_main<DFR_BILINEAR, true, DFR_EDGE_PAPER>(R.P, tgt, R.tmap, R.box_bytes, st)
+                      : launch_main<DFR_BILINEAR, false, DFR_EDGE_PAPER>(R.P, tgt, R.tmap, 0, st);
     else if (order == DFR_BILINEAR) DFR_LAUNCH(DFR_BILINEAR);
     else DFR_LAUNCH(DFR_BICUBIC);
 #undef DFR_LAUNCH
     if (prof && prof->enabled) cudaEventRecord(prof->main_end, st);
     free_scratch(R.sc, st);
     stats->kernels = 3;
-    stats->tiles_fast = stats->tiles_exact = stats->tiles_empty = -1;   // filled from host_stats by the caller
+    stats->tiles_fast = stats->tiles_exact = stats->tiles_empty = -1;   // written to host_stats by the setup kernel
     return err;
 }
 

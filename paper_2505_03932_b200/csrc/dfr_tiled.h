@@ -41,7 +41,7 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
                                    int ony, int onx, int order, float *out, cudaStream_t st,
                                    int32_t *host_stats /* 3 ints the setup kernel can write (mapped host or device memory), or NULL */,
                                    int stats_add /* 0: store the totals, 1: atomically add them (streaming) */,
-                                   TiledStats *stats, ProfileEvents *prof);
+                                   TiledStats *stats, ProfileEvents *prof, int edge = DFR_EDGE_AREA);
 // dfr_reproject_stack: sum / wsum accumulated over the n exposures in one kernel.
 cudaError_t launch_tiled_stack(const float *src, int n, int sny, int snx, const TargetDev &tgt,
                                const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx, int order,

@@ -362,3 +362,37 @@ def test_paper_demo_geometry(P, path):
     out = outs[1][0]
     m = 0.25 * (img[:-1, :-1] + img[1:, :-1] + img[:-1, 1:] + img[1:, 1:])
     assert np.nanmax(np.abs(out[1:, 1:] - m)) < 2e-3 * PR.dyn_range(img)
+
+
+def test_paper_footprint_mode(P):
+    """dfr_reproject_edge(DFR_EDGE_PAPER) against orc_interp_paper (reading G19): bilinear
+    keeps the half-pixel band (-1, -0.5) u (n - 0.5, n) the area rule drops, with the edge
+    pixel's value; inside the area footprint the two modes are bit-identical; nearest is the
+    area rule; bicubic is refused. Mask band: |x + 1|, |x - n| < EDGE_BAND."""
+    rng = np.random.default_rng(69)
+    sny, snx, ony, onx = 140, 212, 190, 260
+    img = S.make_image(sny, snx, 40, rng)
+    src = S.add_sip(S.make_wcs(snx, sny, 150.0, 2.0, 0.0, S.PIXSCALE), 3, snx / 2.0, rng, amp=1e-4)
+    tgt = S.make_wcs(onx, ony, 150.0004, 2.0003, 11.0, S.PIXSCALE * 0.93)
+    d = torch.from_numpy(img[None]).cuda()
+    area = P.dfr_reproject(d, [src], tgt, (ony, onx), 1).cpu().numpy()[0]
+    paper = P.dfr_reproject(d, [src], tgt, (ony, onx), 1, edge=P.EDGE_PAPER).cpu().numpy()[0]
+    xo, yo = oracle.src_coords(tgt, src, ony, onx)
+    ref, foot = oracle.interp_paper(img, xo.ravel(), yo.ravel(), 1)
+    ref, foot = ref.reshape(ony, onx), foot.reshape(ony, onx)
+    near = ((np.abs(xo + 1) < PR.EDGE_BAND) | (np.abs(xo - snx) < PR.EDGE_BAND)
+            | (np.abs(yo + 1) < PR.EDGE_BAND) | (np.abs(yo - sny) < PR.EDGE_BAND))
+    mg, mo = np.isnan(paper), np.isnan(ref)
+    assert not ((mg != mo) & ~near).any()
+    ok = ~mg & ~mo
+    assert np.abs(paper[ok] - ref[ok]).max() <= PR.VALUE_TOL * PR.dyn_range(img)
+    extra = ~np.isnan(paper) & np.isnan(area)
+    assert extra.sum() > 300 and not (np.isnan(paper) & ~np.isnan(area)).any()   # a strict superset
+    both = ~np.isnan(area)
+    assert np.array_equal(paper[both], area[both])
+    # nearest: the same as the area rule; bicubic: refused
+    n0 = P.dfr_reproject(d, [src], tgt, (ony, onx), 0).cpu().numpy()
+    n1 = P.dfr_reproject(d, [src], tgt, (ony, onx), 0, edge=P.EDGE_PAPER).cpu().numpy()
+    assert np.array_equal(np.nan_to_num(n0, nan=-1), np.nan_to_num(n1, nan=-1))
+    with pytest.raises(P.DfrError):
+        P.dfr_reproject(d, [src], tgt, (ony, onx), 3, edge=P.EDGE_PAPER)
