@@ -77,6 +77,11 @@ def test_validation_errors_without_gpu(P):
     assert call(ws=(P.DfrWCS * 1)(bad), out=C.c_void_p(0x10000 + 64)) == -7     # ... reaches DFR_ERR_ALIAS
     assert b"overlap" in L.dfr_last_error()
     assert L.dfr_strerror(-5) == b"singular CD matrix"
+    # explicit footprint rule: unknown mode, and the paper's rule with bicubic, are refused
+    def edge(order, mode):
+        return L.dfr_reproject_edge(fake_src, 1, 8, 8, arr, C.byref(good), 8, 8, order, mode, fake_out, None)
+    assert edge(1, 7) == -3 and edge(3, 1) == -3 and b"bicubic" in L.dfr_last_error()
+    assert L.dfr_reproject_edge(None, 1, 8, 8, arr, C.byref(good), 8, 8, 1, 1, fake_out, None) == -1
     # sky entry points validate too
     assert L.dfr_pix2world(None, fake_src, fake_src, 1, fake_out, fake_out, None) == -1
     assert L.dfr_world2pix(C.byref(good), fake_src, fake_src, -1, fake_out, fake_out, None) == -2
