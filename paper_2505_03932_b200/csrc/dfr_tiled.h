@@ -1,6 +1,8 @@
-// dfr_tiled.h — the tiled fast path (dfr_kernels_tiled.cu): data layout of the
+// dfr_tiled.h — the tiled fast path (dfr_tiled_setup.cu, dfr_tiled_main.cu, dfr_tiled_stack.cu): data layout of the
 // per-(exposure, tile) records and the launchers. DESIGN.md §6 describes it.
 #pragma once
+#include <cuda.h>
+
 #include "dfr_internal.h"
 
 namespace dfr {
@@ -34,6 +36,47 @@ struct ProfileEvents {
     cudaEvent_t setup_begin, main_begin, main_end;
     bool enabled;
 };
+
+struct TiledParams {
+    const float *src;
+    float *out;
+    const TileRec *recs;
+    const int2 *cta_box;                           // [n][ctas_y][ctas_x] box origin (kNoBox: none)
+    const SourceDev *srcdev;
+    int n, e0, sny, snx, ony, onx;                 // e0: first exposure of this launch
+    int tiles_x, tiles_y, ctas_x, ctas_y;
+    int BW, BH;                                    // staged box (STAGE) in source pixels
+    int prefetch_dist;                             // L2 prefetch distance in CTA tiles (0: off)
+    int stage_bytes, rec_off;                      // stack kernel: bytes per stage, offset of its records
+};
+
+constexpr int kNoBox = 0x7fffffff;            // cta_box entry of a CTA tile without FAST tiles
+constexpr int kMaxBoxBytes = 36 * 1024;       // staged box limit: keeps >= 6 CTAs (24 warps) per SM
+
+// ---- host side shared by the launchers (dfr_tiled_setup.cu) ----------------
+struct Scratch {
+    double2 *uv = nullptr;
+    TileRec *recs = nullptr;
+    int2 *cta_box = nullptr;
+    int32_t *counters = nullptr;                    // fast, exact, empty, ticket
+};
+
+// Setup kernels + staging decision shared by the per-exposure and the stacking launchers.
+struct Prepared {
+    TiledParams P;
+    Scratch sc;
+    CUtensorMap tmap;
+    bool stage = false;
+    size_t box_bytes = 0;
+};
+
+cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const SourceDev *srcdev,
+                      const SourceDev *srchost, int ony, int onx, cudaStream_t st,
+                      int32_t *host_stats, int stats_add, Scratch &sc, TiledParams &P);
+void free_scratch(Scratch &sc, cudaStream_t st);
+cudaError_t prepare_tiled(const float *src, int n, int sny, int snx, const TargetDev &tgt,
+                          const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx,
+                          int order, cudaStream_t st, int32_t *host_stats, int stats_add, Prepared &R);
 
 cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
                                    const TargetDev &tgt, const SourceDev *srcdev,

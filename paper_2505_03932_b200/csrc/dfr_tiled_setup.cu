@@ -1,0 +1,491 @@
+// dfr_tiled_setup.cu — setup kernels of the tiled fast path and the host
+// side they share with the main kernels (scratch, staging decision, tensor map).
+//
+//   target_nodes_kernel   (fp64) a1-a2 at 25 sample points per 64x64 CTA tile — shared by
+//                         the whole batch, as SURVEY.md §8(a) a10 notes.
+//   tile_setup_kernel     (fp64) a3-a6 at those points per (exposure, CTA tile); fits the
+//                         cubic through 16 Chebyshev nodes, checks it against the exact
+//                         map at 9 other points, re-centres it on the four 32x32 tiles
+//                         (or refits each tile when the 64x64 fit fails), bounds each
+//                         tile's source footprint rigorously, classifies it FAST / EXACT /
+//                         EMPTY, picks the dj degree the main kernel must keep, and
+//                         reduces the origin of the CTA tile's staged box.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+
+#include "dfr_tiled_device.cuh"
+
+namespace dfr {
+
+// ---------------------------------------------------------------------------------
+// constants of the fit
+// ---------------------------------------------------------------------------------
+struct FitConsts {
+    double W[4][4];            // monomial coefficients of the Lagrange basis: L_a(s) = sum_p W[p][a] s^p
+    double pts[NPTS][2];       // sample points (s, t) in [-1, 1]^2; pixel offset = 16 s
+};
+
+static FitConsts make_fit_consts()
+{
+    FitConsts f;
+    double s[4];
+    for (int a = 0; a < 4; ++a) s[a] = std::cos((2 * a + 1) * 3.14159265358979323846 / 8.0);
+    for (int a = 0; a < 4; ++a) {
+        double b[3];
+        int m = 0;
+        for (int k = 0; k < 4; ++k)
+            if (k != a) b[m++] = s[k];
+        const double den = (s[a] - b[0]) * (s[a] - b[1]) * (s[a] - b[2]);
+        f.W[3][a] = 1.0 / den;
+        f.W[2][a] = -(b[0] + b[1] + b[2]) / den;
+        f.W[1][a] = (b[0] * b[1] + b[0] * b[2] + b[1] * b[2]) / den;
+        f.W[0][a] = -(b[0] * b[1] * b[2]) / den;
+    }
+    for (int b = 0; b < 4; ++b)
+        for (int a = 0; a < 4; ++a) {
+            f.pts[4 * b + a][0] = s[a];
+            f.pts[4 * b + a][1] = s[b];
+        }
+    const double h = 0.70710678118654752440;
+    // check points: extrema of T4 (0, +-1/sqrt2, +-1) where the interpolation error of a cubic
+    // through Chebyshev nodes peaks. The axis points matter: at the centre, on the diagonals
+    // and at the corners |T4(s)| = |T4(t)| with equal signs, so fourth-order errors of
+    // opposite sign in s and t (u^4 - v^4) cancel there; (+-h, 0) and (0, +-h) separate them.
+    const double chk[9][2] = {{0, 0}, {h, 0}, {-h, 0}, {0, h}, {0, -h}, {1, 1}, {-1, 1}, {1, -1}, {-1, -1}};
+    for (int k = 0; k < 9; ++k) {
+        f.pts[16 + k][0] = chk[k][0];
+        f.pts[16 + k][1] = chk[k][1];
+    }
+    return f;
+}
+
+// ---------------------------------------------------------------------------------
+// setup kernels (fp64)
+// ---------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+target_nodes_kernel(const __grid_constant__ TargetDev tgt, const __grid_constant__ FitConsts fc,
+                    int ctas_x, int ctas, double2 *__restrict__ uv, int32_t *__restrict__ counters)
+{
+    // tile counters + ticket of the setup kernel start from zero (no memset in the stream)
+    if (blockIdx.x == 0 && threadIdx.x < 4) counters[threadIdx.x] = 0;
+    // sample points of the 64x64 CTA tiles (the parent fit of tile_setup_kernel)
+    pdl_trigger();                                  // the setup kernel may stage its constants meanwhile
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= ctas * NPTS) return;
+    const int c = idx / NPTS, k = idx - c * NPTS;
+    constexpr double edge = TS * CTA_T;
+    const double cx0 = (c % ctas_x) * edge + 0.5 * (edge - 1), cy0 = (c / ctas_x) * edge + 0.5 * (edge - 1);
+    double U, V;
+    target_uv(tgt, cx0 + 0.5 * edge * fc.pts[k][0], cy0 + 0.5 * edge * fc.pts[k][1], U, V);
+    uv[(size_t)k * ctas + c] = make_double2(U, V);          // [point][CTA tile]: coalesced for the setup kernel
+}
+
+// Triangle size and row offset of an order-N packed polynomial (see Poly).
+__host__ __device__ constexpr int tri(int n) { return (n + 1) * (n + 2) / 2; }
+__host__ __device__ constexpr int tri_off(int n, int p) { return p * (n + 1) - (p * (p - 1)) / 2; }
+
+// a3-a6 with the exposure's constants in shared memory, SIP order fixed at compile time
+// (lower orders are zero-padded): sm = { m[9], c1, c2, ap[tri(N)], bp[tri(N)] }.
+// The reciprocal is a float seed + two Newton steps (c is O(1) for any valid point);
+// invalid points (c <= 0, NaN) come out as NaN.
+template <int N>
+__device__ __forceinline__ void source_xy_sm(const double *__restrict__ sm, double U, double V,
+                                             double &x, double &y)
+{
+    const double a = fma(sm[0], U, fma(sm[1], V, sm[2]));
+    const double b = fma(sm[3], U, fma(sm[4], V, sm[5]));
+    const double c = fma(sm[6], U, fma(sm[7], V, sm[8]));
+    float rf;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rf) : "f"((float)c));
+    double r = (double)rf;
+    r = r * fma(-c, r, 2.0);
+    r = r * fma(-c, r, 2.0);
+    if (!(c > 0.0)) r = __longlong_as_double(0x7ff8000000000000LL);
+    const double us = a * r, vs = b * r;
+    x = us + sm[9];
+    y = vs + sm[10];
+    if (N > 0) {
+        x += poly_eval_fixed<N>(sm + 11, us, vs);
+        y += poly_eval_fixed<N>(sm + 11 + tri(N), us, vs);
+    }
+}
+
+// Cubic fit of the pixel map over one square region: 16 Chebyshev nodes -> tensor-product
+// cubic in (s, t) in [-1, 1]^2 (separably: along s within each node row, then along t),
+// then VERIFIED against the exact map at 9 other points (centre, T4 extrema on the axes, corners).
+// uvf(k) returns the target-side (U, V) of sample point k. C[4q + p] = coefficient of s^p t^q.
+template <int N, class UVF>
+__device__ __forceinline__ bool fit_cubic(const double *__restrict__ sm, const FitConsts &fc, UVF uvf,
+                                          double (&Cx)[16], double (&Cy)[16])
+{
+    double Rx[4][4], Ry[4][4];                  // [node row b][power of s]
+    double nanacc = 0.0;
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+        double xs[4], ys[4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            const double2 q = uvf(4 * b + a);
+            source_xy_sm<N>(sm, q.x, q.y, xs[a], ys[a]);
+            nanacc = fma(xs[a], 0.0, fma(ys[a], 0.0, nanacc));
+        }
+#pragma unroll
+        for (int pp = 0; pp < 4; ++pp) {
+            Rx[b][pp] = fma(fc.W[pp][0], xs[0], fma(fc.W[pp][1], xs[1], fma(fc.W[pp][2], xs[2], fc.W[pp][3] * xs[3])));
+            Ry[b][pp] = fma(fc.W[pp][0], ys[0], fma(fc.W[pp][1], ys[1], fma(fc.W[pp][2], ys[2], fc.W[pp][3] * ys[3])));
+        }
+    }
+#pragma unroll
+    for (int qq = 0; qq < 4; ++qq)
+#pragma unroll
+        for (int pp = 0; pp < 4; ++pp) {
+            Cx[4 * qq + pp] = fma(fc.W[qq][0], Rx[0][pp], fma(fc.W[qq][1], Rx[1][pp], fma(fc.W[qq][2], Rx[2][pp], fc.W[qq][3] * Rx[3][pp])));
+            Cy[4 * qq + pp] = fma(fc.W[qq][0], Ry[0][pp], fma(fc.W[qq][1], Ry[1][pp], fma(fc.W[qq][2], Ry[2][pp], fc.W[qq][3] * Ry[3][pp])));
+        }
+    bool good = true;
+#pragma unroll
+    for (int k = 16; k < NPTS; ++k) {
+        const double2 q = uvf(k);
+        double x, y;
+        source_xy_sm<N>(sm, q.x, q.y, x, y);
+        const double ss = fc.pts[k][0], tt = fc.pts[k][1];
+        double px = 0.0, py = 0.0;
+#pragma unroll
+        for (int qq = 3; qq >= 0; --qq) {
+            const double rx = fma(fma(fma(Cx[4 * qq + 3], ss, Cx[4 * qq + 2]), ss, Cx[4 * qq + 1]), ss, Cx[4 * qq]);
+            const double ry = fma(fma(fma(Cy[4 * qq + 3], ss, Cy[4 * qq + 2]), ss, Cy[4 * qq + 1]), ss, Cy[4 * qq]);
+            px = fma(px, tt, rx);
+            py = fma(py, tt, ry);
+        }
+        good = good && (fabs(px - x) <= (double)FIT_TOL) && (fabs(py - y) <= (double)FIT_TOL);   // false on NaN
+    }
+    return good && (nanacc == 0.0);
+}
+
+// p(s0 + s'/2) as a cubic in s': the re-centring of a parent cubic (unit = 32 px) on one of
+// its halves (unit = 16 px). Exact up to fp64 rounding.
+__device__ __forceinline__ void shift_half(double &c0, double &c1, double &c2, double &c3, double s0)
+{
+    const double d0 = fma(s0, fma(s0, fma(s0, c3, c2), c1), c0);
+    const double d1 = 0.5 * fma(s0, fma(3.0 * s0, c3, 2.0 * c2), c1);
+    const double d2 = 0.25 * fma(3.0 * s0, c3, c2);
+    c0 = d0; c1 = d1; c2 = d2; c3 = 0.125 * c3;
+}
+
+// The record of one 32x32 tile from its cubic (unit = 16 px about the tile centre):
+// footprint bound, classification, dj degree, integer base, fp32 coefficients.
+// Returns the flag; (bx0, by0) is the first floor index the tile can touch.
+__device__ __forceinline__ int emit_tile(double (&Cx)[16], double (&Cy)[16], bool finite, int sny, int snx,
+                                         TileRec *__restrict__ out, int &bx0, int &by0)
+{
+    // Rigorous range of the fitted polynomial over the tile: |s|, |t| <= 31/32 < 1, so
+    // |x - C00| <= sum of the other |C_pq|. The main kernel evaluates exactly this
+    // polynomial (in fp32: + kBoxSlack), which is what makes its unchecked gathers safe.
+    double ex = 0.0, ey = 0.0;
+#pragma unroll
+    for (int k = 1; k < 16; ++k) { ex += fabs(Cx[k]); ey += fabs(Cy[k]); }
+    constexpr double kBoxSlack = 1e-3;
+    const double xmin = Cx[0] - ex - kBoxSlack, xmax = Cx[0] + ex + kBoxSlack;
+    const double ymin = Cy[0] - ey - kBoxSlack, ymax = Cy[0] + ey + kBoxSlack;
+    // Degree of the per-lane column polynomials in dj: the t^2, t^3 terms (any power of s)
+    // are dropped by the main kernel when they cannot move a coordinate by kDegTol px.
+    double q2x = 0.0, q2y = 0.0, q3x = 0.0, q3y = 0.0;
+#pragma unroll
+    for (int pp = 0; pp < 4; ++pp) {
+        q2x += fabs(Cx[8 + pp]); q2y += fabs(Cy[8 + pp]);
+        q3x += fabs(Cx[12 + pp]); q3y += fabs(Cy[12 + pp]);
+    }
+    constexpr double kDegTol = 2.5e-7;
+    TileRec r;
+    r.deg = fmax(q3x, q3y) >= kDegTol ? 3 : (fmax(q2x, q2y) >= kDegTol ? 2 : 1);
+    int flag = TILE_EXACT;
+    r.ix0 = r.iy0 = r.bx0 = r.by0 = r.bx1 = r.by1 = 0;
+    double bx = 0.0, by = 0.0;
+    if (finite && fabs(xmin) < 1e9 && fabs(xmax) < 1e9 && fabs(ymin) < 1e9 && fabs(ymax) < 1e9) {
+        bx = floor(Cx[0]); by = floor(Cy[0]);
+        r.ix0 = (int)bx; r.iy0 = (int)by;
+        r.bx0 = (int)floor(xmin); r.bx1 = (int)floor(xmax);
+        r.by0 = (int)floor(ymin); r.by1 = (int)floor(ymax);
+        const bool small = (r.bx1 - r.bx0) < 2048 && (r.by1 - r.by0) < 2048 &&
+                           abs(r.bx0 - r.ix0) < 2048 && abs(r.bx1 - r.ix0) < 2048 &&
+                           abs(r.by0 - r.iy0) < 2048 && abs(r.by1 - r.iy0) < 2048;
+        if (small) {
+            // outside the footprint [-0.5, n-0.5) by a 2 px margin on one side => all NaN
+            const bool outside = (xmax + 2.0 < -0.5) || (xmin - 2.0 >= snx - 0.5) ||
+                                 (ymax + 2.0 < -0.5) || (ymin - 2.0 >= sny - 0.5);
+            flag = outside ? TILE_EMPTY : TILE_FAST;
+        } else {
+            bx = by = 0.0;
+        }
+    }
+    r.flag = flag;
+    bx0 = r.bx0; by0 = r.by0;
+    // s = di / 16: coefficient of di^p dj^q is C[p][q] / 16^(p+q)
+    double sq = 1.0;
+#pragma unroll
+    for (int qq = 0; qq < 4; ++qq) {
+        double sp = sq;
+#pragma unroll
+        for (int pp = 0; pp < 4; ++pp) {
+            const double c0x = (qq == 0 && pp == 0) ? Cx[0] - bx : Cx[4 * qq + pp];
+            const double c0y = (qq == 0 && pp == 0) ? Cy[0] - by : Cy[4 * qq + pp];
+            r.cx[4 * qq + pp] = (float)(c0x * sp);
+            r.cy[4 * qq + pp] = (float)(c0y * sp);
+            sp *= 1.0 / kHalf;
+        }
+        sq *= 1.0 / kHalf;
+    }
+    *out = r;
+    return flag;
+}
+
+// One thread per (64x64 CTA tile, exposure); a block is 128 consecutive CTA tiles of ONE
+// exposure, so the exposure's constants are staged once in shared memory and every
+// coefficient read is a broadcast LDS. Two levels:
+//   1. the cubic is fitted and verified over the whole 64x64 CTA tile (25 map evaluations);
+//      if it holds, the four 32x32 tile records are its exact re-centrings (no more map
+//      evaluations) — 4x less fp64 work than fitting each tile;
+//   2. if it does not (strongly curved maps), each 32x32 tile gets its own fit, with the
+//      target side (a1-a2) evaluated on the fly; a tile whose own fit fails is EXACT.
+// (Measured on B200, C2: 16.8 us; four threads per CTA tile sharing the parent fit through
+// shared memory took 21-23 us — more waves of a latency-bound kernel — so this stays.)
+constexpr int kSetupThreads = 128;
+
+template <int N>
+__global__ void __launch_bounds__(kSetupThreads)
+tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ srcdev,
+                  const __grid_constant__ TargetDev tgt, const __grid_constant__ FitConsts fc, int e0,
+                  int tiles_x, int tiles_y, int ctas_x, int ctas, int sny, int snx,
+                  TileRec *__restrict__ recs, int2 *__restrict__ cta_box, int32_t *__restrict__ counters,
+                  int total_blocks, int32_t *__restrict__ host_stats, int stats_add)
+{
+    __shared__ double sm[11 + 2 * tri(N)];
+    const int e = e0 + blockIdx.y;
+    {
+        const SourceDev &s = srcdev[e];
+        for (int k = threadIdx.x; k < 11 + 2 * tri(N); k += blockDim.x) {
+            double v;
+            if (k < 9) v = s.m[k];
+            else if (k == 9) v = s.c1;
+            else if (k == 10) v = s.c2;
+            else {
+                // slot of the order-N layout -> (p, q) -> slot of the stored order-n layout
+                const int t = (k - 11) % tri(N);
+                const Poly &P = (k - 11) < tri(N) ? s.ap : s.bp;
+                int p = 0;
+                while (p < N && tri_off(N, p + 1) <= t) ++p;
+                const int q = t - tri_off(N, p), n = P.order;
+                v = (p + q <= n) ? P.c[tri_off(n, p) + q] : 0.0;
+            }
+            sm[k] = v;
+        }
+    }
+    pdl_trigger();                                  // the main kernel's launch may overlap this one
+    __syncthreads();
+    pdl_wait();                                     // the node table is complete
+    const int c = blockIdx.x * kSetupThreads + threadIdx.x;
+    int nflag[3] = {0, 0, 0};
+    if (c < ctas) {
+        const int cty = c / ctas_x, ctx = c - cty * ctas_x;
+        double Px[16], Py[16];                      // parent cubic, unit = 32 px
+        const bool parent = fit_cubic<N>(sm, fc, [&](int k) { return __ldg(uv + (size_t)k * ctas + c); }, Px, Py);
+        int box_x = kNoBox, box_y = kNoBox;
+#pragma unroll 1
+        for (int sub = 0; sub < CTA_T * CTA_T; ++sub) {
+            const int ttx = ctx * CTA_T + (sub % CTA_T), tty = cty * CTA_T + (sub / CTA_T);
+            if (ttx >= tiles_x || tty >= tiles_y) continue;
+            double Cx[16], Cy[16];
+            bool good = true;
+            if (parent) {
+                const double s0 = (sub % CTA_T) ? 0.5 : -0.5, t0 = (sub / CTA_T) ? 0.5 : -0.5;
+#pragma unroll
+                for (int k = 0; k < 16; ++k) { Cx[k] = Px[k]; Cy[k] = Py[k]; }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {       // along s, each power of t
+                    shift_half(Cx[4 * q], Cx[4 * q + 1], Cx[4 * q + 2], Cx[4 * q + 3], s0);
+                    shift_half(Cy[4 * q], Cy[4 * q + 1], Cy[4 * q + 2], Cy[4 * q + 3], s0);
+                }
+#pragma unroll
+                for (int pp = 0; pp < 4; ++pp) {    // along t, each power of s
+                    shift_half(Cx[pp], Cx[4 + pp], Cx[8 + pp], Cx[12 + pp], t0);
+                    shift_half(Cy[pp], Cy[4 + pp], Cy[8 + pp], Cy[12 + pp], t0);
+                }
+            } else {
+                const double cx0 = ttx * TS + kCentre, cy0 = tty * TS + kCentre;
+                good = fit_cubic<N>(sm, fc, [&](int k) {
+                    double U, V;
+                    target_uv(tgt, cx0 + kHalf * fc.pts[k][0], cy0 + kHalf * fc.pts[k][1], U, V);
+                    return make_double2(U, V);
+                }, Cx, Cy);
+            }
+            int bx0, by0;
+            const int flag = emit_tile(Cx, Cy, good, sny, snx,
+                                       recs + ((size_t)e * tiles_x * tiles_y + (size_t)tty * tiles_x + ttx), bx0, by0);
+            ++nflag[flag];
+            if (flag == TILE_FAST) { box_x = min(box_x, bx0); box_y = min(box_y, by0); }
+        }
+        // origin of the CTA tile's staged box = min over its FAST tiles (kNoBox: none)
+        cta_box[(size_t)e * ctas + c] = make_int2(box_x, box_y);
+    }
+    // tile statistics: per-warp sums -> device counters; the last block of the last launch
+    // (ticket) writes the totals straight into the caller's mapped host memory, so
+    // dfr_last_stats needs neither a memset nor a copy in the stream
+#pragma unroll
+    for (int f = 0; f < 3; ++f) {
+        const int w = __reduce_add_sync(0xffffffffu, nflag[f]);
+        if ((threadIdx.x & 31) == 0 && w) atomicAdd(&counters[f], w);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0 && host_stats) {
+        __threadfence();
+        if (atomicAdd(&counters[3], 1) == total_blocks - 1) {
+            __threadfence();
+            for (int f = 0; f < 3; ++f) {
+                const int32_t v = *(volatile int32_t *)&counters[f];
+                if (stats_add) atomicAdd(&host_stats[f], v);     // streaming calls: device-side totals
+                else host_stats[f] = v;
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *,
+                                  const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
+                                  const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn get_encode()
+{
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+
+// Source-pixel extent of a 64x64 output tile, from the Jacobian of the map probed in fp64
+// on the host at the centre of the output grid, per exposure (3 map evaluations each; the
+// Jacobian varies by well under 1 % over a frame, the caller adds 2 % + fixed margins, and
+// the kernel checks every pixel against the staged box anyway). False if no probe is finite.
+static bool probe_extent(const TargetDev &tgt, const SourceDev *hs, int n, int ony, int onx,
+                         double &ext_x, double &ext_y)
+{
+    const double span = TS * CTA_T - 1;
+    const double ci = 0.5 * (onx - 1), cj = 0.5 * (ony - 1), h = 16.0;
+    double U0, V0, U1, V1, U2, V2;
+    target_uv(tgt, ci, cj, U0, V0);
+    target_uv(tgt, ci + h, cj, U1, V1);
+    target_uv(tgt, ci, cj + h, U2, V2);
+    const int step = n > 256 ? n / 256 : 1;
+    bool any = false;
+    ext_x = ext_y = 0.0;
+    for (int e = 0; e < n; e += step) {
+        double x0, y0, x1, y1, x2, y2;
+        source_xy(hs[e], U0, V0, x0, y0);
+        source_xy(hs[e], U1, V1, x1, y1);
+        source_xy(hs[e], U2, V2, x2, y2);
+        const double jxx = (x1 - x0) / h, jxy = (x2 - x0) / h, jyx = (y1 - y0) / h, jyy = (y2 - y0) / h;
+        if (!(std::isfinite(jxx) && std::isfinite(jxy) && std::isfinite(jyx) && std::isfinite(jyy))) continue;
+        any = true;
+        ext_x = std::fmax(ext_x, span * (std::fabs(jxx) + std::fabs(jxy)));
+        ext_y = std::fmax(ext_y, span * (std::fabs(jyx) + std::fabs(jyy)));
+    }
+    return any;
+}
+
+cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const SourceDev *srcdev,
+                             const SourceDev *srchost, int ony, int onx, cudaStream_t st,
+                             int32_t *host_stats, int stats_add, Scratch &sc, TiledParams &P)
+{
+    static const FitConsts fc = make_fit_consts();
+    P.n = n; P.sny = sny; P.snx = snx; P.ony = ony; P.onx = onx;
+    P.tiles_x = (onx + TS - 1) / TS;
+    P.tiles_y = (ony + TS - 1) / TS;
+    P.ctas_x = (P.tiles_x + CTA_T - 1) / CTA_T;
+    P.ctas_y = (P.tiles_y + CTA_T - 1) / CTA_T;
+    P.srcdev = srcdev;
+    const int ntile = P.tiles_x * P.tiles_y;
+    cudaError_t err;
+    const int ctas = P.ctas_x * P.ctas_y;
+    if ((err = cudaMallocAsync((void **)&sc.uv, sizeof(double2) * (size_t)ctas * NPTS, st)) != cudaSuccess) return err;
+    if ((err = cudaMallocAsync((void **)&sc.recs, sizeof(TileRec) * (size_t)ntile * n, st)) != cudaSuccess) return err;
+    P.recs = sc.recs;
+    if ((err = cudaMallocAsync((void **)&sc.cta_box, sizeof(int2) * (size_t)ctas * n, st)) != cudaSuccess) return err;
+    P.cta_box = sc.cta_box;
+    if ((err = cudaMallocAsync((void **)&sc.counters, 4 * sizeof(int32_t), st)) != cudaSuccess) return err;
+    target_nodes_kernel<<<(ctas * NPTS + 127) / 128, 128, 0, st>>>(tgt, fc, P.ctas_x, ctas, sc.uv, sc.counters);
+    if ((err = cudaGetLastError()) != cudaSuccess) return err;
+    // SIP order class of the batch: inverse polynomials are zero-padded up to N
+    int maxo = 0;
+    for (int e = 0; e < n; ++e) maxo = std::max(maxo, std::max(srchost[e].ap.order, srchost[e].bp.order));
+    const unsigned bx = (unsigned)((ctas + kSetupThreads - 1) / kSetupThreads);
+    const long long total_blocks = (long long)bx * n;
+    if (total_blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    for (int e0 = 0; e0 < n; e0 += 65535) {
+        const dim3 grid(bx, (unsigned)std::min(n - e0, 65535));
+        if (maxo == 0) err = launch_pdl(tile_setup_kernel<0>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
+        else if (maxo <= 3) err = launch_pdl(tile_setup_kernel<3>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
+        else if (maxo <= 4) err = launch_pdl(tile_setup_kernel<4>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
+        else if (maxo <= 5) err = launch_pdl(tile_setup_kernel<5>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
+        else err = launch_pdl(tile_setup_kernel<9>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
+        if (err != cudaSuccess) return err;
+    }
+    return cudaSuccess;
+}
+
+void free_scratch(Scratch &sc, cudaStream_t st)
+{
+    if (sc.uv) cudaFreeAsync(sc.uv, st);
+    if (sc.recs) cudaFreeAsync(sc.recs, st);
+    if (sc.cta_box) cudaFreeAsync(sc.cta_box, st);
+    if (sc.counters) cudaFreeAsync(sc.counters, st);
+}
+
+cudaError_t prepare_tiled(const float *src, int n, int sny, int snx, const TargetDev &tgt,
+                                 const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx,
+                                 int order, cudaStream_t st, int32_t *host_stats, int stats_add, Prepared &R)
+{
+    std::memset(&R.P, 0, sizeof R.P);
+    std::memset(&R.tmap, 0, sizeof R.tmap);
+    R.P.src = src;
+    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, srchost, ony, onx, st, host_stats, stats_add, R.sc, R.P);
+    if (err != cudaSuccess) return err;
+    // ---- staging decision: box size from a host probe; TMA needs 16-byte rows
+    double ex, ey;
+    const int tlo = (order == DFR_BICUBIC) ? 1 : 0, thi = (order == DFR_BICUBIC) ? 2 : 1;
+    EncodeTiledFn enc = get_encode();
+    static const bool no_stage = std::getenv("DFR_NO_STAGE") != nullptr;   // debugging / A-B timing only
+    if (!no_stage && enc && (snx % 4 == 0) && ((uintptr_t)src % 16 == 0) && probe_extent(tgt, srchost, n, ony, onx, ex, ey)) {
+        // floor-range spread + taps + 1 px safety each side; + 3: the origin is rounded down
+        // to a multiple of 4 floats; then the width itself is rounded up to 16 bytes
+        const int bw = ((int)std::ceil(ex * 1.02) + 2 + tlo + thi + 2 + 3 + 3) & ~3;
+        const int bh = (int)std::ceil(ey * 1.02) + 2 + tlo + thi + 2;
+        if (bw <= 256 && bh <= 256 && (size_t)bw * bh * sizeof(float) <= (size_t)kMaxBoxBytes) {
+            const cuuint64_t dims[3] = {(cuuint64_t)snx, (cuuint64_t)sny, (cuuint64_t)n};
+            const cuuint64_t strides[2] = {(cuuint64_t)snx * 4, (cuuint64_t)snx * sny * 4};
+            const cuuint32_t boxd[3] = {(cuuint32_t)bw, (cuuint32_t)bh, 1};
+            const cuuint32_t estr[3] = {1, 1, 1};
+            CUresult r = enc(&R.tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)src, dims, strides, boxd, estr,
+                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                             CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r == CUDA_SUCCESS) { R.stage = true; R.P.BW = bw; R.P.BH = bh; }
+        }
+    }
+    R.box_bytes = R.stage ? (size_t)R.P.BW * R.P.BH * sizeof(float) : 0;
+    return cudaSuccess;
+}
+
+}  // namespace dfr
