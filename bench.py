@@ -40,10 +40,56 @@ METRIC = "output Mpix/s reprojected (2048^2 TAN-SIP3 bilinear, batch 32)"
 UNIT = "Mpix/s"
 BATCH, NPIX = 32, 2048
 FALLBACK_HBM_GBS = 6650.0          # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
-# dram__bytes_read.sum + dram__bytes_write.sum of one tiled_reproject_kernel launch on this
-# workload, from the `ncu --set full` capture summarised in profiles/ (cannot be measured live)
-NCU_TRAFFIC_BYTES = 536.94e6 + 493.84e6
-NCU_TRAFFIC_SOURCE = "profiles/r01_main_kernel_ncu.md"
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernels cannot be
+# measured live (they need ncu): profiles/ncu_traffic.json holds them together with the hash of
+# the kernel sources they were captured from; a line built from other sources reports null.
+NCU_TRAFFIC_FILE = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+
+
+def kernel_source_hash():
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_2505_03932_b200", "csrc")
+    for f in sorted(glob.glob(os.path.join(csrc, "*.cu")) + glob.glob(os.path.join(csrc, "*.cuh"))
+                    + glob.glob(os.path.join(csrc, "*.h"))):
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(kernel):
+    """(bytes per launch, source) from profiles/ncu_traffic.json, or (None, why)."""
+    try:
+        d = json.load(open(NCU_TRAFFIC_FILE))[kernel]
+    except (OSError, KeyError, ValueError):
+        return None, "no ncu capture recorded for " + kernel
+    if d.get("source_hash") != kernel_source_hash():
+        return None, f"stale: {d.get('summary')} was captured from other kernel sources"
+    return float(d["dram_bytes_read"]) + float(d["dram_bytes_write"]), d.get("summary")
+
+
+def source_pixels_touched(P, torch, src_wcs, tgt, src_shape, shape_out, chunk=4):
+    """Unique source pixels the bilinear taps of one step read (algorithmic
+    bytes = 4 B per output pixel + 4 B per unique source pixel touched), counted on the device
+    from the coordinates the kernels themselves use (dfr_src_coords), outside any timed region."""
+    sny, snx = src_shape
+    n = len(src_wcs)
+    total = 0
+    for e0 in range(0, n, chunk):
+        ws = src_wcs[e0:e0 + chunk]
+        x, y = P.dfr_src_coords(ws, tgt, src_shape, shape_out, P.BILINEAR)
+        for k in range(len(ws)):
+            xe, ye = x[k].reshape(-1), y[k].reshape(-1)
+            ok = (xe >= -0.5) & (xe < snx - 0.5) & (ye >= -0.5) & (ye < sny - 0.5)
+            ix, iy = torch.floor(xe[ok]).long(), torch.floor(ye[ok]).long()
+            mask = torch.zeros(sny * snx, dtype=torch.bool, device=x.device)
+            for dy in (0, 1):
+                for dx in (0, 1):
+                    mask[(iy + dy).clamp(0, sny - 1) * snx + (ix + dx).clamp(0, snx - 1)] = True
+            total += int(mask.sum().item())
+        del x, y
+    return total
 
 
 def peaks():
@@ -165,9 +211,16 @@ def run_stack(args):
     for _ in range(max(args.warmup, 3)):
         step()
     torch.cuda.synchronize()
+    def load(seconds):
+        t_end = time.perf_counter() + seconds
+        while time.perf_counter() < t_end:
+            for _ in range(50):
+                step()
+            torch.cuda.synchronize()
+
     sampler = ClockSampler(0)
     sampler.start()
-    time.sleep(0.3)
+    load(args.load_seconds)
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     torch.cuda.synchronize()
     ev[0].record()
@@ -177,7 +230,7 @@ def run_stack(args):
     torch.cuda.synchronize()
     total_ms = ev[0].elapsed_time(ev[-1])
     per_step = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
-    time.sleep(0.2)
+    load(0.5 * args.load_seconds)
     sampler.stop()
     P.dfr_profile_enable(True)
     ms = []
@@ -189,8 +242,10 @@ def run_stack(args):
     stats = P.dfr_last_stats()
     in_mpix = BATCH * NPIX * NPIX / 1e6
     hbm, which, _ = peaks()
-    alg = 4.0 * BATCH * NPIX * NPIX + 8.0 * NPIX * NPIX       # sources read once + sum and wsum written
+    touched = source_pixels_touched(P, torch, w.src_wcs, w.tgt_wcs, (NPIX, NPIX), (NPIX, NPIX))
+    alg = 4.0 * touched + 8.0 * NPIX * NPIX       # source pixels touched, read once + sum and wsum written
     achieved = alg / (main_ms * 1e-3) / 1e9
+    traffic, traffic_src = ncu_traffic("tiled_stack_kernel<1,1>")
     line = {"metric": "input exposure Mpix/s reprojected and stacked (32 x 2048^2 TAN-SIP3 bilinear -> one 2048^2 sum + weight)",
             "value": in_mpix * args.steps / (total_ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
@@ -199,7 +254,8 @@ def run_stack(args):
                        "l2": "inputs per step are 537 MB > 126 MB L2 (no flush needed)", "tiles": stats},
             "ms_per_step_median": statistics.median(per_step),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm,
-                         "traffic": None, "peak_source": which, "kernel": "tiled_stack_kernel", "kernel_ms": main_ms,
+                         "traffic": traffic, "traffic_source": traffic_src, "peak_source": which,
+                         "kernel": "tiled_stack_kernel<1,1>", "kernel_ms": main_ms, "source_pixels_touched": touched,
                          "setup_kernels_ms": statistics.mean(m[0] for m in ms), "algorithmic_bytes_per_launch": alg,
                          "note": "issue-bound, not HBM-bound: see DESIGN.md §6.5"},
             "cpu_baseline": None, "e2e": None, "gpu_launches": int(stats["kernels"]) * args.steps,
@@ -216,6 +272,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--load-seconds", type=float, default=0.7,
+                    help="untimed back-to-back steps before (and half as long after) the timed region")
     ap.add_argument("--path", default="auto", choices=["auto", "exact"])
     ap.add_argument("--mode", default="reproject", choices=["reproject", "stack"],
                     help="stack: the fused reproject-and-stack entry point (SURVEY.md §8(f) f1) on the same "
@@ -269,36 +327,54 @@ def main():
     barrier()
     stats = P.dfr_last_stats()
 
+    def load(seconds):
+        """untimed back-to-back steps: keeps the GPU under the SAME load around the timed
+        region, so the 100 ms clock sampler reads clocks while these kernels run"""
+        t_end = time.perf_counter() + seconds
+        while time.perf_counter() < t_end:
+            for _ in range(50):
+                step()
+            torch.cuda.synchronize()
+
+    def timed(k_steps):
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(k_steps + 1)]
+        barrier()
+        ev[0].record()
+        for k in range(k_steps):
+            step()
+            ev[k + 1].record()
+        barrier()
+        return ev[0].elapsed_time(ev[-1]), [ev[k].elapsed_time(ev[k + 1]) for k in range(k_steps)]
+
+    # ---- burst figure: K steps right after the warm-up, GPU otherwise idle (boost clocks)
+    burst_ms, burst_steps = timed(args.steps)
+    burst_ms = max_over_ranks(burst_ms, device="cuda")
+    # ---- the timed region proper: K steps inside a sustained run of the same steps, CUDA events
+    # on the launching (current) stream; clocks and throttle reasons sampled during it
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-        time.sleep(0.3)
-    # ---- timed region: K steps, CUDA events on the launching (current) stream
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    barrier()
-    ev[0].record()
-    for k in range(args.steps):
-        step()
-        ev[k + 1].record()
-    barrier()
-    total_ms = ev[0].elapsed_time(ev[-1])
-    per_step = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
+    load(args.load_seconds)
+    total_ms, per_step = timed(args.steps)
+    # ---- dominant kernel, timed live by the library's own events on the launching stream, still
+    # inside the sustained run (20 plain steps between two profiled ones keep the GPU loaded)
+    kern_ms = None
+    if path == P.PATH_AUTO:
+        ms = []
+        for _ in range(min(args.steps, 10)):
+            for _ in range(20):
+                step()
+            P.dfr_profile_enable(True)
+            step()
+            ms.append(P.dfr_profile_last())          # waits for this call's last event
+            P.dfr_profile_enable(False)
+        kern_ms = {"setup_ms": statistics.mean(m[0] for m in ms), "main_ms": statistics.mean(m[1] for m in ms)}
+    load(0.5 * args.load_seconds)
     if rank == 0:
-        time.sleep(0.2)
         sampler.stop()
     total_ms = max_over_ranks(total_ms, device="cuda")
     value = out_mpix * world * args.steps / (total_ms * 1e-3)
 
-    # ---- dominant kernel, timed live by the library's own events on the launching stream
-    kern_ms = None
-    if path == P.PATH_AUTO:
-        P.dfr_profile_enable(True)
-        ms = []
-        for _ in range(min(args.steps, 10)):
-            step()
-            ms.append(P.dfr_profile_last())          # waits for the call's last event
-        P.dfr_profile_enable(False)
-        kern_ms = {"setup_ms": statistics.mean(m[0] for m in ms), "main_ms": statistics.mean(m[1] for m in ms)}
     nan_frac = float(torch.isnan(out).float().mean().item())
 
     # ---- e2e: HOST pinned buffers through dfr_reproject_host (copies inside the timed region)
@@ -324,19 +400,24 @@ def main():
             dist.destroy_process_group()
         return 0
 
-    # ---- roofline: algorithmic bytes = 4 B stored per output pixel + 4 B per source pixel read once
+    # ---- roofline: algorithmic bytes = 4 B stored per output pixel (NaN
+    # included) + 4 B per UNIQUE source pixel the taps touch, counted from the kernels' own
+    # coordinates; 8 B per output pixel is the upper bound (`frac_upper`)
     hbm, which, sm_max = peaks()
-    # (8 B per output pixel is the upper bound SURVEY.md §8(d) states; the
-    # source pixels outside every output footprint and the NaN pixels are NOT subtracted)
-    alg_bytes = 8.0 * BATCH * NPIX * NPIX
+    touched = source_pixels_touched(P, torch, w.src_wcs, w.tgt_wcs, (NPIX, NPIX), (NPIX, NPIX))
+    alg_bytes = 4.0 * BATCH * NPIX * NPIX + 4.0 * touched
+    upper_bytes = 8.0 * BATCH * NPIX * NPIX
     dom_ms = kern_ms["main_ms"] if kern_ms else statistics.median(per_step)
     achieved = alg_bytes / (dom_ms * 1e-3) / 1e9
+    traffic, traffic_src = ncu_traffic("tiled_reproject_kernel<1,1,0>") if kern_ms else (None, None)
     roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s",
-                "frac": achieved / hbm, "traffic": NCU_TRAFFIC_BYTES if kern_ms else None,
-                "traffic_source": NCU_TRAFFIC_SOURCE, "peak_source": which,
-                "kernel": "tiled_reproject_kernel" if kern_ms else "whole dfr_reproject call",
+                "frac": achieved / hbm, "frac_upper": upper_bytes / (dom_ms * 1e-3) / 1e9 / hbm,
+                "frac_whole_call": alg_bytes / (statistics.median(per_step) * 1e-3) / 1e9 / hbm,
+                "traffic": traffic, "traffic_source": traffic_src, "peak_source": which,
+                "kernel": "tiled_reproject_kernel<1,1,0>" if kern_ms else "whole dfr_reproject call",
                 "kernel_ms": dom_ms, "setup_kernels_ms": kern_ms["setup_ms"] if kern_ms else None,
-                "algorithmic_bytes_per_launch": alg_bytes}
+                "algorithmic_bytes_per_launch": alg_bytes, "source_pixels_touched": touched,
+                "upper_bound_bytes_per_launch": upper_bytes}
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -345,9 +426,16 @@ def main():
         v1, dt1, cores = time_oracle(w, n_exp)
         passes = int(min(8, max(1, round(10.0 / max(dt1, 1e-3)))))
         v, dt, cores = time_oracle(w, n_exp, passes)
+        import oracle
+        oracle.set_threads(1)
+        w1 = S.Workload("c2-1", w.images[:1], w.src_wcs[:1], w.tgt_wcs, w.shape_out, (1,))
+        v1t, dt1t, _ = time_oracle(w1, 1)
+        oracle.set_threads(cores)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"all {n_exp} exposures of the step, full 2048x2048 frames, {passes} pass(es) after "
-                         f"one sizing pass ({dt:.1f} s wall, {dt * cores:.0f} core-seconds)"}
+                         f"one sizing pass ({dt:.1f} s wall, {dt * cores:.0f} core-seconds)",
+               "value_1thread": v1t,
+               "sample_1thread": f"exposure 0 of the step, full 2048x2048 frame, one pass ({dt1t:.1f} s)"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
@@ -357,6 +445,10 @@ def main():
                        "l2": "inputs+outputs per step are 1074 MB > 126 MB L2 (no flush needed)",
                        "nan_fraction": nan_frac, "tiles": stats},
             "ms_per_step_median": statistics.median(per_step),
+            "burst": {"value": out_mpix * world * args.steps / (burst_ms * 1e-3), "ms_per_step": burst_ms / args.steps,
+                      "ms_per_step_median": statistics.median(burst_steps),
+                      "note": "the same K steps timed right after the warm-up on an idle GPU (boost clocks); "
+                              "`value` is measured inside a sustained run, where the power cap lowers the SM clock"},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
             "gpu_launches": int(stats["kernels"]) * args.steps,
             "clocks": sampler.summary()}

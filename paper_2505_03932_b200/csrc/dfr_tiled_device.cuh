@@ -220,16 +220,20 @@ __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
 }
 __device__ __forceinline__ f32x2 splat2(float v) { return pk2(v, v); }
 
-// Keys weights (a = -0.75) on a packed pair of fractions; same formulas as keys_weights.
+// Keys weights (a = -0.75) on a packed pair of fractions t in [0, 1): the same cubics as
+// keys_weights, factored so the outer taps share u = t (1 - t):
+//   w0 = a t (1-t)^2 = (a u)(1-t),  w3 = a t^2 (1-t) = (a u) t,
+//   w1 = ((a+2) t - (a+3)) t^2 + 1,  w2 = ((a+2)(1-t) - (a+3)) (1-t)^2 + 1      (11 packed ops, was 15)
 __device__ __forceinline__ void keys_weights2(f32x2 t, f32x2 w[4])
 {
     const float A = -0.75f;
     const f32x2 one = splat2(1.0f);
-    const f32x2 t1 = add2(t, one), s = sub2(one, t), s1 = sub2(splat2(2.0f), t);
-    w[0] = fma2(fma2(fma2(splat2(A), t1, splat2(-5.0f * A)), t1, splat2(8.0f * A)), t1, splat2(-4.0f * A));
+    const f32x2 s = sub2(one, t);
+    const f32x2 au = mul2(mul2(t, s), splat2(A));
+    w[0] = mul2(au, s);
+    w[3] = mul2(au, t);
     w[1] = fma2(fma2(splat2(A + 2.0f), t, splat2(-(A + 3.0f))), mul2(t, t), one);
     w[2] = fma2(fma2(splat2(A + 2.0f), s, splat2(-(A + 3.0f))), mul2(s, s), one);
-    w[3] = fma2(fma2(fma2(splat2(A), s1, splat2(-5.0f * A)), s1, splat2(8.0f * A)), s1, splat2(-4.0f * A));
 }
 
 // Two rows (dj, dj + 1) of an INTERIOR tile of a STAGE kernel: every tap of every pixel is

@@ -22,8 +22,11 @@ namespace dfr {
 // ---------------------------------------------------------------------------------
 // EDGE (DFR_EDGE_*) is a template parameter so that the default kernel is compiled exactly as
 // without it (a run-time flag cost 3 % through register allocation alone).
+#ifndef DFR_BICUBIC_MINB
+#define DFR_BICUBIC_MINB 8
+#endif
 template <int ORDER, bool STAGE, int EDGE = DFR_EDGE_AREA>
-__global__ void __launch_bounds__(32 * CTA_T * CTA_T, 8)
+__global__ void __launch_bounds__(32 * CTA_T * CTA_T, ORDER == DFR_BICUBIC ? DFR_BICUBIC_MINB : 8)
 tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_constant__ TargetDev tgt,
                        const __grid_constant__ CUtensorMap tmap)
 {
@@ -181,8 +184,10 @@ static cudaError_t launch_main(const TiledParams &P, const TargetDev &tgt, const
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess &&
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 32 * CTA_T * CTA_T, smem) == cudaSuccess)
             Q.prefetch_dist = sms * per_sm / 2;     // measured on B200, C2: flat optimum between 1/2 and 3/4 of a wave
-        static const char *pd = std::getenv("DFR_PREFETCH");      // A-B timing only
+#ifdef DFR_DEV_HOOKS                                                 // A-B timing builds only (never the shipped library)
+        static const char *pd = std::getenv("DFR_PREFETCH");
         if (pd) Q.prefetch_dist = std::atoi(pd);
+#endif
     }
     for (int e0 = 0; e0 < P.n; e0 += 65535) {
         Q.e0 = e0;

@@ -467,11 +467,17 @@ cudaError_t prepare_tiled(const float *src, int n, int sny, int snx, const Targe
     double ex, ey;
     const int tlo = (order == DFR_BICUBIC) ? 1 : 0, thi = (order == DFR_BICUBIC) ? 2 : 1;
     EncodeTiledFn enc = get_encode();
-    static const bool no_stage = std::getenv("DFR_NO_STAGE") != nullptr;   // debugging / A-B timing only
+    bool no_stage = false;
+    int bw_align = 4;
+#ifdef DFR_DEV_HOOKS                                                 // A-B timing builds only (never the shipped library)
+    no_stage = std::getenv("DFR_NO_STAGE") != nullptr;
+    if (const char *a = std::getenv("DFR_BW_ALIGN")) bw_align = std::atoi(a);
+#endif
     if (!no_stage && enc && (snx % 4 == 0) && ((uintptr_t)src % 16 == 0) && probe_extent(tgt, srchost, n, ony, onx, ex, ey)) {
         // floor-range spread + taps + 1 px safety each side; + 3: the origin is rounded down
         // to a multiple of 4 floats; then the width itself is rounded up to 16 bytes
-        const int bw = ((int)std::ceil(ex * 1.02) + 2 + tlo + thi + 2 + 3 + 3) & ~3;
+        int bw = ((int)std::ceil(ex * 1.02) + 2 + tlo + thi + 2 + 3 + 3) & ~3;
+        bw = (bw + bw_align - 1) / bw_align * bw_align;
         const int bh = (int)std::ceil(ey * 1.02) + 2 + tlo + thi + 2;
         if (bw <= 256 && bh <= 256 && (size_t)bw * bh * sizeof(float) <= (size_t)kMaxBoxBytes) {
             const cuuint64_t dims[3] = {(cuuint64_t)snx, (cuuint64_t)sny, (cuuint64_t)n};

@@ -75,6 +75,9 @@ def parity(w, order, out, exposures):
             "nan_frac": float(np.mean(nan)), "mask_diff_in_edge_band": band, "exposures_checked": list(exposures)}
 
 
+PROFILE_RUNS = 0        # --profile-runs N: N plain launches per case, nothing else (for ncu captures)
+
+
 def device_case(name, w, order, exposures, flush, oracle_exposures=1):
     src = torch.from_numpy(w.images).cuda()
     n = len(w.src_wcs)
@@ -84,6 +87,13 @@ def device_case(name, w, order, exposures, flush, oracle_exposures=1):
     def step():
         P.dfr_reproject(src, ws, tw, w.shape_out, order, out=out)
 
+    if PROFILE_RUNS:
+        for _ in range(PROFILE_RUNS):
+            if flush is not None:
+                flush.fill_(1.0)
+            step()
+        torch.cuda.synchronize()
+        return {"config": name, "order": ORDER_NAME[order], "profile_runs": PROFILE_RUNS, "tiles": P.dfr_last_stats()}
     med, best = time_gpu(step, flush)
     P.dfr_profile_enable(True)
     km = []
@@ -171,7 +181,18 @@ def main():
     ap.add_argument("--c4-exposures", type=int, default=1024)
     ap.add_argument("--c4-images", type=int, default=128)
     ap.add_argument("--skip", default="")
+    ap.add_argument("--only", default="", help="comma list of c0..c4: run only these")
+    ap.add_argument("--orders", default="0,1,3", help="interpolation orders of the C3 rows")
+    ap.add_argument("--profile-runs", type=int, default=0,
+                    help="N plain launches per device case and nothing else (no parity, no timing): the command "
+                         "ncu captures are taken from")
     args = ap.parse_args()
+    if args.only:
+        args.skip = ",".join(c for c in ("c0", "c1", "c2", "c3", "c4") if c not in args.only.split(","))
+    global PROFILE_RUNS
+    PROFILE_RUNS = args.profile_runs
+    if PROFILE_RUNS:
+        args.skip += ",c4"
     P.lib()
     oracle.build()
     assert torch.cuda.is_available()
@@ -185,7 +206,7 @@ def main():
         rows.append(device_case("C2", S.config2(), 1, [0, 13, 31], None, oracle_exposures=4))
     if "c3" not in args.skip:
         w3 = S.config3()
-        for o in (0, 1, 3):
+        for o in (int(t) for t in args.orders.split(",")):
             rows.append(device_case("C3", w3, o, [0], flush))
     for r in rows:
         print(json.dumps(r), flush=True)
@@ -193,6 +214,8 @@ def main():
     if "c4" not in args.skip:
         c4 = stream_case(args.c4_exposures, args.c4_images)
         print(json.dumps(c4), flush=True)
+    if PROFILE_RUNS:
+        return
     os.makedirs(os.path.dirname(args.out), exist_ok=True)
     with open(args.out + ".json", "w") as f:
         json.dump({"device": rows, "stream": c4, "hbm_peak_gbs": hbm_peak()}, f, indent=1)

@@ -32,7 +32,12 @@ def test_headline_line():
     assert d["config"]["workload"].startswith("configs[2]") and "model" not in d["config"]
     r = d["roofline"]
     assert r["bound"] == "hbm" and 0.3 < r["frac"] < 1.2 and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
-    assert r["traffic"] and 0.8 < r["traffic"] / r["algorithmic_bytes_per_launch"] < 1.2
+    # traffic comes from the tracked ncu capture; null (with the reason) when the kernel sources changed since
+    assert r["traffic"] is None or 0.8 < r["traffic"] / r["algorithmic_bytes_per_launch"] < 1.2
+    assert r["traffic"] is not None or r["traffic_source"]
+    # 4 B per output pixel + 4 B per unique source pixel touched <= 8 B per output pixel
+    assert 0.85 * r["upper_bound_bytes_per_launch"] < r["algorithmic_bytes_per_launch"] <= r["upper_bound_bytes_per_launch"]
+    assert r["frac"] <= r["frac_upper"] and r["frac_whole_call"] < r["frac"]
     assert d["gpu_launches"] == 3 * d["steps"] and d["value"] > 1e5
     e = d["e2e"]
     assert e["h2d_bytes_per_step"] == 32 * 2048 * 2048 * 4 == e["d2h_bytes_per_step"] and e["matches_device_path"]
@@ -46,7 +51,7 @@ def test_stack_line():
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     d = run("--mode", "stack", "--steps", "3", "--warmup", "3")
-    assert BASE_KEYS <= set(d) and d["roofline"]["kernel"] == "tiled_stack_kernel"
+    assert BASE_KEYS <= set(d) and d["roofline"]["kernel"].startswith("tiled_stack_kernel")
     assert 20.0 < d["config"]["depth_mean"] <= 32.0
 
 

@@ -168,18 +168,20 @@ def test_sip_order_9(P):
 
 def test_config2_batch_full_size(P):
     """configs[2] at full size in the launch configuration bench.py times (batch 32 in one
-    call): three exposures element by element, plus 40 000 sampled pixels over all 32
-    computed one by one by the oracle."""
+    call): ALL 32 exposures element by element (mask + values, tests/parity.py), plus 40 000
+    sampled pixels computed one by one through the oracle's sky entry points
+    (pix2world -> world2pix -> interp: a second route through the oracle)."""
     w = S.config2()
     out = run_gpu(P, w, 1, 0)
     st = P.dfr_last_stats()
     sny, snx = w.images.shape[1:]
-    fr = []
-    for e in (0, 13, 31):
+    fr, worst = [], 0.0
+    for e in range(32):
         xo, yo = oracle.src_coords(w.tgt_wcs, w.src_wcs[e], *w.shape_out)
         ref = oracle.interp(w.images[e], xo.ravel(), yo.ravel(), 1).reshape(w.shape_out).astype(np.float32)
         r = PR.check_image(out[e], ref, xo, yo, w.images[e], 1)
         fr.append(r["nan_frac"])
+        worst = max(worst, r["max"] / r["dr"])
     assert 0.005 < np.mean(fr) < 0.12
     rng = np.random.default_rng(222)
     for e in range(32):
@@ -193,7 +195,7 @@ def test_config2_batch_full_size(P):
         assert np.array_equal(np.isnan(got)[~band], np.isnan(ref)[~band])
         ok = ~np.isnan(got) & ~np.isnan(ref)
         assert np.max(np.abs(got[ok] - ref[ok])) <= PR.VALUE_TOL * PR.dyn_range(w.images[e])
-    print("C2 stats", st)
+    print("C2 stats", st, "worst value error", worst, "x DR, mean NaN fraction", np.mean(fr))
 
 
 def test_config3_three_orders(P):
@@ -396,3 +398,69 @@ def test_paper_footprint_mode(P):
     assert np.array_equal(np.nan_to_num(n0, nan=-1), np.nan_to_num(n1, nan=-1))
     with pytest.raises(P.DfrError):
         P.dfr_reproject(d, [src], tgt, (ony, onx), 3, edge=P.EDGE_PAPER)
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+@pytest.mark.parametrize("order", [0, 1, 3])
+def test_nan_source_pixels_propagate(P, path, order):
+    """Reading G14: NaN pixels in the source propagate by IEEE through the taps read (and only
+    those). Blocks, lines and isolated NaN pixels, including on the image rim. Which taps are
+    read depends on floor(x) (rint for nearest), so the NaN mask is compared away from the
+    footprint edge AND away from coordinates within 2 x COORD_TOL of an integer (a half-integer
+    for nearest), where a legal coordinate difference changes the tap set."""
+    rng = np.random.default_rng(14)
+    sny, snx, ony, onx = 236, 300, 250, 270
+    img = S.make_image(sny, snx, 60, rng)
+    img[40:52, 60:90] = np.nan                      # a block
+    img[120, :] = np.nan                            # a row
+    img[:, 200] = np.nan                            # a column
+    img[0, 0] = img[sny - 1, snx - 1] = img[sny - 1, 10] = np.nan      # rim pixels (edge replication)
+    ys, xs = rng.integers(0, sny, 150), rng.integers(0, snx, 150)
+    img[ys, xs] = np.nan                            # isolated pixels
+    src = S.add_sip(S.make_wcs(snx, sny, 150.0, 2.0, 0.0, S.PIXSCALE), 3, snx / 2.0, rng, amp=1e-4)
+    tgt = S.add_sip(S.make_wcs(onx, ony, 150.002, 2.001, 9.0, S.PIXSCALE * 1.04), 3, onx / 2.0, rng, amp=1e-4)
+    out = P.dfr_reproject(torch.from_numpy(img[None]).cuda(), [src], tgt, (ony, onx), order,
+                          path=PATHS[path]).cpu().numpy()[0]
+    xo, yo = oracle.src_coords(tgt, src, ony, onx)
+    ref = oracle.interp(img, xo.ravel(), yo.ravel(), order).reshape(ony, onx)
+    inside = ~PR.edge_band(xo, yo, sny, snx) & np.isfinite(xo)
+    off = 0.5 if order == 0 else 0.0
+    fx, fy = xo - off - np.floor(xo - off), yo - off - np.floor(yo - off)
+    amb = (np.minimum(fx, 1 - fx) < PR.TIE_BAND) | (np.minimum(fy, 1 - fy) < PR.TIE_BAND)
+    cmp = inside & ~amb
+    mg, mo = np.isnan(out), np.isnan(ref)
+    assert np.array_equal(mg[cmp], mo[cmp]), f"{int((mg != mo)[cmp].sum())} NaN-propagation mismatches"
+    foot = np.isfinite(xo) & (xo >= -0.5) & (xo < snx - 0.5) & (yo >= -0.5) & (yo < sny - 0.5)
+    assert (mo & foot).sum() > 500 and (~mo).sum() > 0.5 * ony * onx     # NaNs inside the footprint exist
+    ok = ~mg & ~mo & cmp
+    assert np.abs(out[ok] - ref[ok]).max() <= PR.VALUE_TOL * PR.dyn_range(img)
+
+
+@pytest.mark.parametrize("fit_order", [3, 5])
+def test_fitted_inverse_sip_end_to_end(P, fit_order):
+    """§8(f) f4 end to end: a source WCS that carries only the forward SIP (A/B) gets AP/BP
+    from dfr_wcs_fit_inverse_sip; the reprojection through those coefficients must equal the
+    oracle fed the SAME fitted coefficients (coordinates, mask, values; all three orders)."""
+    rng = np.random.default_rng(65)
+    sny, snx, ony, onx = 400, 520, 410, 500
+    img = S.make_image(sny, snx, 120, rng)
+    src = S.make_wcs(snx, sny, 150.0, 2.0, 0.0, S.PIXSCALE)
+    src.a, src.b = S.draw_sip(4, snx / 2.0, rng, amp=3e-4)
+    src.a_order = src.b_order = 4                   # ~0.5 px distortion, no AP/BP
+    tgt = S.make_wcs(onx, ony, 150.003, 2.002, -6.0, S.PIXSCALE)
+    packed = P.pack_wcs(src)
+    resid = P.dfr_wcs_fit_inverse_sip(packed, fit_order, snx, sny)
+    assert 0.0 < resid < 0.2 and packed.ap_order == fit_order and packed.bp_order == fit_order
+    fitted = src.copy()
+    fitted.ap_order = fitted.bp_order = fit_order
+    fitted.ap = np.array(packed.ap[:]).reshape(10, 10)
+    fitted.bp = np.array(packed.bp[:]).reshape(10, 10)
+    assert np.abs(fitted.ap).max() > 0
+    w = S.Workload("f4", img[None], [fitted], tgt, (ony, onx), (0, 1, 3))
+    for path in PATHS.values():
+        rep, _ = full_parity(P, w, path)
+    # without the fitted inverse the coordinates differ by the distortion itself
+    xa, _ = oracle.src_coords(tgt, fitted, ony, onx)
+    xb, _ = oracle.src_coords(tgt, src, ony, onx)
+    assert np.nanmax(np.abs(xa - xb)) > 0.05
+    print("f4", fit_order, "fit residual", resid, rep[("coords", 0)])

@@ -100,34 +100,13 @@ def test_stack_accumulate_over_batches_and_nan_pixels(P):
 
 
 def test_stack_config2_full_size(P):
-    """configs[2] (32 x 2048^2 -> 2048^2) in the launch configuration bench.py --stack
-    times: wsum everywhere, sum on 60 000 sampled pixels computed one by one by the oracle."""
+    """configs[2] (32 x 2048^2 -> 2048^2) in the launch configuration bench.py --mode stack
+    times: the WHOLE sum and wsum frames against orc_stack, element by element."""
     w = S.config2()
-    src = torch.from_numpy(w.images).cuda()
-    s, ws = P.dfr_reproject_stack(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1)
-    torch.cuda.synchronize()
-    st = P.dfr_last_stats()
-    s, ws = s.cpu().numpy(), ws.cpu().numpy()
-    sny, snx = w.images.shape[1:]
-    rng = np.random.default_rng(333)
-    ii = rng.integers(0, 2048, 60000).astype(np.float64)
-    jj = rng.integers(0, 2048, 60000).astype(np.float64)
-    ra, dec = oracle.pix2world(w.tgt_wcs, ii, jj)
-    so, wo, band = np.zeros(ii.size), np.zeros(ii.size), np.zeros(ii.size, dtype=bool)
-    for e in range(32):
-        xo, yo = oracle.world2pix(w.src_wcs[e], ra, dec)
-        v = oracle.interp(w.images[e], xo, yo, 1)
-        ok = ~np.isnan(v)
-        so += np.where(ok, v, 0.0)
-        wo += ok
-        band |= PR.edge_band(xo, yo, sny, snx)
-    gs, gw = s[jj.astype(int), ii.astype(int)], ws[jj.astype(int), ii.astype(int)]
-    assert np.array_equal(gw[~band], wo[~band].astype(np.float32))
-    dr = max(PR.dyn_range(im) for im in w.images)
-    err = np.abs(gs[~band] - so[~band])
-    assert err.max() <= PR.VALUE_TOL * dr * 32
-    assert ws.max() == 32.0 and 20.0 < ws.mean() < 32.0
-    print("C2 stack", st, "max err", err.max(), "limit", PR.VALUE_TOL * dr * 32, "mean depth", ws.mean())
+    st = check_stack(P, w, 1)
+    stats = P.dfr_last_stats()
+    assert st["depth_max"] == 32.0
+    print("C2 stack", stats, st)
 
 
 def test_stack_unaligned_pitch_and_exact_tiles(P):
