@@ -78,7 +78,8 @@ typedef enum dfr_status {
     DFR_ERR_SINGULAR_CD = -5,    /* det(CD) == 0 or not finite                    */
     DFR_ERR_NONFINITE_WCS = -6,  /* NaN/Inf in crpix, crval, cd or used SIP terms */
     DFR_ERR_ALIAS = -7,          /* out overlaps src_batch                        */
-    DFR_ERR_CUDA = -8            /* CUDA runtime/driver failure (see dfr_last_error) */
+    DFR_ERR_CUDA = -8,           /* CUDA runtime/driver failure (see dfr_last_error) */
+    DFR_ERR_WEIGHT = -9          /* NaN/Inf in the stacking weights               */
 } dfr_status;
 
 /* Path selection for dfr_reproject_ex / dfr_src_coords_ex.
@@ -115,7 +116,24 @@ int dfr_reproject(const float *src_batch, int32_t n, int32_t src_ny, int32_t src
                   int32_t out_ny, int32_t out_nx, int32_t order,
                   float *out, void *stream);
 
-/* Same, with an explicit footprint rule (DFR_EDGE_*). */
+/* Same, with an explicit footprint rule (DFR_EDGE_*) and, optionally, the footprint array
+ * (PAPER.md:69: "simultaneously projecting an identity tensor called the footprint"; :27: a drop-in
+ * for reproject_interp, which returns (array, footprint)).
+ *   footprint : DEVICE float32 [n][out_ny][out_nx], or NULL. Must not overlap src_batch or out.
+ *               DFR_EDGE_PAPER with bilinear: the projected identity itself — the zero-padded
+ *               bilinear interpolation of an all-ones image at the pixel's source coordinate:
+ *               1 on [0, n-1]^2, falling linearly to 0 at -1 and at n on each axis (product of
+ *               the two); `out` is valid exactly where it is > 0. Every other mode (AREA; PAPER
+ *               with nearest): 1 where the source coordinate lies in the footprint, else 0.
+ *               NaN pixels of the source do not change it: it describes geometry only.
+ * `out` is bit-identical with and without a footprint array (the footprint is written by a
+ * separate pass over the same per-tile coordinates). Errors as dfr_reproject. */
+int dfr_reproject_fp(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+                     const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                     int32_t out_ny, int32_t out_nx, int32_t order, int32_t edge_mode,
+                     float *out, float *footprint, void *stream);
+
+/* dfr_reproject_fp without a footprint array. */
 int dfr_reproject_edge(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
                        const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
                        int32_t out_ny, int32_t out_nx, int32_t order, int32_t edge_mode,
@@ -137,6 +155,21 @@ int dfr_reproject_host(const float *src_host, int32_t n, int32_t src_ny, int32_t
                        const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
                        int32_t out_ny, int32_t out_nx, int32_t order,
                        float *out_host, int32_t batch);
+
+/* The same over several devices of this node (exposures are
+ * independent). The n exposures are cut into ndev contiguous shards (dfr_shard_range); shard k
+ * runs the pipeline above on device devices[k] from its own host thread; there is no collective.
+ * A device may be listed more than once (two pipelines on it). Every listed device must be
+ * visible to the process. The calling thread's current device is left unchanged. */
+int dfr_reproject_host_multi(const float *src_host, int32_t n, int32_t src_ny, int32_t src_nx,
+                             const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                             int32_t out_ny, int32_t out_nx, int32_t order,
+                             float *out_host, int32_t batch, const int32_t *devices, int32_t ndev);
+
+/* The partition rule of the *_multi entry points: shard k of `parts` over n units is
+ * [*lo, *hi), contiguous, sizes differing by at most one (the first n % parts shards are the
+ * longer ones). HOST only. */
+int dfr_shard_range(int32_t n, int32_t parts, int32_t k, int32_t *lo, int32_t *hi);
 
 /* ---- fused reproject-and-stack --------- */
 
@@ -172,6 +205,16 @@ int dfr_stack_host(const float *src_host, int32_t n, int32_t src_ny, int32_t src
                    const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
                    int32_t out_ny, int32_t out_nx, int32_t order, const float *weights,
                    float *sum_host, float *wsum_host, int32_t batch);
+
+/* dfr_stack_host over several devices: every shard (as dfr_reproject_host_multi) co-adds its
+ * exposures into a sum / wsum pair on its own device; the one exchange step of the path follows:
+ * the partial pairs are copied to the first shard's device (peer copy) and added there in shard
+ * order, so the result does not depend on timing between devices. */
+int dfr_stack_host_multi(const float *src_host, int32_t n, int32_t src_ny, int32_t src_nx,
+                         const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                         int32_t out_ny, int32_t out_nx, int32_t order, const float *weights,
+                         float *sum_host, float *wsum_host, int32_t batch,
+                         const int32_t *devices, int32_t ndev);
 
 /* mean[k] = sum[k] / wsum[k], NaN where wsum[k] == 0. DEVICE float32[npix] each;
  * mean may be the same array as sum. */
@@ -226,6 +269,27 @@ int dfr_last_stats(int64_t stats[4]);
  * (per-tile fit), ms[1] = main reprojection kernel. */
 int dfr_profile_enable(int on);
 int dfr_profile_last(float ms[2]);
+
+/* What the library keeps between calls, per device: a private cudaMemPool for stream-ordered
+ * scratch (the application's default pool is never touched), per host thread a few KB of pinned
+ * staging memory, three events and 16 bytes of mapped counters, and — after a *_host call — the
+ * pipeline's device buffers (3 x batch x (input + output frames)), reused by later calls.
+ * dfr_release() synchronises the CURRENT device, frees the calling thread's state for it, every
+ * idle pipeline on it, and trims the scratch pool. Safe to call at any time between calls. */
+int dfr_release(void);
+
+/* Register-only instruction-rate probes (the ALU side of the roofline wants
+ * MEASURED denominators). Runs one short kernel per class on the current device, every SM
+ * loaded with 32 warps of independent chains, and writes into out[k] (HOST, n >=
+ * DFR_PROBE_COUNT entries, k = DFR_PROBE_*) the thread-level INSTRUCTIONS retired per clock
+ * per SM; a packed FFMA2 counts as one instruction (two fp32 FMAs). The three mixed classes
+ * interleave two instruction kinds 1:1 and report their combined instruction rate: a rate
+ * above either kind alone means the two do not share a pipe. Synchronous; ~50 ms. */
+enum { DFR_PROBE_FFMA = 0, DFR_PROBE_FFMA2 = 1, DFR_PROBE_FADD2_RM = 2, DFR_PROBE_DFMA = 3,
+       DFR_PROBE_IMAD = 4, DFR_PROBE_LOP3 = 5, DFR_PROBE_LDS = 6,
+       DFR_PROBE_FFMA_FFMA2 = 7, DFR_PROBE_FFMA2_IMAD = 8, DFR_PROBE_FFMA2_LOP3 = 9,
+       DFR_PROBE_COUNT = 10 };
+int dfr_probe_rates(double *out, int32_t n);
 
 const char *dfr_strerror(int code);
 const char *dfr_last_error(void);

@@ -20,10 +20,11 @@ PATH_AUTO, PATH_EXACT, PATH_TILED = 0, 1, 2
 EDGE_AREA, EDGE_PAPER = 0, 1
 _ORDER_NAMES = {"nearest": 0, "nearest-neighbor": 0, "bilinear": 1, "bicubic": 3}
 
-EXPORTS = ["dfr_reproject", "dfr_reproject_edge", "dfr_reproject_ex", "dfr_reproject_host", "dfr_reproject_stack",
-           "dfr_stack_finalize", "dfr_stack_host", "dfr_pix2world",
+EXPORTS = ["dfr_reproject", "dfr_reproject_edge", "dfr_reproject_ex", "dfr_reproject_fp", "dfr_reproject_host",
+           "dfr_reproject_host_multi", "dfr_reproject_stack", "dfr_shard_range", "dfr_release",
+           "dfr_stack_finalize", "dfr_stack_host", "dfr_stack_host_multi", "dfr_pix2world",
            "dfr_world2pix", "dfr_src_coords", "dfr_wcs_set_pc_cdelt", "dfr_wcs_fit_inverse_sip", "dfr_last_stats",
-           "dfr_profile_enable", "dfr_profile_last",
+           "dfr_profile_enable", "dfr_profile_last", "dfr_probe_rates",
            "dfr_strerror", "dfr_last_error", "dfr_version"]
 
 
@@ -58,7 +59,13 @@ def lib():
         L.dfr_reproject.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, vp]
         L.dfr_reproject_ex.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, vp, i32]
         L.dfr_reproject_edge.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, i32, fp, vp]
+        L.dfr_reproject_fp.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, i32, fp, fp, vp]
         L.dfr_reproject_host.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, i32]
+        L.dfr_reproject_host_multi.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, i32, C.POINTER(i32), i32]
+        L.dfr_stack_host_multi.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, C.POINTER(C.c_float), fp, fp, i32,
+                                           C.POINTER(i32), i32]
+        L.dfr_shard_range.argtypes = [i32, i32, i32, C.POINTER(i32), C.POINTER(i32)]
+        L.dfr_release.argtypes = []
         L.dfr_reproject_stack.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32,
                                           C.POINTER(C.c_float), fp, fp, i32, vp]
         L.dfr_stack_finalize.argtypes = [fp, fp, i64, fp, vp]
@@ -71,6 +78,7 @@ def lib():
         L.dfr_last_stats.argtypes = [C.POINTER(C.c_int64)]
         L.dfr_profile_enable.argtypes = [C.c_int]
         L.dfr_profile_last.argtypes = [C.POINTER(C.c_float)]
+        L.dfr_probe_rates.argtypes = [C.POINTER(C.c_double), i32]
         L.dfr_strerror.argtypes = [C.c_int]
         L.dfr_strerror.restype = C.c_char_p
         L.dfr_last_error.restype = C.c_char_p
@@ -131,10 +139,11 @@ def _need_cuda(t, dtype, name):
 
 
 def dfr_reproject(src_batch, src_wcs, tgt_wcs, shape_out=None, order=BILINEAR, out=None,
-                  stream=None, path=PATH_AUTO, edge=EDGE_AREA):
-    """dfr_reproject / dfr_reproject_ex (include/dfr.h). src_batch: CUDA float32
+                  stream=None, path=PATH_AUTO, edge=EDGE_AREA, footprint=None):
+    """dfr_reproject / dfr_reproject_ex / dfr_reproject_fp (include/dfr.h). src_batch: CUDA float32
     [n][ny][nx] (or [ny][nx]); returns the CUDA float32 [n][out_ny][out_nx] output.
-    shape_out defaults to the input shape."""
+    shape_out defaults to the input shape. footprint=True (or a CUDA float32
+    tensor of the output's shape) also returns the footprint array: (out, footprint)."""
     import torch
     if src_batch.dim() == 2:
         src_batch = src_batch[None]
@@ -150,22 +159,30 @@ def dfr_reproject(src_batch, src_wcs, tgt_wcs, shape_out=None, order=BILINEAR, o
     _need_cuda(out, torch.float32, "out")
     if tuple(out.shape) != (n, ony, onx):
         raise ValueError("out has the wrong shape")
+    fp_t = None
+    if footprint is not None and footprint is not False:
+        fp_t = torch.empty_like(out) if footprint is True else footprint
+        _need_cuda(fp_t, torch.float32, "footprint")
+        if tuple(fp_t.shape) != (n, ony, onx):
+            raise ValueError("footprint has the wrong shape")
     with torch.cuda.device(src_batch.device):
-        if edge != EDGE_AREA:
+        if edge != EDGE_AREA or fp_t is not None:
             if path != PATH_AUTO:
-                raise ValueError("an explicit path and an explicit edge rule cannot be combined")
-            _check(lib().dfr_reproject_edge(src_batch.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx,
-                                            _order(order), int(edge), out.data_ptr(), _stream_ptr(stream)))
+                raise ValueError("an explicit path cannot be combined with an explicit edge rule or a footprint array")
+            _check(lib().dfr_reproject_fp(src_batch.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx,
+                                          _order(order), int(edge), out.data_ptr(),
+                                          fp_t.data_ptr() if fp_t is not None else None, _stream_ptr(stream)))
         else:
             _check(lib().dfr_reproject_ex(src_batch.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx,
                                           _order(order), out.data_ptr(), _stream_ptr(stream), int(path)))
-    return out
+    return out if fp_t is None else (out, fp_t)
 
 
 def dfr_reproject_host(src_host, src_wcs, tgt_wcs, shape_out=None, order=BILINEAR, out_host=None,
-                       batch=32):
+                       batch=32, devices=None):
     """dfr_reproject_host: HOST float32 arrays (numpy, or CPU torch tensors — pinned
-    for full PCIe rate) in and out; copies and kernels are pipelined inside the library."""
+    for full PCIe rate) in and out; copies and kernels are pipelined inside the library.
+    devices=[0, 1, ...] shards the exposures over several GPUs (dfr_reproject_host_multi)."""
     import torch
     src_t = torch.as_tensor(src_host)
     if src_t.dim() == 2:
@@ -175,6 +192,8 @@ def dfr_reproject_host(src_host, src_wcs, tgt_wcs, shape_out=None, order=BILINEA
     n, sny, snx = src_t.shape
     ony, onx = (sny, snx) if shape_out is None else (int(shape_out[0]), int(shape_out[1]))
     ws = pack_wcs_array(src_wcs)
+    if len(ws) != n:
+        raise ValueError("one source WCS per exposure")
     tw = pack_wcs(tgt_wcs)
     if out_host is None:
         out_host = torch.empty((n, ony, onx), dtype=torch.float32, pin_memory=True)
@@ -182,8 +201,13 @@ def dfr_reproject_host(src_host, src_wcs, tgt_wcs, shape_out=None, order=BILINEA
     if out_t.is_cuda or out_t.dtype != torch.float32 or not out_t.is_contiguous() \
             or tuple(out_t.shape) != (n, ony, onx):
         raise ValueError("out_host must be a contiguous float32 host array [n][ny][nx]")
-    _check(lib().dfr_reproject_host(src_t.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx,
-                                    _order(order), out_t.data_ptr(), int(batch)))
+    if devices is None:
+        _check(lib().dfr_reproject_host(src_t.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx,
+                                        _order(order), out_t.data_ptr(), int(batch)))
+    else:
+        dv = (C.c_int32 * len(devices))(*[int(d) for d in devices])
+        _check(lib().dfr_reproject_host_multi(src_t.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx,
+                                              _order(order), out_t.data_ptr(), int(batch), dv, len(devices)))
     return out_host
 
 
@@ -223,7 +247,7 @@ def dfr_reproject_stack(src_batch, src_wcs, tgt_wcs, shape_out=None, order=BILIN
     return sum, wsum
 
 
-def dfr_stack_host(src_host, src_wcs, tgt_wcs, shape_out=None, order=BILINEAR, weights=None, batch=32):
+def dfr_stack_host(src_host, src_wcs, tgt_wcs, shape_out=None, order=BILINEAR, weights=None, batch=32, devices=None):
     """dfr_stack_host: HOST float32 exposures in (pinned for full PCIe rate), HOST (sum, wsum)
     float32 [out_ny][out_nx] out; uploads and the stacking kernels are pipelined in the library."""
     import torch
@@ -246,8 +270,13 @@ def dfr_stack_host(src_host, src_wcs, tgt_wcs, shape_out=None, order=BILINEAR, w
         wp = w.ctypes.data_as(C.POINTER(C.c_float))
     s = torch.empty((ony, onx), dtype=torch.float32, pin_memory=True)
     c = torch.empty((ony, onx), dtype=torch.float32, pin_memory=True)
-    _check(lib().dfr_stack_host(src_t.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx, _order(order), wp,
-                                s.data_ptr(), c.data_ptr(), int(batch)))
+    if devices is None:
+        _check(lib().dfr_stack_host(src_t.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx, _order(order), wp,
+                                    s.data_ptr(), c.data_ptr(), int(batch)))
+    else:
+        dv = (C.c_int32 * len(devices))(*[int(d) for d in devices])
+        _check(lib().dfr_stack_host_multi(src_t.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx, _order(order), wp,
+                                          s.data_ptr(), c.data_ptr(), int(batch), dv, len(devices)))
     return s, c
 
 
@@ -339,6 +368,28 @@ def dfr_profile_last():
     ms = (C.c_float * 2)()
     _check(lib().dfr_profile_last(ms))
     return float(ms[0]), float(ms[1])
+
+
+PROBE_NAMES = ["FFMA", "FFMA2", "FADD2.RM", "DFMA", "IMAD", "LOP3", "LDS", "FFMA+FFMA2", "FFMA2+IMAD", "FFMA2+LOP3"]
+
+
+def dfr_probe_rates() -> dict:
+    """dfr_probe_rates: thread-level instructions per clock per SM for each probe class."""
+    out = (C.c_double * len(PROBE_NAMES))()
+    _check(lib().dfr_probe_rates(out, len(PROBE_NAMES)))
+    return dict(zip(PROBE_NAMES, [float(v) for v in out]))
+
+
+def dfr_shard_range(n: int, parts: int, k: int):
+    """dfr_shard_range: [lo, hi) of shard k of `parts` over n units (the *_multi partition rule)."""
+    lo, hi = C.c_int32(0), C.c_int32(0)
+    _check(lib().dfr_shard_range(int(n), int(parts), int(k), C.byref(lo), C.byref(hi)))
+    return int(lo.value), int(hi.value)
+
+
+def dfr_release():
+    """dfr_release: free what the library keeps for the current device (include/dfr.h)."""
+    _check(lib().dfr_release())
 
 
 def dfr_version() -> int:

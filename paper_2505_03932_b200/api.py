@@ -124,27 +124,42 @@ def _groups(arrays):
 
 
 def calculate_reprojection(source_hdus, target_wcs, shape_out=None, order="bilinear", device="cuda",
-                           return_torch=False):
+                           return_torch=False, return_footprint=False, paper_footprint=False):
     """PAPER.md:30-36. source_hdus: one HDU-like / (array, header) pair, or a list of them
     (each with its own WCS); target_wcs: header mapping, WCS-like object or
     DfrWCS; shape_out defaults to the input shape; order: 'nearest',
     'bilinear', 'bicubic'. Returns [ny][nx] for one source, [n][ny][nx] for a list; pixels
-    outside a source's footprint are NaN."""
+    outside a source's footprint are NaN. return_footprint=True returns (array, footprint)
+    like reproject_interp: 1 inside the footprint, 0 outside; with
+    paper_footprint=True (nearest / bilinear) the footprint rule is the paper's literal one
+    (the projected identity, valid on (-1, n)) and the array is that identity."""
     import torch
+    from . import EDGE_AREA, EDGE_PAPER
     single, arrays, wcs = _gather(source_hdus)
     shape_out = tuple(arrays[0].shape) if shape_out is None else (int(shape_out[0]), int(shape_out[1]))
     tgt = _as_wcs(target_wcs, shape_out)
+    edge = EDGE_PAPER if paper_footprint else EDGE_AREA
     out = torch.empty((len(arrays),) + shape_out, dtype=torch.float32, device=device)
+    foot = torch.empty_like(out) if return_footprint else None
     for idx in _groups(arrays):                     # sources may differ in shape (PAPER.md:32)
         src = torch.from_numpy(np.stack([arrays[k] for k in idx])).to(device)
-        res = dfr_reproject(src, [wcs[k] for k in idx], tgt, shape_out, order)
+        res = dfr_reproject(src, [wcs[k] for k in idx], tgt, shape_out, order, edge=edge,
+                            footprint=True if return_footprint else None)
+        res, fp = res if return_footprint else (res, None)
         if len(idx) == len(arrays):
-            out = res
+            out, foot = res, fp
         else:
-            out[torch.as_tensor(idx, device=device)] = res
+            sel = torch.as_tensor(idx, device=device)
+            out[sel] = res
+            if return_footprint:
+                foot[sel] = fp
     if single:
         out = out[0]
-    return out if return_torch else out.cpu().numpy()
+        foot = foot[0] if return_footprint else None
+    if not return_torch:
+        out = out.cpu().numpy()
+        foot = foot.cpu().numpy() if return_footprint else None
+    return (out, foot) if return_footprint else out
 
 
 def calculate_stack(source_hdus, target_wcs, shape_out=None, order="bilinear", weights=None, device="cuda",

@@ -1,29 +1,21 @@
 // dfr_api.cu — the C ABI of include/dfr.h: argument validation, host
 // pre-composition, stream-ordered scratch, kernel launches. No compute happens
 // on the host beyond the O(n) per-exposure constant folding of dfr_host.cu.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <mutex>
+#include <string>
+#include <thread>
 #include <vector>
 
+#include "dfr_context.h"
 #include "dfr_internal.h"
 #include "dfr_tiled.h"
 
 namespace dfr {
 const char *last_error_cstr();
-
-static std::once_flag g_pool_once;
-static void tune_pool()
-{
-    // keep stream-ordered scratch cached between calls (no OS round trip per call)
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return;
-    cudaMemPool_t pool;
-    if (cudaDeviceGetDefaultMemPool(&pool, dev) != cudaSuccess) return;
-    uint64_t thr = UINT64_MAX;
-    cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
-}
 
 static int check_common(int32_t n, int32_t sny, int32_t snx, const dfr_wcs *sw, const dfr_wcs *tw,
                         int32_t ony, int32_t onx, int32_t order)
@@ -47,136 +39,419 @@ static int check_common(int32_t n, int32_t sny, int32_t snx, const dfr_wcs *sw, 
     return DFR_OK;
 }
 
-// Per-thread record of the last call: tile counters land in pinned host memory through an
-// async copy; dfr_last_stats waits for it. Also the optional timing events (dfr_profile_*).
+static int check_weights(const float *weights, int32_t n)
+{
+    for (int32_t e = 0; weights && e < n; ++e)
+        if (!std::isfinite(weights[e])) { set_error("weights[%d] is not finite", e); return DFR_ERR_WEIGHT; }
+    return DFR_OK;
+}
+
+static bool overlaps(const void *a, size_t na, const void *b, size_t nb)
+{
+    const char *a0 = (const char *)a, *b0 = (const char *)b;
+    return a0 < b0 + nb && b0 < a0 + na;
+}
+
+// ---- per-thread record of the last call (dfr_last_stats, dfr_profile_*) ----------------------
+// The tile counters land in mapped host memory of the device the call ran on (DevCtx);
+// dfr_last_stats waits for that device's `done` event.
 struct LastCall {
-    int32_t *pinned = nullptr;          // 3 counters: fast, exact, empty (mapped host memory,
-    int32_t *pinned_dev = nullptr;      // written by the setup kernel through this device pointer)
-    cudaEvent_t done = nullptr;
+    DevCtx *ctx = nullptr;
     bool pending = false;
     int64_t kernels = 0;
     bool tiled = false;
-    ProfileEvents prof = {nullptr, nullptr, nullptr, false};
 };
 static thread_local LastCall g_last;
-static thread_local int64_t g_stats_acc[4] = {0, 0, 0, 0};   // used by dfr_reproject_host
-static thread_local bool g_accumulate = false;
-static thread_local int32_t *g_stream_totals = nullptr;      // DEVICE int[3]: tile totals of a streaming call
+static thread_local bool g_profile = false;                   // dfr_profile_enable (per host thread)
+static thread_local int64_t g_stats_acc[4] = {0, 0, 0, 0};    // totals of a streaming call
+static thread_local bool g_accumulate = false;                // inside a streaming call
 
 // Streaming calls (dfr_reproject_host, dfr_stack_host): the batches add their tile counters
 // into one device array (no host wait between batches); harvested once at the end.
-static cudaError_t stream_stats_begin()
+static cudaError_t stream_stats_begin(DevCtx *c)
 {
     cudaError_t err;
-    if (!g_stream_totals && (err = cudaMalloc((void **)&g_stream_totals, 4 * sizeof(int32_t))) != cudaSuccess) return err;
-    if ((err = cudaMemset(g_stream_totals, 0, 4 * sizeof(int32_t))) != cudaSuccess) return err;
+    if (!c->stream_totals && (err = cudaMalloc((void **)&c->stream_totals, 4 * sizeof(int32_t))) != cudaSuccess) return err;
+    if ((err = cudaMemset(c->stream_totals, 0, 4 * sizeof(int32_t))) != cudaSuccess) return err;
     for (int k = 0; k < 4; ++k) g_stats_acc[k] = 0;
     g_last.pending = false;
     g_accumulate = true;
     return cudaSuccess;
 }
 
-static void stream_stats_end()
+static void stream_stats_end(DevCtx *c)
 {
     g_accumulate = false;
     int32_t t[3] = {0, 0, 0};
-    if (cudaMemcpy(t, g_stream_totals, sizeof t, cudaMemcpyDeviceToHost) == cudaSuccess)
+    if (cudaMemcpy(t, c->stream_totals, sizeof t, cudaMemcpyDeviceToHost) == cudaSuccess)
         for (int k = 0; k < 3; ++k) g_stats_acc[k] = t[k];
     g_last.pending = false;
     g_last.kernels = -1;                 // marks "use the accumulated totals"
 }
 
-static int stack_impl(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
-                      const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs, int32_t out_ny, int32_t out_nx,
-                      int32_t order, const float *weights, float *sum, float *wsum, int32_t accumulate,
-                      cudaStream_t st);
+// ---- per-call constants -------------------------------------------------------------------
+// Host constants -> one stream-ordered device block [SourceDev x n | float weights x n], staged
+// through the thread's pinned ring (dfr_context.h) so the upload never blocks the host. `hsrc`
+// stays valid until kRingSlots - 1 further calls on this thread and device: long enough for the
+// launchers, which read it for the staging decision only.
+struct CallConsts {
+    TargetDev tgt;
+    const SourceDev *hsrc = nullptr;
+    SourceDev *dsrc = nullptr;
+    float *dweights = nullptr;
+    void *block = nullptr;
+    void release(cudaStream_t st) { if (block) cudaFreeAsync(block, st); block = nullptr; }
+};
 
-static cudaError_t ensure_last()
+static int upload_consts(DevCtx *c, int32_t n, const dfr_wcs *sw, const dfr_wcs *tw, bool with_weights,
+                         const float *weights, cudaStream_t st, CallConsts &K)
 {
-    cudaError_t err;
-    if (!g_last.pinned) {
-        if ((err = cudaHostAlloc((void **)&g_last.pinned, 4 * sizeof(int32_t), cudaHostAllocMapped)) != cudaSuccess) return err;
-        if ((err = cudaHostGetDevicePointer((void **)&g_last.pinned_dev, g_last.pinned, 0)) != cudaSuccess) return err;
-    }
-    if (!g_last.done && (err = cudaEventCreateWithFlags(&g_last.done, cudaEventDisableTiming)) != cudaSuccess) return err;
-    return cudaSuccess;
-}
-
-static void collect_stats(int64_t out[4])
-{
-    out[0] = out[1] = out[2] = 0;
-    out[3] = g_last.kernels;
-    if (g_last.tiled && g_last.pending) {
-        cudaEventSynchronize(g_last.done);
-        out[0] = g_last.pinned[0];
-        out[1] = g_last.pinned[1];
-        out[2] = g_last.pinned[2];
-    } else if (!g_last.tiled) {
-        out[1] = -1;                                          // exact path: no tiles
-    }
-}
-
-// Host constants -> device scratch (stream-ordered). Caller frees with cudaFreeAsync.
-static int upload_sources(int32_t n, const dfr_wcs *sw, const dfr_wcs *tw, cudaStream_t st,
-                          std::vector<SourceDev> &h, SourceDev **dev_out)
-{
-    h.resize((size_t)n);
+    make_target(tw, &K.tgt);
+    const size_t b_src = sizeof(SourceDev) * (size_t)n, bytes = b_src + (with_weights ? sizeof(float) * (size_t)n : 0);
+    PinnedSlot *slot = nullptr;
+    cudaError_t err = stage_acquire(c, bytes, &slot);
+    if (err != cudaSuccess) return cuda_fail(err, "pinned staging buffer");
+    SourceDev *h = static_cast<SourceDev *>(slot->host);
     for (int32_t e = 0; e < n; ++e) make_source(tw, &sw[e], &h[e]);
-    SourceDev *d = nullptr;
-    cudaError_t err = cudaMallocAsync((void **)&d, sizeof(SourceDev) * (size_t)n, st);
-    if (err != cudaSuccess) return cuda_fail(err, "cudaMallocAsync(sources)");
-    // pageable source: the runtime stages the bytes before returning, so `h` may die
-    err = cudaMemcpyAsync(d, h.data(), sizeof(SourceDev) * (size_t)n, cudaMemcpyHostToDevice, st);
-    if (err != cudaSuccess) { cudaFreeAsync(d, st); return cuda_fail(err, "cudaMemcpyAsync(sources)"); }
-    *dev_out = d;
+    if (with_weights) {
+        float *hw = reinterpret_cast<float *>(static_cast<char *>(slot->host) + b_src);
+        for (int32_t e = 0; e < n; ++e) hw[e] = weights ? weights[e] : 1.0f;
+    }
+    if ((err = scratch_alloc(&K.block, bytes, st)) != cudaSuccess) return cuda_fail(err, "scratch allocation (constants)");
+    err = cudaMemcpyAsync(K.block, slot->host, bytes, cudaMemcpyHostToDevice, st);
+    if (err == cudaSuccess) err = stage_done(slot, st);
+    if (err != cudaSuccess) { K.release(st); return cuda_fail(err, "cudaMemcpyAsync(constants)"); }
+    K.hsrc = h;
+    K.dsrc = static_cast<SourceDev *>(K.block);
+    K.dweights = with_weights ? reinterpret_cast<float *>(static_cast<char *>(K.block) + b_src) : nullptr;
     return DFR_OK;
 }
 
+static bool tiled_grid_fits(int32_t ony) { return ((ony + TS * CTA_T - 1) / (TS * CTA_T)) <= 65535; }
+
 static int reproject_impl(const float *src, int32_t n, int32_t sny, int32_t snx,
                           const dfr_wcs *sw, const dfr_wcs *tw, int32_t ony, int32_t onx,
-                          int32_t order, float *out, cudaStream_t st, int32_t path, int32_t edge = DFR_EDGE_AREA)
+                          int32_t order, float *out, cudaStream_t st, int32_t path, int32_t edge = DFR_EDGE_AREA,
+                          float *foot = nullptr)
 {
-    std::call_once(g_pool_once, tune_pool);
+    DevCtx *c = nullptr;
+    cudaError_t err = current_ctx(&c);
+    if (err != cudaSuccess) return cuda_fail(err, "device context");
+    if (g_profile && (err = ensure_profile_events(c)) != cudaSuccess) return cuda_fail(err, "cudaEventCreate");
+    c->prof.enabled = g_profile;
     g_last.pending = false;
-    TargetDev tgt;
-    make_target(tw, &tgt);
-    std::vector<SourceDev> hsrc;
-    SourceDev *dsrc = nullptr;
-    int rc = upload_sources(n, sw, tw, st, hsrc, &dsrc);
+    g_last.ctx = c;
+    CallConsts K;
+    int rc = upload_consts(c, n, sw, tw, false, nullptr, st, K);
     if (rc != DFR_OK) return rc;
-    cudaError_t err;
     TiledStats ts = {0, 0, 0, 0};
-    if (path == DFR_PATH_EXACT) {
-        if (g_last.prof.enabled) cudaEventRecord(g_last.prof.setup_begin, st), cudaEventRecord(g_last.prof.main_begin, st);
-        err = launch_exact_reproject(src, n, sny, snx, tgt, dsrc, ony, onx, order, out, st, edge);
-        if (g_last.prof.enabled) cudaEventRecord(g_last.prof.main_end, st);
-        g_last.kernels = 1;
-        g_last.tiled = false;
+    // a grid taller than 65535 CTA tiles (out_ny > 4.19 M rows) does not fit the tiled launch
+    if (path == DFR_PATH_EXACT || !tiled_grid_fits(ony)) {
+        if (c->prof.enabled) cudaEventRecord(c->prof.setup_begin, st), cudaEventRecord(c->prof.main_begin, st);
+        err = launch_exact_reproject(src, n, sny, snx, K.tgt, K.dsrc, ony, onx, order, out, st, edge, foot);
+        if (c->prof.enabled) cudaEventRecord(c->prof.main_end, st);
+        if (g_accumulate) {
+            g_stats_acc[3] += 1;
+        } else {
+            g_last.kernels = 1;
+            g_last.tiled = false;
+        }
     } else {
-        err = ensure_last();
-        if (err == cudaSuccess)
-            err = launch_tiled_reproject(src, n, sny, snx, tgt, dsrc, hsrc.data(), ony, onx, order, out, st,
-                                         g_accumulate ? g_stream_totals : g_last.pinned_dev, g_accumulate ? 1 : 0,
-                                         &ts, &g_last.prof, edge);
+        err = launch_tiled_reproject(src, n, sny, snx, K.tgt, K.dsrc, K.hsrc, ony, onx, order, out, st,
+                                     g_accumulate ? c->stream_totals : c->pinned_dev, g_accumulate ? 1 : 0,
+                                     &ts, &c->prof, edge, foot);
         if (g_accumulate) {
             g_stats_acc[3] += ts.kernels;
         } else {
-            if (err == cudaSuccess) err = cudaEventRecord(g_last.done, st);
+            if (err == cudaSuccess) err = cudaEventRecord(c->done, st);
             g_last.kernels = ts.kernels;
             g_last.tiled = true;
             g_last.pending = (err == cudaSuccess);
         }
     }
-    cudaFreeAsync(dsrc, st);
+    K.release(st);
     if (err != cudaSuccess) return cuda_fail(err, "reproject launch");
     return DFR_OK;
 }
 
+// validated arguments -> constants, scratch, launches (stream-ordered)
+static int stack_impl(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+                      const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs, int32_t out_ny, int32_t out_nx,
+                      int32_t order, const float *weights, float *sum, float *wsum, int32_t accumulate,
+                      cudaStream_t st)
+{
+    if (!tiled_grid_fits(out_ny)) { set_error("out_ny %d is too tall for the stacking kernel", out_ny); return DFR_ERR_SHAPE; }
+    DevCtx *c = nullptr;
+    cudaError_t err = current_ctx(&c);
+    if (err != cudaSuccess) return cuda_fail(err, "device context");
+    if (g_profile && (err = ensure_profile_events(c)) != cudaSuccess) return cuda_fail(err, "cudaEventCreate");
+    c->prof.enabled = g_profile;
+    g_last.pending = false;
+    g_last.ctx = c;
+    CallConsts K;
+    int rc = upload_consts(c, n, src_wcs, tgt_wcs, true, weights, st, K);
+    if (rc != DFR_OK) return rc;
+    TiledStats ts = {0, 0, 0, 0};
+    err = launch_tiled_stack(src_batch, n, src_ny, src_nx, K.tgt, K.dsrc, K.hsrc, out_ny, out_nx, order,
+                             K.dweights, sum, wsum, accumulate != 0, st,
+                             g_accumulate ? c->stream_totals : c->pinned_dev, g_accumulate ? 1 : 0, &ts, &c->prof);
+    if (!g_accumulate && err == cudaSuccess) err = cudaEventRecord(c->done, st);
+    K.release(st);
+    if (g_accumulate) {
+        g_stats_acc[3] += ts.kernels;
+    } else {
+        g_last.kernels = ts.kernels;
+        g_last.tiled = true;
+        g_last.pending = (err == cudaSuccess);
+    }
+    if (err != cudaSuccess) return cuda_fail(err, "reproject_stack launch");
+    return DFR_OK;
+}
+
+// ---- host-buffer pipelines ----------------------------------------------
+// A pipeline = kSlots (stream, device input buffer, device output buffer) triples on one device:
+// H2D(b + 1) || kernels(b) || D2H(b - 1). Pipelines are kept between calls (their buffers are as
+// large as the largest batch seen) in a process-wide pool; a call borrows one per shard, so
+// concurrent calls, and two shards on one device, never share buffers. dfr_release frees the idle ones.
+namespace {
+struct Slot {
+    cudaStream_t st = nullptr;
+    float *din = nullptr, *dout = nullptr;
+    size_t in_bytes = 0, out_bytes = 0;
+};
+constexpr int kSlots = 3;
+struct HostPipe {
+    int dev = -1;
+    bool busy = false;
+    Slot slot[kSlots];
+};
+std::mutex g_pipe_mu;
+std::vector<HostPipe *> g_pipes;
+
+HostPipe *pipe_acquire(int dev)
+{
+    std::lock_guard<std::mutex> lock(g_pipe_mu);
+    for (HostPipe *p : g_pipes)
+        if (p->dev == dev && !p->busy) { p->busy = true; return p; }
+    HostPipe *p = new HostPipe;
+    p->dev = dev;
+    p->busy = true;
+    g_pipes.push_back(p);
+    return p;
+}
+
+void pipe_release(HostPipe *p)
+{
+    std::lock_guard<std::mutex> lock(g_pipe_mu);
+    p->busy = false;
+}
+
+void pipe_free_idle(int dev)
+{
+    std::lock_guard<std::mutex> lock(g_pipe_mu);
+    for (size_t k = 0; k < g_pipes.size();) {
+        HostPipe *p = g_pipes[k];
+        if (p->dev != dev || p->busy) { ++k; continue; }
+        for (Slot &s : p->slot) {
+            if (s.din) cudaFree(s.din);
+            if (s.dout) cudaFree(s.dout);
+            if (s.st) cudaStreamDestroy(s.st);
+        }
+        delete p;
+        g_pipes.erase(g_pipes.begin() + (long)k);
+    }
+}
+
+cudaError_t ensure_slot(Slot &s, size_t in_bytes, size_t out_bytes)
+{
+    cudaError_t err;
+    if (!s.st && (err = cudaStreamCreateWithFlags(&s.st, cudaStreamNonBlocking)) != cudaSuccess) return err;
+    if (s.in_bytes < in_bytes) {
+        if (s.din) cudaFree(s.din);
+        s.din = nullptr; s.in_bytes = 0;
+        if ((err = cudaMalloc((void **)&s.din, in_bytes)) != cudaSuccess) return err;
+        s.in_bytes = in_bytes;
+    }
+    if (s.out_bytes < out_bytes) {
+        if (s.dout) cudaFree(s.dout);
+        s.dout = nullptr; s.out_bytes = 0;
+        if ((err = cudaMalloc((void **)&s.dout, out_bytes)) != cudaSuccess) return err;
+        s.out_bytes = out_bytes;
+    }
+    return cudaSuccess;
+}
+
+// Borrowed pipeline of the current device with `used` slots sized for one batch.
+struct PipeLease {
+    HostPipe *p = nullptr;
+    DevCtx *ctx = nullptr;
+    int used = 0;
+    ~PipeLease() { if (p) pipe_release(p); }
+};
+
+int pipe_begin(PipeLease &L, int nb, size_t in_bytes, size_t out_bytes_slot0, size_t out_bytes_other)
+{
+    int dev = 0;
+    cudaError_t err = cudaGetDevice(&dev);
+    if (err == cudaSuccess) err = current_ctx(&L.ctx);
+    if (err != cudaSuccess) return cuda_fail(err, "device context");
+    L.p = pipe_acquire(dev);
+    L.used = nb < kSlots ? nb : kSlots;
+    for (int k = 0; k < L.used; ++k) {
+        err = ensure_slot(L.p->slot[k], in_bytes, k == 0 ? out_bytes_slot0 : out_bytes_other);
+        if (err != cudaSuccess) return cuda_fail(err, "pipeline buffers");
+    }
+    if ((err = stream_stats_begin(L.ctx)) != cudaSuccess) return cuda_fail(err, "stream statistics");
+    return DFR_OK;
+}
+
+int pipe_end(PipeLease &L, int rc)
+{
+    for (int k = 0; k < L.used; ++k) {
+        const cudaError_t err = cudaStreamSynchronize(L.p->slot[k].st);
+        if (err != cudaSuccess && rc == DFR_OK) rc = cuda_fail(err, "pipeline sync");
+    }
+    stream_stats_end(L.ctx);
+    return rc;
+}
+
+// dfr_reproject_host on the current device (arguments validated by the caller)
+int reproject_host_impl(const float *src_host, int32_t n, int32_t src_ny, int32_t src_nx,
+                        const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs, int32_t out_ny, int32_t out_nx,
+                        int32_t order, float *out_host, int32_t batch)
+{
+    const size_t in_px = (size_t)src_ny * src_nx, out_px = (size_t)out_ny * out_nx;
+    const int nb = (n + batch - 1) / batch;
+    PipeLease L;
+    int rc = pipe_begin(L, nb, in_px * batch * sizeof(float), out_px * batch * sizeof(float), out_px * batch * sizeof(float));
+    if (rc != DFR_OK) return rc;
+    for (int b = 0; b < nb; ++b) {
+        Slot &s = L.p->slot[b % kSlots];
+        const int32_t e0 = b * batch, ne = (n - e0 < batch) ? n - e0 : batch;
+        // slot reuse is ordered by the slot's own stream: H2D(b) waits for D2H(b - kSlots)
+        cudaError_t err = cudaMemcpyAsync(s.din, src_host + in_px * e0, in_px * ne * sizeof(float),
+                                          cudaMemcpyHostToDevice, s.st);
+        if (err != cudaSuccess) { rc = cuda_fail(err, "H2D"); break; }
+        rc = reproject_impl(s.din, ne, src_ny, src_nx, src_wcs + e0, tgt_wcs, out_ny, out_nx, order,
+                            s.dout, s.st, DFR_PATH_AUTO);
+        if (rc != DFR_OK) break;
+        err = cudaMemcpyAsync(out_host + out_px * e0, s.dout, out_px * ne * sizeof(float),
+                              cudaMemcpyDeviceToHost, s.st);
+        if (err != cudaSuccess) { rc = cuda_fail(err, "D2H"); break; }
+    }
+    return pipe_end(L, rc);
+}
+
+// dfr_stack_host on the current device: leaves sum | wsum in the pipeline's slot-0 output buffer
+// and copies them to sum_host / wsum_host unless `keep` is given (then *keep receives the device
+// pointer, valid until the lease `L` ends — the multi-device form reduces there).
+int stack_host_impl(PipeLease &L, const float *src_host, int32_t n, int32_t src_ny, int32_t src_nx,
+                    const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs, int32_t out_ny, int32_t out_nx,
+                    int32_t order, const float *weights, float *sum_host, float *wsum_host, int32_t batch,
+                    float **keep)
+{
+    const size_t in_px = (size_t)src_ny * src_nx, out_bytes = sizeof(float) * (size_t)out_ny * out_nx;
+    const int nb = (n + batch - 1) / batch;
+    // slot 0's output buffer holds sum and wsum; every slot needs an input buffer and a stream
+    int rc = pipe_begin(L, nb, in_px * batch * sizeof(float), 2 * out_bytes, 0);
+    if (rc != DFR_OK) return rc;
+    float *dsum = L.p->slot[0].dout, *dwsum = dsum + (size_t)out_ny * out_nx;
+    cudaEvent_t zeroed = nullptr;
+    cudaError_t err = cudaEventCreateWithFlags(&zeroed, cudaEventDisableTiming);
+    if (err == cudaSuccess) err = cudaMemsetAsync(dsum, 0, 2 * out_bytes, L.p->slot[0].st);
+    if (err == cudaSuccess) err = cudaEventRecord(zeroed, L.p->slot[0].st);
+    for (int k = 1; k < L.used && err == cudaSuccess; ++k) err = cudaStreamWaitEvent(L.p->slot[k].st, zeroed, 0);
+    if (err != cudaSuccess) rc = cuda_fail(err, "pipeline start");
+    for (int b = 0; b < nb && rc == DFR_OK; ++b) {
+        Slot &s = L.p->slot[b % kSlots];
+        const int32_t e0 = b * batch, ne = (n - e0 < batch) ? n - e0 : batch;
+        // the slot's stream orders its own reuse: H2D(b) waits for the kernels of b - kSlots;
+        // batches of different slots add into sum / wsum concurrently (atomic adds)
+        err = cudaMemcpyAsync(s.din, src_host + in_px * e0, in_px * ne * sizeof(float), cudaMemcpyHostToDevice, s.st);
+        if (err != cudaSuccess) { rc = cuda_fail(err, "H2D"); break; }
+        rc = stack_impl(s.din, ne, src_ny, src_nx, src_wcs + e0, tgt_wcs, out_ny, out_nx, order,
+                        weights ? weights + e0 : nullptr, dsum, dwsum, 1, s.st);
+    }
+    rc = pipe_end(L, rc);
+    if (zeroed) cudaEventDestroy(zeroed);
+    if (rc != DFR_OK) return rc;
+    if (keep) { *keep = dsum; return DFR_OK; }
+    err = cudaMemcpy(sum_host, dsum, out_bytes, cudaMemcpyDeviceToHost);
+    if (err == cudaSuccess) err = cudaMemcpy(wsum_host, dwsum, out_bytes, cudaMemcpyDeviceToHost);
+    return err == cudaSuccess ? DFR_OK : cuda_fail(err, "D2H");
+}
+
+// Contiguous shard k of n exposures over `parts` shards: the first n % parts shards get one more.
+void shard_range(int32_t n, int parts, int k, int32_t *lo, int32_t *hi)
+{
+    const int32_t q = n / parts, r = n % parts;
+    *lo = k * q + std::min(k, (int)r);
+    *hi = *lo + q + (k < r ? 1 : 0);
+}
+
+int check_devices(const int32_t *devices, int32_t ndev)
+{
+    if (!devices) { set_error("NULL device list"); return DFR_ERR_NULL; }
+    if (ndev < 1 || ndev > 64) { set_error("ndev = %d outside [1, 64]", ndev); return DFR_ERR_SHAPE; }
+    int count = 0;
+    const cudaError_t err = cudaGetDeviceCount(&count);
+    if (err != cudaSuccess) return cuda_fail(err, "cudaGetDeviceCount");
+    for (int k = 0; k < ndev; ++k)
+        if (devices[k] < 0 || devices[k] >= count) {
+            set_error("devices[%d] = %d, but %d CUDA device(s) are visible", k, devices[k], count);
+            return DFR_ERR_SHAPE;
+        }
+    return DFR_OK;
+}
+
+struct ShardResult {
+    int rc = DFR_OK;
+    std::string error;
+    int64_t stats[4] = {0, 0, 0, 0};
+};
+}  // namespace
 }  // namespace dfr
 
 using namespace dfr;
 
 extern "C" {
+
+int dfr_reproject_fp(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+                     const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                     int32_t out_ny, int32_t out_nx, int32_t order, int32_t edge_mode,
+                     float *out, float *footprint, void *stream)
+{
+    if (!src_batch || !out) { set_error("NULL image pointer"); return DFR_ERR_NULL; }
+    int rc = check_common(n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order);
+    if (rc != DFR_OK) return rc;
+    if (edge_mode != DFR_EDGE_AREA && edge_mode != DFR_EDGE_PAPER) {
+        set_error("unknown edge mode %d", edge_mode);
+        return DFR_ERR_ORDER;
+    }
+    if (edge_mode == DFR_EDGE_PAPER && order == DFR_BICUBIC) {
+        set_error("the paper's footprint normalisation is not defined for bicubic interpolation");
+        return DFR_ERR_ORDER;
+    }
+    const size_t sb = sizeof(float) * (size_t)n * src_ny * src_nx, ob = sizeof(float) * (size_t)n * out_ny * out_nx;
+    if (overlaps(out, ob, src_batch, sb)) { set_error("out overlaps src_batch"); return DFR_ERR_ALIAS; }
+    if (footprint && (overlaps(footprint, ob, src_batch, sb) || overlaps(footprint, ob, out, ob))) {
+        set_error("footprint overlaps src_batch or out");
+        return DFR_ERR_ALIAS;
+    }
+    // nearest: the zero-padded identity is 1 exactly on the area footprint
+    const int32_t edge = (order == DFR_NEAREST) ? DFR_EDGE_AREA : edge_mode;
+    return reproject_impl(src_batch, n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order,
+                          out, (cudaStream_t)stream, DFR_PATH_AUTO, edge, footprint);
+}
+
+int dfr_reproject_edge(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+                       const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                       int32_t out_ny, int32_t out_nx, int32_t order, int32_t edge_mode,
+                       float *out, void *stream)
+{
+    return dfr_reproject_fp(src_batch, n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order, edge_mode,
+                            out, nullptr, stream);
+}
 
 int dfr_reproject_ex(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
                      const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
@@ -190,36 +465,12 @@ int dfr_reproject_ex(const float *src_batch, int32_t n, int32_t src_ny, int32_t 
         set_error("unknown path %d", path);
         return DFR_ERR_ORDER;
     }
-    const char *s0 = (const char *)src_batch, *s1 = s0 + sizeof(float) * (size_t)n * src_ny * src_nx;
-    const char *o0 = (const char *)out, *o1 = o0 + sizeof(float) * (size_t)n * out_ny * out_nx;
-    if (o0 < s1 && s0 < o1) { set_error("out overlaps src_batch"); return DFR_ERR_ALIAS; }
+    if (overlaps(out, sizeof(float) * (size_t)n * out_ny * out_nx, src_batch, sizeof(float) * (size_t)n * src_ny * src_nx)) {
+        set_error("out overlaps src_batch");
+        return DFR_ERR_ALIAS;
+    }
     return reproject_impl(src_batch, n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order,
                           out, (cudaStream_t)stream, path);
-}
-
-int dfr_reproject_edge(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
-                       const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
-                       int32_t out_ny, int32_t out_nx, int32_t order, int32_t edge_mode,
-                       float *out, void *stream)
-{
-    if (!src_batch || !out) { set_error("NULL image pointer"); return DFR_ERR_NULL; }
-    int rc = check_common(n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order);
-    if (rc != DFR_OK) return rc;
-    if (edge_mode != DFR_EDGE_AREA && edge_mode != DFR_EDGE_PAPER) {
-        set_error("unknown edge mode %d", edge_mode);
-        return DFR_ERR_ORDER;
-    }
-    if (edge_mode == DFR_EDGE_PAPER && order == DFR_BICUBIC) {
-        set_error("the paper's footprint normalisation is not defined for bicubic interpolation");
-        return DFR_ERR_ORDER;
-    }
-    const char *s0 = (const char *)src_batch, *s1 = s0 + sizeof(float) * (size_t)n * src_ny * src_nx;
-    const char *o0 = (const char *)out, *o1 = o0 + sizeof(float) * (size_t)n * out_ny * out_nx;
-    if (o0 < s1 && s0 < o1) { set_error("out overlaps src_batch"); return DFR_ERR_ALIAS; }
-    // nearest: the zero-padded identity is 1 exactly on the area footprint
-    const int32_t edge = (order == DFR_NEAREST) ? DFR_EDGE_AREA : edge_mode;
-    return reproject_impl(src_batch, n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order,
-                          out, (cudaStream_t)stream, DFR_PATH_AUTO, edge);
 }
 
 int dfr_reproject(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
@@ -238,20 +489,18 @@ int dfr_src_coords(int32_t n, int32_t src_ny, int32_t src_nx,
     if (!x || !y) { set_error("NULL coordinate pointer"); return DFR_ERR_NULL; }
     int rc = check_common(n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order);
     if (rc != DFR_OK) return rc;
-    std::call_once(g_pool_once, tune_pool);
     cudaStream_t st = (cudaStream_t)stream;
-    TargetDev tgt;
-    make_target(tgt_wcs, &tgt);
-    SourceDev *dsrc = nullptr;
-    std::vector<SourceDev> hsrc;
-    rc = upload_sources(n, src_wcs, tgt_wcs, st, hsrc, &dsrc);
+    DevCtx *c = nullptr;
+    cudaError_t err = current_ctx(&c);
+    if (err != cudaSuccess) return cuda_fail(err, "device context");
+    CallConsts K;
+    rc = upload_consts(c, n, src_wcs, tgt_wcs, false, nullptr, st, K);
     if (rc != DFR_OK) return rc;
-    cudaError_t err;
-    if (path == DFR_PATH_EXACT)
-        err = launch_exact_coords(n, tgt, dsrc, out_ny, out_nx, x, y, st);
+    if (path == DFR_PATH_EXACT || !tiled_grid_fits(out_ny))
+        err = launch_exact_coords(n, K.tgt, K.dsrc, out_ny, out_nx, x, y, st);
     else
-        err = launch_tiled_coords(n, src_ny, src_nx, tgt, dsrc, hsrc.data(), out_ny, out_nx, order, x, y, st);
-    cudaFreeAsync(dsrc, st);
+        err = launch_tiled_coords(n, src_ny, src_nx, K.tgt, K.dsrc, K.hsrc, out_ny, out_nx, order, x, y, st);
+    K.release(st);
     if (err != cudaSuccess) return cuda_fail(err, "src_coords launch");
     return DFR_OK;
 }
@@ -265,66 +514,15 @@ int dfr_reproject_stack(const float *src_batch, int32_t n, int32_t src_ny, int32
     if (!src_batch || !sum || !wsum) { set_error("NULL image pointer"); return DFR_ERR_NULL; }
     int rc = check_common(n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order);
     if (rc != DFR_OK) return rc;
-    const char *s0 = (const char *)src_batch, *s1 = s0 + sizeof(float) * (size_t)n * src_ny * src_nx;
-    const size_t ob = sizeof(float) * (size_t)out_ny * out_nx;
-    const char *a0 = (const char *)sum, *b0 = (const char *)wsum;
-    if ((a0 < s1 && s0 < a0 + ob) || (b0 < s1 && s0 < b0 + ob) || (a0 < b0 + ob && b0 < a0 + ob)) {
+    const size_t sb = sizeof(float) * (size_t)n * src_ny * src_nx, ob = sizeof(float) * (size_t)out_ny * out_nx;
+    if (overlaps(sum, ob, src_batch, sb) || overlaps(wsum, ob, src_batch, sb) || overlaps(sum, ob, wsum, ob)) {
         set_error("sum / wsum overlap src_batch or each other");
         return DFR_ERR_ALIAS;
     }
-    for (int32_t e = 0; weights && e < n; ++e)
-        if (!std::isfinite(weights[e])) { set_error("weights[%d] is not finite", e); return DFR_ERR_NONFINITE_WCS; }
+    if ((rc = check_weights(weights, n)) != DFR_OK) return rc;
     return stack_impl(src_batch, n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order, weights, sum, wsum,
                       accumulate, (cudaStream_t)stream);
 }
-
-}  // extern "C"
-
-namespace dfr {
-// validated arguments -> constants, scratch, launches (stream-ordered)
-static int stack_impl(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
-                      const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs, int32_t out_ny, int32_t out_nx,
-                      int32_t order, const float *weights, float *sum, float *wsum, int32_t accumulate,
-                      cudaStream_t st)
-{
-    std::vector<float> hw((size_t)n, 1.0f);
-    for (int32_t e = 0; weights && e < n; ++e) hw[e] = weights[e];
-    std::call_once(g_pool_once, tune_pool);
-    int rc;
-    g_last.pending = false;
-    TargetDev tgt;
-    make_target(tgt_wcs, &tgt);
-    std::vector<SourceDev> hsrc;
-    SourceDev *dsrc = nullptr;
-    rc = upload_sources(n, src_wcs, tgt_wcs, st, hsrc, &dsrc);
-    if (rc != DFR_OK) return rc;
-    float *dw = nullptr;
-    TiledStats ts = {0, 0, 0, 0};
-    cudaError_t err = ensure_last();
-    if (err == cudaSuccess) err = cudaMallocAsync((void **)&dw, sizeof(float) * (size_t)n, st);
-    // pageable source: the runtime stages the bytes before returning, so `hw` may die
-    if (err == cudaSuccess) err = cudaMemcpyAsync(dw, hw.data(), sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, st);
-    if (err == cudaSuccess)
-        err = launch_tiled_stack(src_batch, n, src_ny, src_nx, tgt, dsrc, hsrc.data(), out_ny, out_nx, order,
-                                 dw, sum, wsum, accumulate != 0, st,
-                                 g_accumulate ? g_stream_totals : g_last.pinned_dev, g_accumulate ? 1 : 0,
-                                 &ts, &g_last.prof);
-    if (!g_accumulate && err == cudaSuccess) err = cudaEventRecord(g_last.done, st);
-    if (dw) cudaFreeAsync(dw, st);
-    cudaFreeAsync(dsrc, st);
-    if (g_accumulate) {
-        g_stats_acc[3] += ts.kernels;
-    } else {
-        g_last.kernels = ts.kernels;
-        g_last.tiled = true;
-        g_last.pending = (err == cudaSuccess);
-    }
-    if (err != cudaSuccess) return cuda_fail(err, "reproject_stack launch");
-    return DFR_OK;
-}
-}  // namespace dfr
-
-extern "C" {
 
 int dfr_stack_finalize(const float *sum, const float *wsum, int64_t npix, float *mean, void *stream)
 {
@@ -341,12 +539,15 @@ static int sky_common(const dfr_wcs *w, const void *a, const void *b, const void
     if (!w || (npts > 0 && (!a || !b || !c || !d))) { set_error("NULL pointer"); return DFR_ERR_NULL; }
     int rc = validate_wcs(w);
     if (rc != DFR_OK) return rc;
-    std::call_once(g_pool_once, tune_pool);
-    SkyDev h;
-    make_sky(w, &h);
-    cudaError_t err = cudaMallocAsync((void **)dev, sizeof(SkyDev), st);
-    if (err != cudaSuccess) return cuda_fail(err, "cudaMallocAsync(sky)");
-    err = cudaMemcpyAsync(*dev, &h, sizeof h, cudaMemcpyHostToDevice, st);
+    DevCtx *ctx = nullptr;
+    cudaError_t err = current_ctx(&ctx);
+    if (err != cudaSuccess) return cuda_fail(err, "device context");
+    PinnedSlot *slot = nullptr;
+    if ((err = stage_acquire(ctx, sizeof(SkyDev), &slot)) != cudaSuccess) return cuda_fail(err, "pinned staging buffer");
+    make_sky(w, static_cast<SkyDev *>(slot->host));
+    if ((err = scratch_alloc((void **)dev, sizeof(SkyDev), st)) != cudaSuccess) return cuda_fail(err, "scratch allocation (sky)");
+    err = cudaMemcpyAsync(*dev, slot->host, sizeof(SkyDev), cudaMemcpyHostToDevice, st);
+    if (err == cudaSuccess) err = stage_done(slot, st);
     if (err != cudaSuccess) { cudaFreeAsync(*dev, st); return cuda_fail(err, "cudaMemcpyAsync(sky)"); }
     return DFR_OK;
 }
@@ -375,40 +576,7 @@ int dfr_world2pix(const dfr_wcs *w, const double *ra_deg, const double *dec_deg,
     return err == cudaSuccess ? DFR_OK : cuda_fail(err, "world2pix launch");
 }
 
-// ---- end-to-end streaming form ------------------------
-namespace {
-struct Slot {
-    cudaStream_t st = nullptr;
-    float *din = nullptr, *dout = nullptr;
-    size_t in_bytes = 0, out_bytes = 0;
-};
-constexpr int kSlots = 3;
-struct HostPipe {
-    std::mutex mu;
-    int dev = -1;
-    Slot slot[kSlots];
-} g_pipe;
-
-static cudaError_t ensure_slot(Slot &s, size_t in_bytes, size_t out_bytes)
-{
-    cudaError_t err;
-    if (!s.st && (err = cudaStreamCreateWithFlags(&s.st, cudaStreamNonBlocking)) != cudaSuccess) return err;
-    if (s.in_bytes < in_bytes) {
-        if (s.din) cudaFree(s.din);
-        s.din = nullptr; s.in_bytes = 0;
-        if ((err = cudaMalloc((void **)&s.din, in_bytes)) != cudaSuccess) return err;
-        s.in_bytes = in_bytes;
-    }
-    if (s.out_bytes < out_bytes) {
-        if (s.dout) cudaFree(s.dout);
-        s.dout = nullptr; s.out_bytes = 0;
-        if ((err = cudaMalloc((void **)&s.dout, out_bytes)) != cudaSuccess) return err;
-        s.out_bytes = out_bytes;
-    }
-    return cudaSuccess;
-}
-}  // namespace
-
+// ---- end-to-end streaming forms ------------------------------------
 int dfr_reproject_host(const float *src_host, int32_t n, int32_t src_ny, int32_t src_nx,
                        const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
                        int32_t out_ny, int32_t out_nx, int32_t order,
@@ -419,47 +587,7 @@ int dfr_reproject_host(const float *src_host, int32_t n, int32_t src_ny, int32_t
     if (rc != DFR_OK) return rc;
     if (batch <= 0) batch = 32;
     if (batch > n) batch = n;
-    const size_t in_px = (size_t)src_ny * src_nx, out_px = (size_t)out_ny * out_nx;
-    std::lock_guard<std::mutex> lock(g_pipe.mu);
-    int dev = 0;
-    cudaError_t err = cudaGetDevice(&dev);
-    if (err != cudaSuccess) return cuda_fail(err, "cudaGetDevice");
-    if (g_pipe.dev != dev) {                       // buffers belong to one device
-        for (Slot &s : g_pipe.slot) {
-            if (s.din) cudaFree(s.din);
-            if (s.dout) cudaFree(s.dout);
-            if (s.st) cudaStreamDestroy(s.st);
-            s = Slot();
-        }
-        g_pipe.dev = dev;
-    }
-    const int nb = (n + batch - 1) / batch;
-    const int used = nb < kSlots ? nb : kSlots;
-    for (int k = 0; k < used; ++k) {
-        err = ensure_slot(g_pipe.slot[k], in_px * batch * sizeof(float), out_px * batch * sizeof(float));
-        if (err != cudaSuccess) return cuda_fail(err, "pipeline buffers");
-    }
-    if ((err = stream_stats_begin()) != cudaSuccess) return cuda_fail(err, "stream statistics");
-    for (int b = 0; b < nb; ++b) {
-        Slot &s = g_pipe.slot[b % kSlots];
-        const int32_t e0 = b * batch, ne = (n - e0 < batch) ? n - e0 : batch;
-        // slot reuse is ordered by the slot's own stream: H2D(b) waits for D2H(b - kSlots)
-        err = cudaMemcpyAsync(s.din, src_host + in_px * e0, in_px * ne * sizeof(float),
-                              cudaMemcpyHostToDevice, s.st);
-        if (err != cudaSuccess) { rc = cuda_fail(err, "H2D"); break; }
-        rc = reproject_impl(s.din, ne, src_ny, src_nx, src_wcs + e0, tgt_wcs, out_ny, out_nx, order,
-                            s.dout, s.st, DFR_PATH_AUTO);
-        if (rc != DFR_OK) break;
-        err = cudaMemcpyAsync(out_host + out_px * e0, s.dout, out_px * ne * sizeof(float),
-                              cudaMemcpyDeviceToHost, s.st);
-        if (err != cudaSuccess) { rc = cuda_fail(err, "D2H"); break; }
-    }
-    for (int k = 0; k < used; ++k) {
-        err = cudaStreamSynchronize(g_pipe.slot[k].st);
-        if (err != cudaSuccess && rc == DFR_OK) rc = cuda_fail(err, "pipeline sync");
-    }
-    stream_stats_end();
-    return rc;
+    return reproject_host_impl(src_host, n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order, out_host, batch);
 }
 
 int dfr_stack_host(const float *src_host, int32_t n, int32_t src_ny, int32_t src_nx,
@@ -470,60 +598,125 @@ int dfr_stack_host(const float *src_host, int32_t n, int32_t src_ny, int32_t src
     if (!src_host || !sum_host || !wsum_host) { set_error("NULL image pointer"); return DFR_ERR_NULL; }
     int rc = check_common(n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order);
     if (rc != DFR_OK) return rc;
-    for (int32_t e = 0; weights && e < n; ++e)
-        if (!std::isfinite(weights[e])) { set_error("weights[%d] is not finite", e); return DFR_ERR_NONFINITE_WCS; }
+    if ((rc = check_weights(weights, n)) != DFR_OK) return rc;
     if (batch <= 0) batch = 32;
     if (batch > n) batch = n;
-    const size_t in_px = (size_t)src_ny * src_nx, out_bytes = sizeof(float) * (size_t)out_ny * out_nx;
-    std::lock_guard<std::mutex> lock(g_pipe.mu);
-    int dev = 0;
-    cudaError_t err = cudaGetDevice(&dev);
-    if (err != cudaSuccess) return cuda_fail(err, "cudaGetDevice");
-    if (g_pipe.dev != dev) {                       // buffers belong to one device
-        for (Slot &s : g_pipe.slot) {
-            if (s.din) cudaFree(s.din);
-            if (s.dout) cudaFree(s.dout);
-            if (s.st) cudaStreamDestroy(s.st);
-            s = Slot();
-        }
-        g_pipe.dev = dev;
+    PipeLease L;
+    return stack_host_impl(L, src_host, n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order, weights,
+                           sum_host, wsum_host, batch, nullptr);
+}
+
+int dfr_shard_range(int32_t n, int32_t parts, int32_t k, int32_t *lo, int32_t *hi)
+{
+    if (!lo || !hi) { set_error("NULL pointer"); return DFR_ERR_NULL; }
+    if (n < 0 || parts < 1 || k < 0 || k >= parts) {
+        set_error("bad shard request n=%d parts=%d k=%d", n, parts, k);
+        return DFR_ERR_SHAPE;
     }
-    const int nb = (n + batch - 1) / batch;
-    const int used = nb < kSlots ? nb : kSlots;
-    // slot 0's output buffer holds sum and wsum; every slot needs an input buffer and a stream
-    for (int k = 0; k < used; ++k) {
-        err = ensure_slot(g_pipe.slot[k], in_px * batch * sizeof(float), k == 0 ? 2 * out_bytes : 0);
-        if (err != cudaSuccess) return cuda_fail(err, "pipeline buffers");
-    }
-    float *dsum = g_pipe.slot[0].dout, *dwsum = dsum + (size_t)out_ny * out_nx;
-    cudaEvent_t zeroed = nullptr;
-    if ((err = cudaEventCreateWithFlags(&zeroed, cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(err, "event");
-    err = cudaMemsetAsync(dsum, 0, 2 * out_bytes, g_pipe.slot[0].st);
-    if (err == cudaSuccess) err = cudaEventRecord(zeroed, g_pipe.slot[0].st);
-    for (int k = 1; k < used && err == cudaSuccess; ++k) err = cudaStreamWaitEvent(g_pipe.slot[k].st, zeroed, 0);
-    if (err != cudaSuccess) { cudaEventDestroy(zeroed); return cuda_fail(err, "pipeline start"); }
-    if ((err = stream_stats_begin()) != cudaSuccess) return cuda_fail(err, "stream statistics");
-    for (int b = 0; b < nb; ++b) {
-        Slot &s = g_pipe.slot[b % kSlots];
-        const int32_t e0 = b * batch, ne = (n - e0 < batch) ? n - e0 : batch;
-        // the slot's stream orders its own reuse: H2D(b) waits for the kernels of b - kSlots;
-        // batches of different slots add into sum / wsum concurrently (atomic adds)
-        err = cudaMemcpyAsync(s.din, src_host + in_px * e0, in_px * ne * sizeof(float), cudaMemcpyHostToDevice, s.st);
-        if (err != cudaSuccess) { rc = cuda_fail(err, "H2D"); break; }
-        rc = stack_impl(s.din, ne, src_ny, src_nx, src_wcs + e0, tgt_wcs, out_ny, out_nx, order,
-                        weights ? weights + e0 : nullptr, dsum, dwsum, 1, s.st);
-        if (rc != DFR_OK) break;
-    }
-    for (int k = 0; k < used; ++k) {
-        err = cudaStreamSynchronize(g_pipe.slot[k].st);
-        if (err != cudaSuccess && rc == DFR_OK) rc = cuda_fail(err, "pipeline sync");
-    }
-    cudaEventDestroy(zeroed);
-    stream_stats_end();
+    shard_range(n, parts, k, lo, hi);
+    return DFR_OK;
+}
+
+int dfr_reproject_host_multi(const float *src_host, int32_t n, int32_t src_ny, int32_t src_nx,
+                             const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                             int32_t out_ny, int32_t out_nx, int32_t order,
+                             float *out_host, int32_t batch, const int32_t *devices, int32_t ndev)
+{
+    if (!src_host || !out_host) { set_error("NULL image pointer"); return DFR_ERR_NULL; }
+    int rc = check_common(n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order);
     if (rc != DFR_OK) return rc;
-    err = cudaMemcpy(sum_host, dsum, out_bytes, cudaMemcpyDeviceToHost);
-    if (err == cudaSuccess) err = cudaMemcpy(wsum_host, dwsum, out_bytes, cudaMemcpyDeviceToHost);
-    return err == cudaSuccess ? DFR_OK : cuda_fail(err, "D2H");
+    if ((rc = check_devices(devices, ndev)) != DFR_OK) return rc;
+    if (batch <= 0) batch = 32;
+    const size_t in_px = (size_t)src_ny * src_nx, out_px = (size_t)out_ny * out_nx;
+    std::vector<ShardResult> res((size_t)ndev);
+    std::vector<std::thread> workers;
+    // exposures are independent: contiguous shards, one host thread and one
+    // pipeline per shard, no collective
+    for (int k = 0; k < ndev; ++k)
+        workers.emplace_back([&, k]() {
+            ShardResult &r = res[(size_t)k];
+            int32_t lo, hi;
+            shard_range(n, ndev, k, &lo, &hi);
+            if (hi <= lo) return;
+            const cudaError_t err = cudaSetDevice(devices[k]);
+            if (err != cudaSuccess) { r.rc = cuda_fail(err, "cudaSetDevice"); r.error = last_error_cstr(); return; }
+            r.rc = reproject_host_impl(src_host + in_px * lo, hi - lo, src_ny, src_nx, src_wcs + lo, tgt_wcs, out_ny, out_nx,
+                                       order, out_host + out_px * lo, std::min(batch, hi - lo));
+            if (r.rc != DFR_OK) r.error = last_error_cstr();
+            for (int q = 0; q < 4; ++q) r.stats[q] = g_stats_acc[q];
+        });
+    for (std::thread &t : workers) t.join();
+    for (int q = 0; q < 4; ++q) g_stats_acc[q] = 0;
+    for (const ShardResult &r : res) {
+        if (r.rc != DFR_OK && rc == DFR_OK) { rc = r.rc; set_error("%s", r.error.c_str()); }
+        for (int q = 0; q < 4; ++q) g_stats_acc[q] += r.stats[q];
+    }
+    g_last.pending = false;
+    g_last.kernels = -1;
+    return rc;
+}
+
+int dfr_stack_host_multi(const float *src_host, int32_t n, int32_t src_ny, int32_t src_nx,
+                         const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                         int32_t out_ny, int32_t out_nx, int32_t order, const float *weights,
+                         float *sum_host, float *wsum_host, int32_t batch, const int32_t *devices, int32_t ndev)
+{
+    if (!src_host || !sum_host || !wsum_host) { set_error("NULL image pointer"); return DFR_ERR_NULL; }
+    int rc = check_common(n, src_ny, src_nx, src_wcs, tgt_wcs, out_ny, out_nx, order);
+    if (rc != DFR_OK) return rc;
+    if ((rc = check_weights(weights, n)) != DFR_OK) return rc;
+    if ((rc = check_devices(devices, ndev)) != DFR_OK) return rc;
+    if (batch <= 0) batch = 32;
+    const size_t in_px = (size_t)src_ny * src_nx, npix = (size_t)out_ny * out_nx;
+    std::vector<ShardResult> res((size_t)ndev);
+    std::vector<PipeLease> lease((size_t)ndev);
+    std::vector<float *> partial((size_t)ndev, nullptr);
+    std::vector<std::thread> workers;
+    for (int k = 0; k < ndev; ++k)
+        workers.emplace_back([&, k]() {
+            ShardResult &r = res[(size_t)k];
+            int32_t lo, hi;
+            shard_range(n, ndev, k, &lo, &hi);
+            if (hi <= lo) return;
+            const cudaError_t err = cudaSetDevice(devices[k]);
+            if (err != cudaSuccess) { r.rc = cuda_fail(err, "cudaSetDevice"); r.error = last_error_cstr(); return; }
+            r.rc = stack_host_impl(lease[(size_t)k], src_host + in_px * lo, hi - lo, src_ny, src_nx, src_wcs + lo, tgt_wcs,
+                                   out_ny, out_nx, order, weights ? weights + lo : nullptr, nullptr, nullptr,
+                                   std::min(batch, hi - lo), &partial[(size_t)k]);
+            if (r.rc != DFR_OK) r.error = last_error_cstr();
+            for (int q = 0; q < 4; ++q) r.stats[q] = g_stats_acc[q];
+        });
+    for (std::thread &t : workers) t.join();
+    for (int q = 0; q < 4; ++q) g_stats_acc[q] = 0;
+    for (const ShardResult &r : res) {
+        if (r.rc != DFR_OK && rc == DFR_OK) { rc = r.rc; set_error("%s", r.error.c_str()); }
+        for (int q = 0; q < 4; ++q) g_stats_acc[q] += r.stats[q];
+    }
+    g_last.pending = false;
+    g_last.kernels = -1;
+    if (rc != DFR_OK) return rc;
+    // the one exchange step of the stack: the shards' partial sum | wsum pairs are
+    // copied to the first shard's device (peer copy) and added there, in shard order
+    int first = -1;
+    for (int k = 0; k < ndev; ++k)
+        if (partial[(size_t)k]) { first = k; break; }
+    if (first < 0) { set_error("no exposures"); return DFR_ERR_SHAPE; }
+    int prev = 0;
+    cudaGetDevice(&prev);
+    cudaError_t err = cudaSetDevice(devices[first]);
+    float *tmp = nullptr;
+    if (err == cudaSuccess) err = cudaMalloc((void **)&tmp, 2 * npix * sizeof(float));
+    for (int k = first + 1; k < ndev && err == cudaSuccess; ++k) {
+        if (!partial[(size_t)k]) continue;
+        err = cudaMemcpyPeer(tmp, devices[first], partial[(size_t)k], devices[k], 2 * npix * sizeof(float));
+        if (err == cudaSuccess) err = launch_stack_add(partial[(size_t)first], tmp, (long long)(2 * npix), nullptr);
+        if (err == cudaSuccess) err = cudaStreamSynchronize(nullptr);
+    }
+    if (err == cudaSuccess) err = cudaMemcpy(sum_host, partial[(size_t)first], npix * sizeof(float), cudaMemcpyDeviceToHost);
+    if (err == cudaSuccess) err = cudaMemcpy(wsum_host, partial[(size_t)first] + npix, npix * sizeof(float), cudaMemcpyDeviceToHost);
+    if (tmp) cudaFree(tmp);
+    cudaSetDevice(prev);
+    return err == cudaSuccess ? DFR_OK : cuda_fail(err, "multi-device stack reduction");
 }
 
 int dfr_wcs_set_pc_cdelt(dfr_wcs *w, const double pc[4], const double cdelt[2])
@@ -558,33 +751,51 @@ int dfr_last_stats(int64_t stats[4])
         for (int k = 0; k < 4; ++k) stats[k] = g_stats_acc[k];
         return DFR_OK;
     }
-    collect_stats(stats);
+    stats[0] = stats[1] = stats[2] = 0;
+    stats[3] = g_last.kernels;
+    if (g_last.tiled && g_last.pending && g_last.ctx) {
+        cudaEventSynchronize(g_last.ctx->done);
+        for (int k = 0; k < 3; ++k) stats[k] = g_last.ctx->pinned[k];
+    } else if (!g_last.tiled) {
+        stats[1] = -1;                                        // exact path: no tiles
+    }
     return DFR_OK;
 }
 
 int dfr_profile_enable(int on)
 {
-    ProfileEvents &p = g_last.prof;
-    if (on && !p.setup_begin) {
-        cudaError_t err;
-        if ((err = cudaEventCreate(&p.setup_begin)) != cudaSuccess ||
-            (err = cudaEventCreate(&p.main_begin)) != cudaSuccess ||
-            (err = cudaEventCreate(&p.main_end)) != cudaSuccess)
-            return cuda_fail(err, "cudaEventCreate");
-    }
-    p.enabled = on != 0;
+    g_profile = on != 0;
     return DFR_OK;
 }
 
 int dfr_profile_last(float ms[2])
 {
-    ProfileEvents &p = g_last.prof;
     if (!ms) return DFR_ERR_NULL;
-    if (!p.enabled || !p.main_end) { set_error("profiling is not enabled"); return DFR_ERR_ORDER; }
-    cudaError_t err = cudaEventSynchronize(p.main_end);
-    if (err == cudaSuccess) err = cudaEventElapsedTime(&ms[0], p.setup_begin, p.main_begin);
-    if (err == cudaSuccess) err = cudaEventElapsedTime(&ms[1], p.main_begin, p.main_end);
+    DevCtx *c = g_last.ctx;
+    if (!g_profile || !c || !c->prof.main_end) { set_error("profiling is not enabled"); return DFR_ERR_ORDER; }
+    cudaError_t err = cudaEventSynchronize(c->prof.main_end);
+    if (err == cudaSuccess) err = cudaEventElapsedTime(&ms[0], c->prof.setup_begin, c->prof.main_begin);
+    if (err == cudaSuccess) err = cudaEventElapsedTime(&ms[1], c->prof.main_begin, c->prof.main_end);
     return err == cudaSuccess ? DFR_OK : cuda_fail(err, "profile events");
+}
+
+int dfr_release(void)
+{
+    int dev = 0;
+    const cudaError_t err = cudaGetDevice(&dev);
+    if (err != cudaSuccess) return cuda_fail(err, "cudaGetDevice");
+    if (g_last.ctx && g_last.ctx->dev == dev) g_last = LastCall();
+    release_current_device();
+    pipe_free_idle(dev);
+    return DFR_OK;
+}
+
+int dfr_probe_rates(double *out, int32_t n)
+{
+    if (!out) { set_error("NULL pointer"); return DFR_ERR_NULL; }
+    if (n < DFR_PROBE_COUNT) { set_error("out needs %d entries", (int)DFR_PROBE_COUNT); return DFR_ERR_SHAPE; }
+    const cudaError_t err = probe_rates(out);
+    return err == cudaSuccess ? DFR_OK : cuda_fail(err, "probe kernels");
 }
 
 const char *dfr_strerror(int code)
@@ -599,12 +810,13 @@ const char *dfr_strerror(int code)
     case DFR_ERR_NONFINITE_WCS: return "non-finite WCS field";
     case DFR_ERR_ALIAS: return "output aliases input";
     case DFR_ERR_CUDA: return "CUDA failure";
+    case DFR_ERR_WEIGHT: return "non-finite stacking weight";
     default: return "unknown error";
     }
 }
 
 const char *dfr_last_error(void) { return dfr::last_error_cstr(); }
 
-int dfr_version(void) { return 100; }
+int dfr_version(void) { return 200; }
 
 }  // extern "C"

@@ -100,6 +100,23 @@ __device__ __forceinline__ bool in_footprint(double x, double y, int ny, int nx,
     return (x >= -0.5) && (x < (double)nx - 0.5) && (y >= -0.5) && (y < (double)ny - 0.5);
 }
 
+// The footprint array of dfr_reproject_fp ("projecting an identity
+// tensor called the footprint"). DFR_EDGE_PAPER with bilinear interpolation: the zero-padded
+// interpolation of an all-ones image, i.e. the product over the two axes of the weight of the taps
+// that fall inside the image (1 on [0, n-1], falling linearly to 0 at -1 and at n). Every other
+// mode: 1 inside the area footprint, 0 outside (nearest: the paper's identity is exactly that).
+__device__ __forceinline__ float footprint_value(double x, double y, int ny, int nx, int order, int edge)
+{
+    if (!(x == x) || !(y == y)) return 0.0f;
+    if (edge == DFR_EDGE_PAPER && order == DFR_BILINEAR) {
+        if (!(x > -1.0 && x < (double)nx && y > -1.0 && y < (double)ny)) return 0.0f;
+        const double wx = x < 0.0 ? 1.0 + x : (x > (double)nx - 1.0 ? (double)nx - x : 1.0);
+        const double wy = y < 0.0 ? 1.0 + y : (y > (double)ny - 1.0 ? (double)ny - y : 1.0);
+        return (float)(wx * wy);
+    }
+    return in_footprint(x, y, ny, nx, DFR_EDGE_AREA) ? 1.0f : 0.0f;
+}
+
 __device__ __forceinline__ int clampi(int v, int lo, int hi) { return min(max(v, lo), hi); }
 
 // Keys cubic-convolution weights for taps -1, 0, +1, +2 at fraction t, a = -0.75 (G7).

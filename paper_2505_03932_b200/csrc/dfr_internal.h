@@ -58,7 +58,7 @@ int  cuda_fail(cudaError_t e, const char *what);            // records text, ret
 cudaError_t launch_exact_reproject(const float *src, int n, int sny, int snx,
                                    const TargetDev &tgt, const SourceDev *srcdev,
                                    int ony, int onx, int order, float *out, cudaStream_t st,
-                                   int edge = DFR_EDGE_AREA);
+                                   int edge = DFR_EDGE_AREA, float *foot = nullptr);
 cudaError_t launch_exact_coords(int n, const TargetDev &tgt, const SourceDev *srcdev,
                                 int ony, int onx, double *x, double *y, cudaStream_t st);
 // literal sky kernels
@@ -66,5 +66,8 @@ cudaError_t launch_pix2world(const SkyDev *w, const double *x, const double *y, 
                              double *ra, double *dec, cudaStream_t st);
 cudaError_t launch_world2pix(const SkyDev *w, const double *ra, const double *dec, int64_t npts,
                              double *x, double *y, cudaStream_t st);
+
+// register-only instruction-rate probes (dfr_probe.cu)
+cudaError_t probe_rates(double *out);
 
 }  // namespace dfr

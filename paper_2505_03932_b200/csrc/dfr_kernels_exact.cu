@@ -13,7 +13,7 @@ __global__ void __launch_bounds__(EX_BX *EX_BY)
 exact_reproject_kernel(const float *__restrict__ src, int sny, int snx,
                        const __grid_constant__ TargetDev tgt,
                        const SourceDev *__restrict__ srcdev,
-                       int ony, int onx, float *__restrict__ out, int edge)
+                       int ony, int onx, float *__restrict__ out, int edge, float *__restrict__ foot)
 {
     // blockIdx.x enumerates the EX_BX x EX_BY output tiles row-major (no 65535 limit)
     const int tiles_x = (onx + EX_BX - 1) / EX_BX;
@@ -28,6 +28,7 @@ exact_reproject_kernel(const float *__restrict__ src, int sny, int snx,
     if (in_footprint(x, y, sny, snx, edge))
         val = sample_global<ORDER>(src + (size_t)e * sny * snx, sny, snx, x, y);
     out[((size_t)e * ony + j) * onx + i] = val;
+    if (foot) foot[((size_t)e * ony + j) * onx + i] = footprint_value(x, y, sny, snx, ORDER, edge);
 }
 
 __global__ void __launch_bounds__(EX_BX *EX_BY)
@@ -55,7 +56,7 @@ static dim3 exact_grid(int n, int ony, int onx)
 
 cudaError_t launch_exact_reproject(const float *src, int n, int sny, int snx,
                                    const TargetDev &tgt, const SourceDev *srcdev,
-                                   int ony, int onx, int order, float *out, cudaStream_t st, int edge)
+                                   int ony, int onx, int order, float *out, cudaStream_t st, int edge, float *foot)
 {
     const dim3 block(EX_BX, EX_BY);
     // grid.y is limited to 65535 exposures per launch
@@ -64,12 +65,13 @@ cudaError_t launch_exact_reproject(const float *src, int n, int sny, int snx,
         const dim3 grid = exact_grid(ne, ony, onx);
         const float *s = src + (size_t)e0 * sny * snx;
         float *o = out + (size_t)e0 * ony * onx;
+        float *f = foot ? foot + (size_t)e0 * ony * onx : nullptr;
         if (order == DFR_NEAREST)
-            exact_reproject_kernel<DFR_NEAREST><<<grid, block, 0, st>>>(s, sny, snx, tgt, srcdev + e0, ony, onx, o, edge);
+            exact_reproject_kernel<DFR_NEAREST><<<grid, block, 0, st>>>(s, sny, snx, tgt, srcdev + e0, ony, onx, o, edge, f);
         else if (order == DFR_BILINEAR)
-            exact_reproject_kernel<DFR_BILINEAR><<<grid, block, 0, st>>>(s, sny, snx, tgt, srcdev + e0, ony, onx, o, edge);
+            exact_reproject_kernel<DFR_BILINEAR><<<grid, block, 0, st>>>(s, sny, snx, tgt, srcdev + e0, ony, onx, o, edge, f);
         else
-            exact_reproject_kernel<DFR_BICUBIC><<<grid, block, 0, st>>>(s, sny, snx, tgt, srcdev + e0, ony, onx, o, edge);
+            exact_reproject_kernel<DFR_BICUBIC><<<grid, block, 0, st>>>(s, sny, snx, tgt, srcdev + e0, ony, onx, o, edge, f);
         cudaError_t err = cudaGetLastError();
         if (err != cudaSuccess) return err;
     }

@@ -55,11 +55,13 @@ constexpr int kMaxBoxBytes = 36 * 1024;       // staged box limit: keeps >= 6 CT
 
 // ---- host side shared by the launchers (dfr_tiled_setup.cu) ----------------
 struct Scratch {
+    void *block = nullptr;                          // one stream-ordered allocation holding all four
     double2 *uv = nullptr;
     TileRec *recs = nullptr;
     int2 *cta_box = nullptr;
     int32_t *counters = nullptr;                    // fast, exact, empty, ticket
 };
+cudaError_t scratch_alloc(void **p, size_t bytes, cudaStream_t st);     // dfr_context.cu: the library's own pool
 
 // Setup kernels + staging decision shared by the per-exposure and the stacking launchers.
 struct Prepared {
@@ -84,12 +86,14 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
                                    int ony, int onx, int order, float *out, cudaStream_t st,
                                    int32_t *host_stats /* 3 ints the setup kernel can write (mapped host or device memory), or NULL */,
                                    int stats_add /* 0: store the totals, 1: atomically add them (streaming) */,
-                                   TiledStats *stats, ProfileEvents *prof, int edge = DFR_EDGE_AREA);
+                                   TiledStats *stats, ProfileEvents *prof, int edge = DFR_EDGE_AREA,
+                                   float *foot = nullptr /* DEVICE [n][ony][onx] footprint array, or NULL */);
 // dfr_reproject_stack: sum / wsum accumulated over the n exposures in one kernel.
 cudaError_t launch_tiled_stack(const float *src, int n, int sny, int snx, const TargetDev &tgt,
                                const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx, int order,
                                const float *dev_weights, float *sum, float *wsum, int accumulate,
                                cudaStream_t st, int32_t *host_stats, int stats_add, TiledStats *stats, ProfileEvents *prof);
+cudaError_t launch_stack_add(float *a, const float *b, long long n, cudaStream_t st);
 cudaError_t launch_stack_finalize(const float *sum, const float *wsum, long long npix, float *mean, cudaStream_t st);
 cudaError_t launch_tiled_coords(int n, int sny, int snx, const TargetDev &tgt,
                                 const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx, int order,

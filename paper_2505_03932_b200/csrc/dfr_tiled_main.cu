@@ -22,11 +22,10 @@ namespace dfr {
 // ---------------------------------------------------------------------------------
 // EDGE (DFR_EDGE_*) is a template parameter so that the default kernel is compiled exactly as
 // without it (a run-time flag cost 3 % through register allocation alone).
-#ifndef DFR_BICUBIC_MINB
-#define DFR_BICUBIC_MINB 8
-#endif
+// Bicubic gets 80 registers (6 CTAs / SM): with 64 the 32 taps of a row pair cannot all be in flight
+// (measured on B200, C3: 0.102 -> 0.094 ms; 96 registers / 5 CTAs: 0.093 ms).
 template <int ORDER, bool STAGE, int EDGE = DFR_EDGE_AREA>
-__global__ void __launch_bounds__(32 * CTA_T * CTA_T, ORDER == DFR_BICUBIC ? DFR_BICUBIC_MINB : 8)
+__global__ void __launch_bounds__(32 * CTA_T * CTA_T, ORDER == DFR_BICUBIC ? 6 : 8)
 tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_constant__ TargetDev tgt,
                        const __grid_constant__ CUtensorMap tmap)
 {
@@ -167,6 +166,58 @@ tiled_coords_kernel(const __grid_constant__ TiledParams P, const __grid_constant
     }
 }
 
+// The footprint array of dfr_reproject_fp (footprint_value, dfr_device.cuh) from the same tile records
+// and the same polynomial coordinates as the main kernel, so it is consistent with `out` pixel by
+// pixel: EMPTY tiles are 0, EXACT tiles use the fp64 map, FAST tiles the polynomial coordinate. A
+// separate pass over the records (no image reads, 4 B written per pixel) keeps the main kernel,
+// and with it `out`, exactly as it is without a footprint.
+__global__ void __launch_bounds__(32 * CTA_T * CTA_T)
+tiled_footprint_kernel(const __grid_constant__ TiledParams P, const __grid_constant__ TargetDev tgt,
+                       int order, int edge, float *__restrict__ foot)
+{
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int e = P.e0 + blockIdx.z;
+    const int ttx = blockIdx.x * CTA_T + (warp % CTA_T), tty = blockIdx.y * CTA_T + (warp / CTA_T);
+    if (!(ttx < P.tiles_x && tty < P.tiles_y)) return;
+    const int ntile = P.tiles_x * P.tiles_y;
+    const TileRec *rec = P.recs + ((size_t)e * ntile + tty * P.tiles_x + ttx);
+    const int flag = rec->flag, ix0 = rec->ix0, iy0 = rec->iy0, deg = rec->deg;
+    const int tx0 = ttx * TS, ty0 = tty * TS, col = tx0 + lane;
+    if (col >= P.onx) return;
+    const int rows = min(TS, P.ony - ty0);
+    float *__restrict__ o = foot + ((size_t)e * P.ony + ty0) * P.onx + col;
+    if (flag == TILE_EMPTY) {
+        for (int r = 0; r < rows; ++r) o[(size_t)r * P.onx] = 0.0f;
+        return;
+    }
+    if (flag == TILE_EXACT) {
+        for (int r = 0; r < rows; ++r) {
+            double U, V, x, y;
+            target_uv(tgt, (double)col, (double)(ty0 + r), U, V);
+            source_xy(P.srcdev[e], U, V, x, y);
+            o[(size_t)r * P.onx] = footprint_value(x, y, P.sny, P.snx, order, edge);
+        }
+        return;
+    }
+    float X[4], Y[4];
+    const float di = (float)lane - (float)kCentre;
+    const float4 *c4 = reinterpret_cast<const float4 *>(rec->cx);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const float4 a = __ldg(c4 + q), b = __ldg(c4 + 4 + q);
+        X[q] = fmaf(fmaf(fmaf(a.w, di, a.z), di, a.y), di, a.x);
+        Y[q] = fmaf(fmaf(fmaf(b.w, di, b.z), di, b.y), di, b.x);
+    }
+    if (deg < 3) { X[3] = 0.0f; Y[3] = 0.0f; }                  // as the main kernel does
+    if (deg < 2) { X[2] = 0.0f; Y[2] = 0.0f; }
+    for (int r = 0; r < rows; ++r) {
+        const float dj = (float)r - (float)kCentre;
+        const float xl = fmaf(fmaf(fmaf(X[3], dj, X[2]), dj, X[1]), dj, X[0]);
+        const float yl = fmaf(fmaf(fmaf(Y[3], dj, Y[2]), dj, Y[1]), dj, Y[0]);
+        o[(size_t)r * P.onx] = footprint_value((double)ix0 + (double)xl, (double)iy0 + (double)yl, P.sny, P.snx, order, edge);
+    }
+}
+
 template <int ORDER, bool STAGE, int EDGE = DFR_EDGE_AREA>
 static cudaError_t launch_main(const TiledParams &P, const TargetDev &tgt, const CUtensorMap &tmap,
                                size_t smem, cudaStream_t st)
@@ -203,7 +254,7 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
                                    const SourceDev *srchost,
                                    int ony, int onx, int order, float *out, cudaStream_t st,
                                    int32_t *host_stats, int stats_add, TiledStats *stats, ProfileEvents *prof,
-                                   int edge)
+                                   int edge, float *foot)
 {
     Prepared R;
     if (prof && prof->enabled) cudaEventRecord(prof->setup_begin, st);
@@ -221,8 +272,18 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
     else DFR_LAUNCH(DFR_BICUBIC);
 #undef DFR_LAUNCH
     if (prof && prof->enabled) cudaEventRecord(prof->main_end, st);
-    free_scratch(R.sc, st);
     stats->kernels = 3;
+    if (foot && err == cudaSuccess) {
+        TiledParams Q = R.P;
+        for (int e0 = 0; e0 < n && err == cudaSuccess; e0 += 65535) {
+            Q.e0 = e0;
+            const dim3 grid((unsigned)Q.ctas_x, (unsigned)Q.ctas_y, (unsigned)std::min(n - e0, 65535));
+            tiled_footprint_kernel<<<grid, 32 * CTA_T * CTA_T, 0, st>>>(Q, tgt, order, edge, foot);
+            err = cudaGetLastError();
+        }
+        stats->kernels = 4;
+    }
+    free_scratch(R.sc, st);
     stats->tiles_fast = stats->tiles_exact = stats->tiles_empty = -1;   // written to host_stats by the setup kernel
     return err;
 }

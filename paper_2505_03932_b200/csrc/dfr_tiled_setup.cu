@@ -420,12 +420,18 @@ cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const Sourc
     const int ntile = P.tiles_x * P.tiles_y;
     cudaError_t err;
     const int ctas = P.ctas_x * P.ctas_y;
-    if ((err = cudaMallocAsync((void **)&sc.uv, sizeof(double2) * (size_t)ctas * NPTS, st)) != cudaSuccess) return err;
-    if ((err = cudaMallocAsync((void **)&sc.recs, sizeof(TileRec) * (size_t)ntile * n, st)) != cudaSuccess) return err;
+    // one stream-ordered allocation from the library's pool, carved up (256-byte aligned pieces)
+    auto up = [](size_t b) { return (b + 255) & ~(size_t)255; };
+    const size_t b_uv = up(sizeof(double2) * (size_t)ctas * NPTS), b_recs = up(sizeof(TileRec) * (size_t)ntile * n),
+                 b_box = up(sizeof(int2) * (size_t)ctas * n), b_cnt = up(4 * sizeof(int32_t));
+    if ((err = scratch_alloc(&sc.block, b_uv + b_recs + b_box + b_cnt, st)) != cudaSuccess) return err;
+    char *base = static_cast<char *>(sc.block);
+    sc.uv = reinterpret_cast<double2 *>(base);
+    sc.recs = reinterpret_cast<TileRec *>(base + b_uv);
+    sc.cta_box = reinterpret_cast<int2 *>(base + b_uv + b_recs);
+    sc.counters = reinterpret_cast<int32_t *>(base + b_uv + b_recs + b_box);
     P.recs = sc.recs;
-    if ((err = cudaMallocAsync((void **)&sc.cta_box, sizeof(int2) * (size_t)ctas * n, st)) != cudaSuccess) return err;
     P.cta_box = sc.cta_box;
-    if ((err = cudaMallocAsync((void **)&sc.counters, 4 * sizeof(int32_t), st)) != cudaSuccess) return err;
     target_nodes_kernel<<<(ctas * NPTS + 127) / 128, 128, 0, st>>>(tgt, fc, P.ctas_x, ctas, sc.uv, sc.counters);
     if ((err = cudaGetLastError()) != cudaSuccess) return err;
     // SIP order class of the batch: inverse polynomials are zero-padded up to N
@@ -448,10 +454,8 @@ cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const Sourc
 
 void free_scratch(Scratch &sc, cudaStream_t st)
 {
-    if (sc.uv) cudaFreeAsync(sc.uv, st);
-    if (sc.recs) cudaFreeAsync(sc.recs, st);
-    if (sc.cta_box) cudaFreeAsync(sc.cta_box, st);
-    if (sc.counters) cudaFreeAsync(sc.counters, st);
+    if (sc.block) cudaFreeAsync(sc.block, st);
+    sc = Scratch();
 }
 
 cudaError_t prepare_tiled(const float *src, int n, int sny, int snx, const TargetDev &tgt,
@@ -468,7 +472,12 @@ cudaError_t prepare_tiled(const float *src, int n, int sny, int snx, const Targe
     const int tlo = (order == DFR_BICUBIC) ? 1 : 0, thi = (order == DFR_BICUBIC) ? 2 : 1;
     EncodeTiledFn enc = get_encode();
     bool no_stage = false;
-    int bw_align = 4;
+    // Row pitch of the staged box. Bicubic: a multiple of 32 floats (128 B), so the lanes of a warp,
+    // whose taps span two or three box rows under any rotation, never meet in a bank — its 16 LDS per
+    // pixel made shared-memory wavefronts the wall (ncu, C3: 13.5 M conflicts on 26.8 M wavefronts, data
+    // pipe 79 %; 0.131 -> 0.102 ms). Nearest / bilinear read 1 / 4 taps and are HBM-bound: the narrower
+    // box (fewer L2 -> shared bytes, more CTAs per SM) measured equal or better there.
+    int bw_align = (order == DFR_BICUBIC) ? 32 : 4;
 #ifdef DFR_DEV_HOOKS                                                 // A-B timing builds only (never the shipped library)
     no_stage = std::getenv("DFR_NO_STAGE") != nullptr;
     if (const char *a = std::getenv("DFR_BW_ALIGN")) bw_align = std::atoi(a);
@@ -477,8 +486,9 @@ cudaError_t prepare_tiled(const float *src, int n, int sny, int snx, const Targe
         // floor-range spread + taps + 1 px safety each side; + 3: the origin is rounded down
         // to a multiple of 4 floats; then the width itself is rounded up to 16 bytes
         int bw = ((int)std::ceil(ex * 1.02) + 2 + tlo + thi + 2 + 3 + 3) & ~3;
-        bw = (bw + bw_align - 1) / bw_align * bw_align;
         const int bh = (int)std::ceil(ey * 1.02) + 2 + tlo + thi + 2;
+        const int bwa = (bw + bw_align - 1) / bw_align * bw_align;
+        if (bwa <= 256 && (size_t)bwa * bh * sizeof(float) <= (size_t)kMaxBoxBytes) bw = bwa;
         if (bw <= 256 && bh <= 256 && (size_t)bw * bh * sizeof(float) <= (size_t)kMaxBoxBytes) {
             const cuuint64_t dims[3] = {(cuuint64_t)snx, (cuuint64_t)sny, (cuuint64_t)n};
             const cuuint64_t strides[2] = {(cuuint64_t)snx * 4, (cuuint64_t)snx * sny * 4};

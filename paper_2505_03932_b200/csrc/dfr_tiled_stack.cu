@@ -243,6 +243,13 @@ __global__ void stack_finalize_kernel(const float *__restrict__ sum, const float
     }
 }
 
+// a[k] += b[k]: the reduction step of the multi-device stack (partial sums of two shards)
+__global__ void stack_add_kernel(float *__restrict__ a, const float *__restrict__ b, long long n)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) a[i] += b[i];
+}
+
 template <int ORDER, bool STAGE>
 static cudaError_t launch_stack(TiledParams P, const TargetDev &tgt, const CUtensorMap &tmap, size_t box_bytes,
                                 const StackParams &S, cudaStream_t st)
@@ -316,6 +323,13 @@ cudaError_t launch_tiled_stack(const float *src, int n, int sny, int snx, const 
     stats->kernels = 3;
     stats->tiles_fast = stats->tiles_exact = stats->tiles_empty = -1;
     return err;
+}
+
+cudaError_t launch_stack_add(float *a, const float *b, long long n, cudaStream_t st)
+{
+    if (n <= 0) return cudaSuccess;
+    stack_add_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(a, b, n);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_stack_finalize(const float *sum, const float *wsum, long long npix, float *mean, cudaStream_t st)

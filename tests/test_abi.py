@@ -102,7 +102,7 @@ def test_stack_validation_errors_without_gpu(P):
     assert call(src=None) == -1 and call(s=None) == -1 and call(c=None) == -1   # DFR_ERR_NULL
     assert call(n=0) == -2 and call(order=2) == -3
     assert call(s=C.c_void_p(0x10000 + 16)) == -7 and call(c=a) == -7            # overlap src / each other
-    assert call(weights=(C.c_float * 2)(1.0, float("inf"))) == -6                # non-finite weight
+    assert call(weights=(C.c_float * 2)(1.0, float("inf"))) == -9                # DFR_ERR_WEIGHT
     assert b"weights[1]" in L.dfr_last_error()
     # host-buffer form and finalize
     assert L.dfr_stack_host(None, 2, 8, 8, arr, C.byref(good), 8, 8, 1, None, a, b, 2) == -1
@@ -123,3 +123,45 @@ def test_binding_refuses_cpu_tensors(P):
     with pytest.raises(ValueError):
         P.dfr_reproject(torch.zeros(1, 8, 8), [S.make_wcs(8, 8, 1, 2, 0, S.PIXSCALE)],
                         S.make_wcs(8, 8, 1, 2, 0, S.PIXSCALE))
+
+
+def test_footprint_and_multi_device_validation_without_gpu(P):
+    L = P.lib()
+    w = S.make_wcs(8, 8, 1.0, 2.0, 0.0, S.PIXSCALE)
+    good = P.pack_wcs(w)
+    arr = (P.DfrWCS * 2)(good, good)
+    src, out, fp = C.c_void_p(0x10000), C.c_void_p(0x90000), C.c_void_p(0xA0000)
+
+    def call_fp(order=1, mode=0, out=out, fp=fp):
+        return L.dfr_reproject_fp(src, 2, 8, 8, arr, C.byref(good), 8, 8, order, mode, out, fp, None)
+
+    assert call_fp(mode=3) == -3 and call_fp(order=3, mode=1) == -3
+    assert call_fp(fp=C.c_void_p(0x90000 + 64)) == -7 and b"footprint" in L.dfr_last_error()   # overlaps out
+    assert call_fp(fp=C.c_void_p(0x10000)) == -7                                                # overlaps src
+    assert call_fp(out=None) == -1
+    devs = (C.c_int32 * 2)(0, 0)
+    assert L.dfr_reproject_host_multi(None, 2, 8, 8, arr, C.byref(good), 8, 8, 1, out, 2, devs, 2) == -1
+    assert L.dfr_reproject_host_multi(src, 2, 8, 8, arr, C.byref(good), 8, 8, 1, out, 2, None, 2) == -1
+    assert L.dfr_reproject_host_multi(src, 2, 8, 8, arr, C.byref(good), 8, 8, 1, out, 2, devs, 0) == -2
+    assert L.dfr_stack_host_multi(src, 2, 8, 8, arr, C.byref(good), 8, 8, 2, None, out, fp, 2, devs, 2) == -3
+    assert L.dfr_stack_host_multi(src, 2, 8, 8, arr, C.byref(good), 8, 8, 1, (C.c_float * 2)(1.0, float("nan")),
+                                  out, fp, 2, devs, 2) == -9
+    assert L.dfr_probe_rates(None, 10) == -1 and L.dfr_probe_rates((C.c_double * 4)(), 4) == -2
+
+
+def test_shard_range_is_a_partition_and_matches_the_python_rule(P):
+    from paper_2505_03932_b200.shard import shard_range
+    for n in (0, 1, 5, 32, 33, 1024, 1031):
+        for parts in (1, 2, 3, 7, 8, 64):
+            pieces = [P.dfr_shard_range(n, parts, k) for k in range(parts)]
+            assert pieces[0][0] == 0 and pieces[-1][1] == n
+            assert all(pieces[k][1] == pieces[k + 1][0] for k in range(parts - 1))       # contiguous, ordered
+            sizes = [hi - lo for lo, hi in pieces]
+            assert max(sizes) - min(sizes) <= 1 and sizes == sorted(sizes, reverse=True)
+            for k in range(parts):
+                r = shard_range(n, parts, k)
+                assert (r.start, r.stop) == pieces[k]
+    with pytest.raises(P.DfrError):
+        P.dfr_shard_range(10, 0, 0)
+    with pytest.raises(P.DfrError):
+        P.dfr_shard_range(10, 4, 4)

@@ -464,3 +464,149 @@ def test_fitted_inverse_sip_end_to_end(P, fit_order):
     xb, _ = oracle.src_coords(tgt, src, ony, onx)
     assert np.nanmax(np.abs(xa - xb)) > 0.05
     print("f4", fit_order, "fit residual", resid, rep[("coords", 0)])
+
+
+@pytest.mark.parametrize("order", [0, 1, 3])
+def test_footprint_array_area_rule(P, order):
+    """§8(f) f2: dfr_reproject_fp returns (array, footprint) like reproject_interp.
+    Under the area rule the footprint is 1 where the oracle's footprint rule (O11) holds and 0
+    elsewhere — the oracle side is its interpolation of an all-ones image (1 inside, NaN outside);
+    identical outside the 1e-3 px edge band; `array` is bit-identical with and without it."""
+    rng = np.random.default_rng(27)
+    sny, snx, ony, onx = 236, 300, 250, 330
+    imgs = np.stack([S.make_image(sny, snx, 40, rng) for _ in range(2)])
+    imgs[1, 50:60, 70:90] = np.nan                  # NaN pixels do not change the footprint
+    srcs = [S.add_sip(S.make_wcs(snx, sny, 150.0, 2.0 + 0.002 * k, 5.0 * k, S.PIXSCALE), 3, snx / 2.0, rng, amp=1e-4)
+            for k in range(2)]
+    tgt = S.make_wcs(onx, ony, 150.002, 2.001, 9.0, S.PIXSCALE * 1.04)
+    d = torch.from_numpy(imgs).cuda()
+    plain = P.dfr_reproject(d, srcs, tgt, (ony, onx), order)
+    out, foot = P.dfr_reproject(d, srcs, tgt, (ony, onx), order, footprint=True)
+    assert P.dfr_last_stats()["kernels"] == 4
+    assert torch.equal(torch.nan_to_num(plain, nan=-7.0), torch.nan_to_num(out, nan=-7.0))
+    foot = foot.cpu().numpy()
+    ones = np.ones((sny, snx), dtype=np.float32)
+    for e in range(2):
+        xo, yo = oracle.src_coords(tgt, srcs[e], ony, onx)
+        ref = np.nan_to_num(oracle.interp(ones, xo.ravel(), yo.ravel(), order).reshape(ony, onx), nan=0.0)
+        band = PR.edge_band(xo, yo, sny, snx)
+        assert set(np.unique(foot[e])) <= {0.0, 1.0} and 0.05 < ref.mean() < 0.95
+        assert np.array_equal(foot[e][~band], ref[~band].astype(np.float32))
+        # consistent with the array itself: valid pixels lie inside the footprint
+        assert not (~np.isnan(out[e].cpu().numpy()) & (foot[e] == 0)).any()
+
+
+def test_footprint_array_paper_rule(P):
+    """the footprint is the projected identity. DFR_EDGE_PAPER + bilinear returns
+    orc_interp_paper's `foot` (zero-padded interpolation of ones): |difference| <= COORD_TOL (its
+    slope is at most 1 per pixel on each axis and the coordinates agree to COORD_TOL), 0 / > 0
+    pattern identical outside the edge band of the (-1, n) rule; nearest: the 0/1 area footprint."""
+    rng = np.random.default_rng(69)
+    sny, snx, ony, onx = 140, 212, 190, 260
+    img = S.make_image(sny, snx, 40, rng)
+    src = S.add_sip(S.make_wcs(snx, sny, 150.0, 2.0, 0.0, S.PIXSCALE), 3, snx / 2.0, rng, amp=1e-4)
+    tgt = S.make_wcs(onx, ony, 150.0004, 2.0003, 11.0, S.PIXSCALE * 0.93)
+    d = torch.from_numpy(img[None]).cuda()
+    out, foot = P.dfr_reproject(d, [src], tgt, (ony, onx), 1, edge=P.EDGE_PAPER, footprint=True)
+    plain = P.dfr_reproject(d, [src], tgt, (ony, onx), 1, edge=P.EDGE_PAPER)
+    assert torch.equal(torch.nan_to_num(plain, nan=-7.0), torch.nan_to_num(out, nan=-7.0))
+    out, foot = out.cpu().numpy()[0], foot.cpu().numpy()[0]
+    xo, yo = oracle.src_coords(tgt, src, ony, onx)
+    ref, rfoot = oracle.interp_paper(img, xo.ravel(), yo.ravel(), 1)
+    rfoot = rfoot.reshape(ony, onx)
+    near = ((np.abs(xo + 1) < PR.EDGE_BAND) | (np.abs(xo - snx) < PR.EDGE_BAND)
+            | (np.abs(yo + 1) < PR.EDGE_BAND) | (np.abs(yo - sny) < PR.EDGE_BAND))
+    assert np.array_equal((foot > 0)[~near], (rfoot > 0)[~near])
+    assert np.abs(foot - rfoot)[~near].max() <= PR.COORD_TOL
+    part = (rfoot > 0) & (rfoot < 1)
+    assert part.sum() > 300 and np.abs(foot - rfoot)[part & ~near].max() <= PR.COORD_TOL     # the linear rim is exercised
+    assert np.array_equal(np.isnan(out)[~near], (foot == 0)[~near])          # the array is valid exactly where foot > 0
+    o0, f0 = P.dfr_reproject(d, [src], tgt, (ony, onx), 0, edge=P.EDGE_PAPER, footprint=True)
+    _, f0o = oracle.interp_paper(img, xo.ravel(), yo.ravel(), 0)
+    band = PR.edge_band(xo, yo, sny, snx)
+    assert np.array_equal(f0.cpu().numpy()[0][~band], f0o.reshape(ony, onx)[~band].astype(np.float32))
+    # the Python drop-in returns (array, footprint) (PAPER.md:27)
+    hdr = {"CRPIX1": src.crpix[0], "CRPIX2": src.crpix[1], "CRVAL1": src.crval[0], "CRVAL2": src.crval[1],
+           "CD1_1": src.cd[0], "CD1_2": src.cd[1], "CD2_1": src.cd[2], "CD2_2": src.cd[3]}
+    thdr = {"CRPIX1": tgt.crpix[0], "CRPIX2": tgt.crpix[1], "CRVAL1": tgt.crval[0], "CRVAL2": tgt.crval[1],
+            "CD1_1": tgt.cd[0], "CD1_2": tgt.cd[1], "CD2_1": tgt.cd[2], "CD2_2": tgt.cd[3]}
+    arr, fp = P.calculate_reprojection((img, hdr), thdr, (ony, onx), "bilinear", return_footprint=True)
+    assert arr.shape == fp.shape == (ony, onx) and set(np.unique(fp)) <= {0.0, 1.0}
+    assert np.array_equal(np.isnan(arr), fp == 0)
+
+
+def test_multi_device_entry_points_on_one_gpu(P):
+    """§8(e): dfr_reproject_host_multi / dfr_stack_host_multi shard the exposures over the listed
+    devices; listing device 0 twice (and three times) runs the whole multi-shard path — shard
+    threads, one pipeline per shard, peer copy + add for the stack — on a single GPU. The
+    per-exposure result must equal the single-device call bit for bit; the stack up to float32
+    re-association of the per-shard partial sums."""
+    w = S.config2(batch=7, n=512, nstars=200)
+    src = torch.from_numpy(w.images).pin_memory()
+    one = P.dfr_reproject_host(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1, batch=2).numpy().copy()
+    st1 = P.dfr_last_stats()
+    for devs in ([0], [0, 0], [0, 0, 0]):
+        multi = P.dfr_reproject_host(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1, batch=2, devices=devs).numpy()
+        assert np.array_equal(np.nan_to_num(multi, nan=-1), np.nan_to_num(one, nan=-1)), devs
+        st = P.dfr_last_stats()
+        assert st["tiles_fast"] == st1["tiles_fast"] and st["tiles_empty"] == st1["tiles_empty"]
+    wts = np.arange(1, 8, dtype=np.float32) / 4
+    s1, c1 = P.dfr_stack_host(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1, weights=wts, batch=3)
+    s2, c2 = P.dfr_stack_host(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1, weights=wts, batch=3, devices=[0, 0, 0])
+    assert torch.equal(c1, c2) and torch.allclose(s1, s2, rtol=2e-6, atol=1e-3)
+    so, wo = oracle.stack(w.images, w.src_wcs, w.tgt_wcs, w.shape_out, 1, wts)
+    band = np.zeros(w.shape_out, dtype=bool)
+    for e in range(7):
+        xo, yo = oracle.src_coords(w.tgt_wcs, w.src_wcs[e], *w.shape_out)
+        band |= PR.edge_band(xo, yo, *w.images.shape[1:])
+    assert np.array_equal(c2.numpy()[~band], wo[~band])
+    assert np.abs(s2.numpy() - so)[~band].max() <= PR.VALUE_TOL * max(PR.dyn_range(im) for im in w.images) * wts.sum()
+    with pytest.raises(P.DfrError):
+        P.dfr_reproject_host(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1, devices=[torch.cuda.device_count()])
+    P.dfr_release()                                  # frees the idle pipelines; the next call rebuilds them
+    again = P.dfr_reproject_host(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1, batch=4).numpy()
+    assert np.array_equal(np.nan_to_num(again, nan=-1), np.nan_to_num(one, nan=-1))
+
+
+def test_two_devices_from_one_thread(P):
+    """The library's per-call state (events, mapped counters, scratch pool) is keyed by device: a
+    thread that calls on cuda:0 and then on cuda:1 must get the same results on both."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    w = S.config0()
+    outs = []
+    for dev in (0, 1, 0):
+        src = torch.from_numpy(w.images).to(f"cuda:{dev}")
+        outs.append(P.dfr_reproject(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1).cpu())
+        with torch.cuda.device(dev):
+            assert P.dfr_last_stats()["tiles_fast"] == 64
+    assert torch.equal(torch.nan_to_num(outs[0]), torch.nan_to_num(outs[1]))
+    assert torch.equal(torch.nan_to_num(outs[0]), torch.nan_to_num(outs[2]))
+    src = torch.from_numpy(w.images).pin_memory()
+    a = P.dfr_reproject_host(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1, devices=[0, 1])
+    assert torch.equal(torch.nan_to_num(a), torch.nan_to_num(outs[0]))
+
+
+def test_many_exposures_call_does_not_block_the_host(P):
+    """include/dfr.h promises 'return after enqueue'. The per-call constants (984 B per exposure)
+    are staged through pinned memory, so a 128-exposure call (> 64 KB of constants) must return
+    while an earlier kernel on the same stream is still running (a pageable cudaMemcpyAsync of
+    that size would wait for it)."""
+    import time
+    n = 128
+    rng = np.random.default_rng(3)
+    img = S.make_image(64, 64, 5, rng)
+    srcs = [S.make_wcs(64, 64, 150.0 + 1e-4 * k, 2.0, 0.1 * k, S.PIXSCALE) for k in range(n)]
+    tgt = S.make_wcs(64, 64, 150.0, 2.0, 0.0, S.PIXSCALE)
+    d = torch.from_numpy(np.repeat(img[None], n, 0)).cuda()
+    out = torch.empty((n, 64, 64), dtype=torch.float32, device="cuda")
+    P.dfr_reproject(d, srcs, tgt, (64, 64), 1, out=out)          # warm: pools, staging ring
+    torch.cuda.synchronize()
+    ws, tw = P.pack_wcs_array(srcs), P.pack_wcs(tgt)
+    torch.cuda._sleep(int(4e8))                                  # ~0.2 s of GPU time on the current stream
+    t0 = time.perf_counter()
+    P.dfr_reproject(d, ws, tw, (64, 64), 1, out=out)
+    dt = time.perf_counter() - t0
+    still_running = not torch.cuda.current_stream().query()
+    torch.cuda.synchronize()
+    assert still_running and dt < 0.05, (still_running, dt)
