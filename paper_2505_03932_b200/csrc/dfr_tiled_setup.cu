@@ -205,7 +205,9 @@ __device__ __forceinline__ int emit_tile(double (&Cx)[16], double (&Cy)[16], boo
     r.ix0 = r.iy0 = r.bx0 = r.by0 = r.bx1 = r.by1 = 0;
     double bx = 0.0, by = 0.0;
     if (finite && fabs(xmin) < 1e9 && fabs(xmax) < 1e9 && fabs(ymin) < 1e9 && fabs(ymax) < 1e9) {
-        bx = floor(Cx[0]); by = floor(Cy[0]);
+        // EVEN integer base: the main kernel rounds the tile-relative coordinate x - ix0 half-to-even
+        // (nearest neighbour), which is the rounding of x itself only when ix0 is even
+        bx = 2.0 * floor(0.5 * Cx[0]); by = 2.0 * floor(0.5 * Cy[0]);
         r.ix0 = (int)bx; r.iy0 = (int)by;
         r.bx0 = (int)floor(xmin); r.bx1 = (int)floor(xmax);
         r.by0 = (int)floor(ymin); r.by1 = (int)floor(ymax);

@@ -610,3 +610,34 @@ def test_many_exposures_call_does_not_block_the_host(P):
     still_running = not torch.cuda.current_stream().query()
     torch.cuda.synchronize()
     assert still_running and dt < 0.05, (still_running, dt)
+
+
+def test_nearest_ties_round_half_even_on_both_paths(P):
+    """Reading G8: nearest neighbour rounds half to even. A pure half-pixel CRPIX shift (the
+    paper's demo offset, without its rotation) puts EVERY source coordinate on an
+    exact tie x = k + 0.5; the tiled path (which rounds a tile-relative coordinate) must pick
+    the pixel the oracle's rint picks on the exact half-integer — no tie band excluded. (The
+    fp64 per-pixel path carries ~1e-10 px of rounding noise around the tie, so it may pick
+    either neighbour: it is only required to pick one of the two.)"""
+    rng = np.random.default_rng(8)
+    img = S.make_image(96, 128, 20, rng)
+    src = S.make_wcs(128, 96, 150.0, 2.0, 0.0, S.PIXSCALE)
+    for sx, sy in ((0.5, 0.0), (0.0, 0.5), (0.5, 0.5), (3.5, -2.5)):
+        tgt = src.copy()
+        tgt.crpix = (src.crpix[0] + sx, src.crpix[1] + sy)
+        d = torch.from_numpy(img[None]).cuda()
+        a = P.dfr_reproject(d, [src], tgt, None, 0, path=P.PATH_AUTO).cpu().numpy()[0]
+        assert P.dfr_last_stats()["tiles_fast"] > 0
+        x = P.dfr_reproject(d, [src], tgt, None, 0, path=P.PATH_EXACT).cpu().numpy()[0]
+        xo, yo = oracle.src_coords(tgt, src, 96, 128)
+        exact_tie = (np.abs(xo - np.floor(xo) - 0.5) < 1e-5) | (np.abs(yo - np.floor(yo) - 0.5) < 1e-5)
+        assert exact_tie.mean() > 0.9                     # the geometry really sits on the ties
+        ref = oracle.interp(img, np.round(xo * 2).ravel() / 2, np.round(yo * 2).ravel() / 2, 0).reshape(96, 128)
+        inside = ~PR.edge_band(np.round(xo * 2) / 2, np.round(yo * 2) / 2, 96, 128)
+        assert np.array_equal(np.nan_to_num(a, nan=-1)[inside], np.nan_to_num(ref, nan=-1)[inside].astype(np.float32)), (sx, sy)
+        lo = oracle.interp(img, np.floor(xo).ravel(), np.floor(yo).ravel(), 0).reshape(96, 128)
+        hi = oracle.interp(img, np.ceil(xo - 1e-6).ravel(), np.ceil(yo - 1e-6).ravel(), 0).reshape(96, 128)
+        mixed1 = oracle.interp(img, np.floor(xo).ravel(), np.ceil(yo - 1e-6).ravel(), 0).reshape(96, 128)
+        mixed2 = oracle.interp(img, np.ceil(xo - 1e-6).ravel(), np.floor(yo).ravel(), 0).reshape(96, 128)
+        okx = (x == lo) | (x == hi) | (x == mixed1) | (x == mixed2) | np.isnan(x)
+        assert okx[inside].all(), (sx, sy)
