@@ -288,7 +288,8 @@ int dfr_release(void);
 enum { DFR_PROBE_FFMA = 0, DFR_PROBE_FFMA2 = 1, DFR_PROBE_FADD2_RM = 2, DFR_PROBE_DFMA = 3,
        DFR_PROBE_IMAD = 4, DFR_PROBE_LOP3 = 5, DFR_PROBE_LDS = 6,
        DFR_PROBE_FFMA_FFMA2 = 7, DFR_PROBE_FFMA2_IMAD = 8, DFR_PROBE_FFMA2_LOP3 = 9,
-       DFR_PROBE_COUNT = 10 };
+       DFR_PROBE_FFMA_3REG = 10, DFR_PROBE_FFMA2_3REG = 11,   /* three distinct, changing register operands */
+       DFR_PROBE_COUNT = 12 };
 int dfr_probe_rates(double *out, int32_t n);
 
 const char *dfr_strerror(int code);

@@ -370,7 +370,8 @@ def dfr_profile_last():
     return float(ms[0]), float(ms[1])
 
 
-PROBE_NAMES = ["FFMA", "FFMA2", "FADD2.RM", "DFMA", "IMAD", "LOP3", "LDS", "FFMA+FFMA2", "FFMA2+IMAD", "FFMA2+LOP3"]
+PROBE_NAMES = ["FFMA", "FFMA2", "FADD2.RM", "DFMA", "IMAD", "LOP3", "LDS", "FFMA+FFMA2", "FFMA2+IMAD", "FFMA2+LOP3",
+               "FFMA 3-reg", "FFMA2 3-reg"]
 
 
 def dfr_probe_rates() -> dict:

@@ -356,24 +356,25 @@ int stack_host_impl(PipeLease &L, const float *src_host, int32_t n, int32_t src_
     int rc = pipe_begin(L, nb, in_px * batch * sizeof(float), 2 * out_bytes, 0);
     if (rc != DFR_OK) return rc;
     float *dsum = L.p->slot[0].dout, *dwsum = dsum + (size_t)out_ny * out_nx;
-    cudaEvent_t zeroed = nullptr;
-    cudaError_t err = cudaEventCreateWithFlags(&zeroed, cudaEventDisableTiming);
-    if (err == cudaSuccess) err = cudaMemsetAsync(dsum, 0, 2 * out_bytes, L.p->slot[0].st);
-    if (err == cudaSuccess) err = cudaEventRecord(zeroed, L.p->slot[0].st);
-    for (int k = 1; k < L.used && err == cudaSuccess; ++k) err = cudaStreamWaitEvent(L.p->slot[k].st, zeroed, 0);
+    // `turn`: the stacking kernels add into sum / wsum with plain read-modify-writes (one owner per
+    // pixel), so batch b's kernels wait for batch b - 1's; the uploads, which are what the pipeline
+    // exists for, still overlap them. The first batch overwrites (no memset).
+    cudaEvent_t turn = nullptr;
+    cudaError_t err = cudaEventCreateWithFlags(&turn, cudaEventDisableTiming);
     if (err != cudaSuccess) rc = cuda_fail(err, "pipeline start");
     for (int b = 0; b < nb && rc == DFR_OK; ++b) {
         Slot &s = L.p->slot[b % kSlots];
         const int32_t e0 = b * batch, ne = (n - e0 < batch) ? n - e0 : batch;
-        // the slot's stream orders its own reuse: H2D(b) waits for the kernels of b - kSlots;
-        // batches of different slots add into sum / wsum concurrently (atomic adds)
+        // the slot's stream orders its own reuse: H2D(b) waits for the kernels of b - kSlots
         err = cudaMemcpyAsync(s.din, src_host + in_px * e0, in_px * ne * sizeof(float), cudaMemcpyHostToDevice, s.st);
+        if (err == cudaSuccess && b > 0) err = cudaStreamWaitEvent(s.st, turn, 0);
         if (err != cudaSuccess) { rc = cuda_fail(err, "H2D"); break; }
         rc = stack_impl(s.din, ne, src_ny, src_nx, src_wcs + e0, tgt_wcs, out_ny, out_nx, order,
-                        weights ? weights + e0 : nullptr, dsum, dwsum, 1, s.st);
+                        weights ? weights + e0 : nullptr, dsum, dwsum, b > 0 ? 1 : 0, s.st);
+        if (rc == DFR_OK && (err = cudaEventRecord(turn, s.st)) != cudaSuccess) rc = cuda_fail(err, "pipeline order");
     }
     rc = pipe_end(L, rc);
-    if (zeroed) cudaEventDestroy(zeroed);
+    if (turn) cudaEventDestroy(turn);
     if (rc != DFR_OK) return rc;
     if (keep) { *keep = dsum; return DFR_OK; }
     err = cudaMemcpy(sum_host, dsum, out_bytes, cudaMemcpyDeviceToHost);

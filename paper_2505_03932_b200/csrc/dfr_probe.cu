@@ -108,6 +108,11 @@ probe_kernel(int iters, long long *__restrict__ cycles, float *__restrict__ sink
                     p[k] = p_fma2(p[k], pa, pb);
                     u[k] = p_imad(u[k], 3u, u[(k + 1) % kChains]);
                 }
+                // three DISTINCT, changing register operands per instruction (no operand-reuse hits):
+                // what the interpolation code looks like, unlike the chains above whose multiplier and
+                // addend never change
+                if (KIND == DFR_PROBE_FFMA_3REG) f[k] = p_fma(f[(k + 1) % kChains], f[(k + 2) % kChains], f[k]);
+                if (KIND == DFR_PROBE_FFMA2_3REG) p[k] = p_fma2(p[(k + 1) % kChains], p[(k + 2) % kChains], p[k]);
                 if (KIND == DFR_PROBE_FFMA2_LOP3) {
                     p[k] = p_fma2(p[k], pa, pb);
                     u[k] = p_lop(u[k], u[(k + 1) % kChains], 0x5a5a5a5au);
@@ -135,7 +140,7 @@ static cudaError_t run_probe(int sms, int iters, long long *dcyc, float *dsink, 
     std::vector<long long> h((size_t)blocks);
     if ((err = cudaMemcpy(h.data(), dcyc, sizeof(long long) * (size_t)blocks, cudaMemcpyDeviceToHost)) != cudaSuccess) return err;
     const long long worst = *std::max_element(h.begin(), h.end());
-    const int per_slot = (KIND >= DFR_PROBE_FFMA_FFMA2) ? 2 : 1;         // thread-level INSTRUCTIONS per chain step
+    const int per_slot = (KIND >= DFR_PROBE_FFMA_FFMA2 && KIND <= DFR_PROBE_FFMA2_LOP3) ? 2 : 1;         // thread-level INSTRUCTIONS per chain step
     const double instr = (double)iters * kUnroll * kChains * per_slot * kProbeThreads * kBlocksPerSm;
     *instr_per_clk_sm = instr / (double)worst;
     return cudaSuccess;
@@ -163,6 +168,8 @@ cudaError_t probe_rates(double *out /* [DFR_PROBE_COUNT] thread-instructions per
     DFR_RUN(DFR_PROBE_FFMA_FFMA2);
     DFR_RUN(DFR_PROBE_FFMA2_IMAD);
     DFR_RUN(DFR_PROBE_FFMA2_LOP3);
+    DFR_RUN(DFR_PROBE_FFMA_3REG);
+    DFR_RUN(DFR_PROBE_FFMA2_3REG);
 #undef DFR_RUN
     cudaFree(dcyc);
     cudaFree(dsink);

@@ -78,7 +78,9 @@ cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const Sourc
 void free_scratch(Scratch &sc, cudaStream_t st);
 cudaError_t prepare_tiled(const float *src, int n, int sny, int snx, const TargetDev &tgt,
                           const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx,
-                          int order, cudaStream_t st, int32_t *host_stats, int stats_add, Prepared &R);
+                          int order, cudaStream_t st, int32_t *host_stats, int stats_add, Prepared &R,
+                          int span_tiles = CTA_T /* the staged box serves span_tiles x span_tiles tiles */,
+                          size_t max_box_bytes = kMaxBoxBytes);
 
 cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
                                    const TargetDev &tgt, const SourceDev *srcdev,

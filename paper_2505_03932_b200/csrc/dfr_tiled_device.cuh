@@ -320,6 +320,14 @@ struct StoreSink {
         orow[3 * opitch] = v3;
         orow += 4 * opitch;
     }
+    __device__ __forceinline__ void rows4p(f32x2 va, f32x2 vb)
+    {
+        float v0, v1, v2, v3;
+        unpk2(va, v0, v1);
+        unpk2(vb, v2, v3);
+        rows4(v0, v1, v2, v3);
+    }
+    __device__ __forceinline__ void set_uniform() {}
     __device__ __forceinline__ void row1(float v)
     {
         *orow = v;
@@ -344,10 +352,7 @@ __device__ __forceinline__ void interior_rows(const f32x2 (&X2)[4], const f32x2 
         d = add2(d, step);
         const f32x2 vb = interior_pair<ORDER, DEG>(X2, Y2, d, pitch4, K);
         d = add2(d, step);
-        float v0, v1, v2, v3;
-        unpk2(va, v0, v1);
-        unpk2(vb, v2, v3);
-        sink.rows4(v0, v1, v2, v3);
+        sink.rows4p(va, vb);
     }
 }
 
@@ -416,6 +421,7 @@ __device__ __forceinline__ void warp_tile(const TiledParams &P, const TargetDev 
         const int top = (ORDER == DFR_NEAREST) ? 1 : 0;          // rint(x) <= floor(x) + 1
         const bool interior = bx0 >= Alx && bx1 + top <= Ahx && by0 >= Aly && by1 + top <= Ahy;
         if (interior) {
+            sink.set_uniform();                  // no pixel of this tile can leave the footprint
             f32x2 X2[4], Y2[4];
 #pragma unroll
             for (int q = 0; q < 4; ++q) { X2[q] = splat2(X[q]); Y2[q] = splat2(Y[q]); }

@@ -378,14 +378,14 @@ static EncodeTiledFn get_encode()
 }
 
 
-// Source-pixel extent of a 64x64 output tile, from the Jacobian of the map probed in fp64
+// Source-pixel extent of an output region of span_tiles x span_tiles tiles, from the Jacobian of the map probed in fp64
 // on the host at the centre of the output grid, per exposure (3 map evaluations each; the
 // Jacobian varies by well under 1 % over a frame, the caller adds 2 % + fixed margins, and
 // the kernel checks every pixel against the staged box anyway). False if no probe is finite.
-static bool probe_extent(const TargetDev &tgt, const SourceDev *hs, int n, int ony, int onx,
+static bool probe_extent(const TargetDev &tgt, const SourceDev *hs, int n, int ony, int onx, int span_tiles,
                          double &ext_x, double &ext_y)
 {
-    const double span = TS * CTA_T - 1;
+    const double span = TS * span_tiles - 1;
     const double ci = 0.5 * (onx - 1), cj = 0.5 * (ony - 1), h = 16.0;
     double U0, V0, U1, V1, U2, V2;
     target_uv(tgt, ci, cj, U0, V0);
@@ -462,7 +462,8 @@ void free_scratch(Scratch &sc, cudaStream_t st)
 
 cudaError_t prepare_tiled(const float *src, int n, int sny, int snx, const TargetDev &tgt,
                                  const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx,
-                                 int order, cudaStream_t st, int32_t *host_stats, int stats_add, Prepared &R)
+                                 int order, cudaStream_t st, int32_t *host_stats, int stats_add, Prepared &R,
+                                 int span_tiles, size_t max_box_bytes)
 {
     std::memset(&R.P, 0, sizeof R.P);
     std::memset(&R.tmap, 0, sizeof R.tmap);
@@ -484,14 +485,14 @@ cudaError_t prepare_tiled(const float *src, int n, int sny, int snx, const Targe
     no_stage = std::getenv("DFR_NO_STAGE") != nullptr;
     if (const char *a = std::getenv("DFR_BW_ALIGN")) bw_align = std::atoi(a);
 #endif
-    if (!no_stage && enc && (snx % 4 == 0) && ((uintptr_t)src % 16 == 0) && probe_extent(tgt, srchost, n, ony, onx, ex, ey)) {
+    if (!no_stage && enc && (snx % 4 == 0) && ((uintptr_t)src % 16 == 0) && probe_extent(tgt, srchost, n, ony, onx, span_tiles, ex, ey)) {
         // floor-range spread + taps + 1 px safety each side; + 3: the origin is rounded down
         // to a multiple of 4 floats; then the width itself is rounded up to 16 bytes
         int bw = ((int)std::ceil(ex * 1.02) + 2 + tlo + thi + 2 + 3 + 3) & ~3;
         const int bh = (int)std::ceil(ey * 1.02) + 2 + tlo + thi + 2;
         const int bwa = (bw + bw_align - 1) / bw_align * bw_align;
-        if (bwa <= 256 && (size_t)bwa * bh * sizeof(float) <= (size_t)kMaxBoxBytes) bw = bwa;
-        if (bw <= 256 && bh <= 256 && (size_t)bw * bh * sizeof(float) <= (size_t)kMaxBoxBytes) {
+        if (bwa <= 256 && (size_t)bwa * bh * sizeof(float) <= max_box_bytes) bw = bwa;
+        if (bw <= 256 && bh <= 256 && (size_t)bw * bh * sizeof(float) <= max_box_bytes) {
             const cuuint64_t dims[3] = {(cuuint64_t)snx, (cuuint64_t)sny, (cuuint64_t)n};
             const cuuint64_t strides[2] = {(cuuint64_t)snx * 4, (cuuint64_t)snx * sny * 4};
             const cuuint32_t boxd[3] = {(cuuint32_t)bw, (cuuint32_t)bh, 1};
