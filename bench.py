@@ -275,10 +275,21 @@ def main():
     ap.add_argument("--load-seconds", type=float, default=0.7,
                     help="untimed back-to-back steps before (and half as long after) the timed region")
     ap.add_argument("--path", default="auto", choices=["auto", "exact"])
-    ap.add_argument("--mode", default="reproject", choices=["reproject", "stack"],
+    ap.add_argument("--mode", default="reproject", choices=["reproject", "stack", "probes"],
                     help="stack: the fused reproject-and-stack entry point (SURVEY.md §8(f) f1) on the same "
-                         "workload; not the headline metric")
+                         "workload; probes: the register-only instruction-rate probes; neither is the headline metric")
     args = ap.parse_args()
+    if args.mode == "probes":
+        # register-only instruction-rate probes (dfr_probe_rates): the measured ALU-side denominators
+        import torch
+        import paper_2505_03932_b200 as P
+        P.lib()
+        torch.cuda.set_device(0)
+        rates = P.dfr_probe_rates()
+        print(json.dumps({"probe": "thread-level instructions per clock per SM (32 warps per SM, register-only chains)",
+                          "gpu": torch.cuda.get_device_name(0), "sms": torch.cuda.get_device_properties(0).multi_processor_count,
+                          "rates": rates}))
+        return 0
     if args.mode == "stack" and args.impl == "ours":
         return run_stack(args)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -50,6 +50,15 @@ extern "C" {
 
 #define DFR_SIP_MAX_ORDER 9                     /* SIP convention limit (Shupe 2005) */
 #define DFR_SIP_DIM (DFR_SIP_MAX_ORDER + 1)
+/* ap_order = bp_order = DFR_SIP_INVERSE_EXACT: the WCS carries no inverse polynomials and the
+ * library inverts the forward distortion itself (PAPER.md:51 assumes SIP_INV_A / SIP_INV_B exist;
+ * SURVEY.md §8(f) f4): wherever SIP_INV_A / SIP_INV_B would be applied it solves
+ *   u + A(u, v) = U,  v + B(u, v) = V
+ * for (u, v) in fp64 by fixed-point iteration to 1e-11 px (at most 32 steps: distortions whose
+ * gradient exceeds ~0.4 do not converge and give NaN). Exact where a fitted AP/BP is only as good
+ * as its order allows. On the tiled path the solve runs at the 25 sample points of a tile, not
+ * per pixel. */
+#define DFR_SIP_INVERSE_EXACT (-1)
 
 /* Packed WCS parameter set. POD, no pointers,
  * 3280 bytes, no padding. Polynomial coefficient of u^p v^q is stored at
@@ -59,7 +68,7 @@ typedef struct dfr_wcs {
     double  crpix[2];          /* CRPIX1, CRPIX2 — FITS 1-based */
     double  crval[2];          /* ra0, dec0 in degrees              */
     double  cd[4];             /* CD1_1, CD1_2, CD2_1, CD2_2, deg/pixel */
-    int32_t a_order, b_order, ap_order, bp_order;
+    int32_t a_order, b_order, ap_order, bp_order;   /* 0..9; ap = bp = DFR_SIP_INVERSE_EXACT allowed */
     double  a [DFR_SIP_DIM * DFR_SIP_DIM];     /* SIP_A   */
     double  b [DFR_SIP_DIM * DFR_SIP_DIM];     /* SIP_B                          */
     double  ap[DFR_SIP_DIM * DFR_SIP_DIM];     /* SIP_INV_A      */
@@ -74,7 +83,7 @@ typedef enum dfr_status {
     DFR_ERR_NULL = -1,           /* a required pointer is NULL                    */
     DFR_ERR_SHAPE = -2,          /* n < 1, a dimension < 1, or ny*nx >= 2^31      */
     DFR_ERR_ORDER = -3,          /* order not in {0, 1, 3}                        */
-    DFR_ERR_SIP_ORDER = -4,      /* a SIP order outside [0, DFR_SIP_MAX_ORDER]    */
+    DFR_ERR_SIP_ORDER = -4,      /* a SIP order outside [0, DFR_SIP_MAX_ORDER] (or a lone DFR_SIP_INVERSE_EXACT) */
     DFR_ERR_SINGULAR_CD = -5,    /* det(CD) == 0 or not finite                    */
     DFR_ERR_NONFINITE_WCS = -6,  /* NaN/Inf in crpix, crval, cd or used SIP terms */
     DFR_ERR_ALIAS = -7,          /* out overlaps src_batch                        */
@@ -229,8 +238,8 @@ int dfr_pix2world(const dfr_wcs *w, const double *x, const double *y, int64_t np
                   double *ra_deg, double *dec_deg, void *stream);
 
 /* Sky -> pixel with WCS *w (HOST). Literal formulas of PAPER.md:101-121 in
- * fp64; uses AP/BP only (no iterative inverse; absent AP/BP => no inverse
- * distortion). Points >= 90 degrees from CRVAL give NaN. */
+ * fp64; uses AP/BP (absent AP/BP => no inverse distortion; DFR_SIP_INVERSE_EXACT =>
+ * the forward distortion inverted by iteration). Points >= 90 degrees from CRVAL give NaN. */
 int dfr_world2pix(const dfr_wcs *w, const double *ra_deg, const double *dec_deg, int64_t npts,
                   double *x, double *y, void *stream);
 

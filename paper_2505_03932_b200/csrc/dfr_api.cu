@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <string>
@@ -100,27 +101,44 @@ struct CallConsts {
     SourceDev *dsrc = nullptr;
     float *dweights = nullptr;
     void *block = nullptr;
-    void release(cudaStream_t st) { if (block) cudaFreeAsync(block, st); block = nullptr; }
+    PinnedSlot *slot = nullptr;
+    ConstsCopy cc;                       // set when the tiled path's first kernel is to do the upload
+    // after the call's last launch: the staging slot is free once the stream gets here
+    cudaError_t finish(cudaStream_t st)
+    {
+        cudaError_t err = cudaSuccess;
+        if (slot) err = stage_done(slot, st);
+        slot = nullptr;
+        if (block) cudaFreeAsync(block, st);
+        block = nullptr;
+        return err;
+    }
 };
 
+// by_kernel: leave the upload to the tiled path's first kernel (K.cc); otherwise enqueue a copy.
 static int upload_consts(DevCtx *c, int32_t n, const dfr_wcs *sw, const dfr_wcs *tw, bool with_weights,
-                         const float *weights, cudaStream_t st, CallConsts &K)
+                         const float *weights, cudaStream_t st, bool by_kernel, CallConsts &K)
 {
     make_target(tw, &K.tgt);
-    const size_t b_src = sizeof(SourceDev) * (size_t)n, bytes = b_src + (with_weights ? sizeof(float) * (size_t)n : 0);
-    PinnedSlot *slot = nullptr;
-    cudaError_t err = stage_acquire(c, bytes, &slot);
+    const size_t b_src = sizeof(SourceDev) * (size_t)n;
+    const size_t bytes = (b_src + (with_weights ? sizeof(float) * (size_t)n : 0) + 15) & ~(size_t)15;
+    cudaError_t err = stage_acquire(c, bytes, &K.slot);
     if (err != cudaSuccess) return cuda_fail(err, "pinned staging buffer");
-    SourceDev *h = static_cast<SourceDev *>(slot->host);
+    SourceDev *h = static_cast<SourceDev *>(K.slot->host);
     for (int32_t e = 0; e < n; ++e) make_source(tw, &sw[e], &h[e]);
     if (with_weights) {
-        float *hw = reinterpret_cast<float *>(static_cast<char *>(slot->host) + b_src);
+        float *hw = reinterpret_cast<float *>(static_cast<char *>(K.slot->host) + b_src);
         for (int32_t e = 0; e < n; ++e) hw[e] = weights ? weights[e] : 1.0f;
     }
     if ((err = scratch_alloc(&K.block, bytes, st)) != cudaSuccess) return cuda_fail(err, "scratch allocation (constants)");
-    err = cudaMemcpyAsync(K.block, slot->host, bytes, cudaMemcpyHostToDevice, st);
-    if (err == cudaSuccess) err = stage_done(slot, st);
-    if (err != cudaSuccess) { K.release(st); return cuda_fail(err, "cudaMemcpyAsync(constants)"); }
+    if (by_kernel) {
+        K.cc.src = K.slot->dev;
+        K.cc.dst = K.block;
+        K.cc.bytes = bytes;
+    } else if ((err = cudaMemcpyAsync(K.block, K.slot->host, bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) {
+        K.finish(st);
+        return cuda_fail(err, "cudaMemcpyAsync(constants)");
+    }
     K.hsrc = h;
     K.dsrc = static_cast<SourceDev *>(K.block);
     K.dweights = with_weights ? reinterpret_cast<float *>(static_cast<char *>(K.block) + b_src) : nullptr;
@@ -141,12 +159,13 @@ static int reproject_impl(const float *src, int32_t n, int32_t sny, int32_t snx,
     c->prof.enabled = g_profile;
     g_last.pending = false;
     g_last.ctx = c;
+    // a grid taller than 65535 CTA tiles (out_ny > 4.19 M rows) does not fit the tiled launch
+    const bool exact = path == DFR_PATH_EXACT || !tiled_grid_fits(ony);
     CallConsts K;
-    int rc = upload_consts(c, n, sw, tw, false, nullptr, st, K);
+    int rc = upload_consts(c, n, sw, tw, false, nullptr, st, !exact, K);
     if (rc != DFR_OK) return rc;
     TiledStats ts = {0, 0, 0, 0};
-    // a grid taller than 65535 CTA tiles (out_ny > 4.19 M rows) does not fit the tiled launch
-    if (path == DFR_PATH_EXACT || !tiled_grid_fits(ony)) {
+    if (exact) {
         if (c->prof.enabled) cudaEventRecord(c->prof.setup_begin, st), cudaEventRecord(c->prof.main_begin, st);
         err = launch_exact_reproject(src, n, sny, snx, K.tgt, K.dsrc, ony, onx, order, out, st, edge, foot);
         if (c->prof.enabled) cudaEventRecord(c->prof.main_end, st);
@@ -159,7 +178,7 @@ static int reproject_impl(const float *src, int32_t n, int32_t sny, int32_t snx,
     } else {
         err = launch_tiled_reproject(src, n, sny, snx, K.tgt, K.dsrc, K.hsrc, ony, onx, order, out, st,
                                      g_accumulate ? c->stream_totals : c->pinned_dev, g_accumulate ? 1 : 0,
-                                     &ts, &c->prof, edge, foot);
+                                     &ts, &c->prof, K.cc, edge, foot);
         if (g_accumulate) {
             g_stats_acc[3] += ts.kernels;
         } else {
@@ -169,7 +188,8 @@ static int reproject_impl(const float *src, int32_t n, int32_t sny, int32_t snx,
             g_last.pending = (err == cudaSuccess);
         }
     }
-    K.release(st);
+    const cudaError_t ferr = K.finish(st);
+    if (err == cudaSuccess) err = ferr;
     if (err != cudaSuccess) return cuda_fail(err, "reproject launch");
     return DFR_OK;
 }
@@ -189,14 +209,17 @@ static int stack_impl(const float *src_batch, int32_t n, int32_t src_ny, int32_t
     g_last.pending = false;
     g_last.ctx = c;
     CallConsts K;
-    int rc = upload_consts(c, n, src_wcs, tgt_wcs, true, weights, st, K);
+    int rc = upload_consts(c, n, src_wcs, tgt_wcs, true, weights, st, true, K);
     if (rc != DFR_OK) return rc;
     TiledStats ts = {0, 0, 0, 0};
     err = launch_tiled_stack(src_batch, n, src_ny, src_nx, K.tgt, K.dsrc, K.hsrc, out_ny, out_nx, order,
                              K.dweights, sum, wsum, accumulate != 0, st,
-                             g_accumulate ? c->stream_totals : c->pinned_dev, g_accumulate ? 1 : 0, &ts, &c->prof);
+                             g_accumulate ? c->stream_totals : c->pinned_dev, g_accumulate ? 1 : 0, &ts, &c->prof, K.cc);
     if (!g_accumulate && err == cudaSuccess) err = cudaEventRecord(c->done, st);
-    K.release(st);
+    {
+        const cudaError_t ferr = K.finish(st);
+        if (err == cudaSuccess) err = ferr;
+    }
     if (g_accumulate) {
         g_stats_acc[3] += ts.kernels;
     } else {
@@ -494,14 +517,18 @@ int dfr_src_coords(int32_t n, int32_t src_ny, int32_t src_nx,
     DevCtx *c = nullptr;
     cudaError_t err = current_ctx(&c);
     if (err != cudaSuccess) return cuda_fail(err, "device context");
+    const bool exact = path == DFR_PATH_EXACT || !tiled_grid_fits(out_ny);
     CallConsts K;
-    rc = upload_consts(c, n, src_wcs, tgt_wcs, false, nullptr, st, K);
+    rc = upload_consts(c, n, src_wcs, tgt_wcs, false, nullptr, st, !exact, K);
     if (rc != DFR_OK) return rc;
-    if (path == DFR_PATH_EXACT || !tiled_grid_fits(out_ny))
+    if (exact)
         err = launch_exact_coords(n, K.tgt, K.dsrc, out_ny, out_nx, x, y, st);
     else
-        err = launch_tiled_coords(n, src_ny, src_nx, K.tgt, K.dsrc, K.hsrc, out_ny, out_nx, order, x, y, st);
-    K.release(st);
+        err = launch_tiled_coords(n, src_ny, src_nx, K.tgt, K.dsrc, K.hsrc, out_ny, out_nx, order, x, y, st, K.cc);
+    {
+        const cudaError_t ferr = K.finish(st);
+        if (err == cudaSuccess) err = ferr;
+    }
     if (err != cudaSuccess) return cuda_fail(err, "src_coords launch");
     return DFR_OK;
 }

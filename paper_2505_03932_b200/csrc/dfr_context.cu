@@ -115,7 +115,12 @@ cudaError_t stage_acquire(DevCtx *c, size_t bytes, PinnedSlot **slot)
         s.cap = 0;
         size_t cap = 4096;
         while (cap < bytes) cap *= 2;
-        if ((err = cudaHostAlloc(&s.host, cap, cudaHostAllocDefault)) != cudaSuccess) return err;
+        if ((err = cudaHostAlloc(&s.host, cap, cudaHostAllocMapped)) != cudaSuccess) return err;
+        if ((err = cudaHostGetDevicePointer(&s.dev, s.host, 0)) != cudaSuccess) {
+            cudaFreeHost(s.host);
+            s.host = nullptr;
+            return err;
+        }
         s.cap = cap;
     }
     *slot = &s;

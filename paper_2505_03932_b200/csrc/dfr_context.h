@@ -14,11 +14,12 @@ namespace dfr {
 // work in the stream the way a pageable cudaMemcpyAsync above 64 KB does.
 struct PinnedSlot {
     void *host = nullptr;
+    void *dev = nullptr;                // the same memory as the device sees it (mapped)
     size_t cap = 0;
     cudaEvent_t copied = nullptr;       // recorded after the last upload out of this slot
     bool used = false;
 };
-constexpr int kRingSlots = 4;
+constexpr int kRingSlots = 16;     // a host thread may run this many calls ahead of the device
 
 // Per (host thread, device) state.
 struct DevCtx {
@@ -41,8 +42,9 @@ cudaError_t ensure_profile_events(DevCtx *c);
 // application's default pool is left untouched). Free with cudaFreeAsync.
 cudaError_t scratch_alloc(void **p, size_t bytes, cudaStream_t st);
 
-// A pinned staging buffer of at least `bytes` whose previous upload has completed. Fill it,
-// enqueue the cudaMemcpyAsync out of it on `st`, then call stage_done(slot, st).
+// A pinned, device-mapped staging buffer of at least `bytes` whose previous use has completed.
+// Fill it, enqueue the work that reads it on `st` (a cudaMemcpyAsync, or a kernel reading
+// slot->dev), then call stage_done(slot, st).
 cudaError_t stage_acquire(DevCtx *c, size_t bytes, PinnedSlot **slot);
 cudaError_t stage_done(PinnedSlot *slot, cudaStream_t st);
 

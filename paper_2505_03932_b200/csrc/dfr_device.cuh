@@ -69,6 +69,26 @@ __host__ __device__ __forceinline__ void target_uv(const TargetDev &t, double i,
     V = v + poly_eval(t.b, u, v);
 }
 
+// DFR_SIP_INVERSE_EXACT: solve u + A(u, v) = U, v + B(u, v) = V by fixed-point iteration
+// (u, v) <- (U - A(u, v), V - B(u, v)) to 1e-11 px. Contraction rate = the distortion's gradient
+// (1e-3 ... 3e-2 for real optics): 4-8 steps; NaN if 32 steps do not converge.
+constexpr int kInvIters = 32;
+constexpr double kInvTol = 1e-11;
+template <class PA, class PB>
+__host__ __device__ __forceinline__ void invert_sip(PA polyA, PB polyB, double U, double V, double &u, double &v)
+{
+    u = U;
+    v = V;
+    bool done = false;
+    for (int it = 0; it < kInvIters && !done; ++it) {
+        const double un = U - polyA(u, v), vn = V - polyB(u, v);
+        done = fabs(un - u) + fabs(vn - v) < kInvTol;
+        u = un;
+        v = vn;
+    }
+    if (!done) u = v = NAN;                     // includes NaN input
+}
+
 // a3-a6: (U, V) -> fractional source pixel (x, y) for one exposure
 // (PAPER.md:91-121 in the projective form of dfr_host.cu). NaN when the sky
 // point is >= 90 deg from the source tangent point.
@@ -84,6 +104,14 @@ __host__ __device__ __forceinline__ void source_xy(const SourceDev &s, double U,
     }
     const double rc = 1.0 / c;
     const double us = a * rc, vs = b * rc;
+    if (s.inv_exact) {
+        double u, v;
+        invert_sip([&](double p, double q) { return poly_eval(s.ap, p, q); },
+                   [&](double p, double q) { return poly_eval(s.bp, p, q); }, us, vs, u, v);
+        x = u + s.c1;
+        y = v + s.c2;
+        return;
+    }
     x = us + poly_eval(s.ap, us, vs) + s.c1;
     y = vs + poly_eval(s.bp, us, vs) + s.c2;
 }

@@ -51,7 +51,8 @@ static bool poly_finite(const double *c, int order)
 
 int validate_wcs(const dfr_wcs *w)
 {
-    const int32_t ords[4] = {w->a_order, w->b_order, w->ap_order, w->bp_order};
+    const bool inv_exact = w->ap_order == DFR_SIP_INVERSE_EXACT && w->bp_order == DFR_SIP_INVERSE_EXACT;
+    const int32_t ords[4] = {w->a_order, w->b_order, inv_exact ? 0 : w->ap_order, inv_exact ? 0 : w->bp_order};
     for (int k = 0; k < 4; ++k)
         if (ords[k] < 0 || ords[k] > DFR_SIP_MAX_ORDER) {
             set_error("SIP order %d outside [0, %d]", ords[k], DFR_SIP_MAX_ORDER);
@@ -68,7 +69,7 @@ int validate_wcs(const dfr_wcs *w)
             return DFR_ERR_NONFINITE_WCS;
         }
     if (!poly_finite(w->a, w->a_order) || !poly_finite(w->b, w->b_order) ||
-        !poly_finite(w->ap, w->ap_order) || !poly_finite(w->bp, w->bp_order)) {
+        !poly_finite(w->ap, ords[2]) || !poly_finite(w->bp, ords[3])) {
         set_error("non-finite SIP coefficient");
         return DFR_ERR_NONFINITE_WCS;
     }
@@ -140,8 +141,15 @@ void make_source(const dfr_wcs *t, const dfr_wcs *s, SourceDev *out)
     mat3(Es, T1, out->m);
     out->c1 = s->crpix[0] - 1.0;
     out->c2 = s->crpix[1] - 1.0;
-    pack_poly(s->ap, s->ap_order, &out->ap);
-    pack_poly(s->bp, s->bp_order, &out->bp);
+    out->inv_exact = (s->ap_order == DFR_SIP_INVERSE_EXACT) ? 1 : 0;
+    out->pad_ = 0;
+    if (out->inv_exact) {                               // the forward polynomials, inverted on the device
+        pack_poly(s->a, s->a_order, &out->ap);
+        pack_poly(s->b, s->b_order, &out->bp);
+    } else {
+        pack_poly(s->ap, s->ap_order, &out->ap);
+        pack_poly(s->bp, s->bp_order, &out->bp);
+    }
 }
 
 void make_sky(const dfr_wcs *w, SkyDev *out)
@@ -159,8 +167,10 @@ void make_sky(const dfr_wcs *w, SkyDev *out)
     out->cdi[3] = w->cd[0] / det;
     pack_poly(w->a, w->a_order, &out->a);
     pack_poly(w->b, w->b_order, &out->b);
-    pack_poly(w->ap, w->ap_order, &out->ap);
-    pack_poly(w->bp, w->bp_order, &out->bp);
+    out->inv_exact = (w->ap_order == DFR_SIP_INVERSE_EXACT) ? 1 : 0;
+    out->pad_ = 0;
+    pack_poly(w->ap, out->inv_exact ? 0 : w->ap_order, &out->ap);
+    pack_poly(w->bp, out->inv_exact ? 0 : w->bp_order, &out->bp);
 }
 
 // ---- inverse SIP fit ---------------------------------------

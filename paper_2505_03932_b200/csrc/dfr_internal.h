@@ -33,7 +33,9 @@ struct TargetDev {
 struct SourceDev {
     double m[9];
     double c1, c2;                          // crpix_s - 1
-    Poly   ap, bp;                          // SIP_INV_A, SIP_INV_B
+    Poly   ap, bp;                          // SIP_INV_A, SIP_INV_B; inv_exact: SIP_A, SIP_B
+    int32_t inv_exact;                      // DFR_SIP_INVERSE_EXACT: invert ap/bp (= A/B) by iteration
+    int32_t pad_;
 };
 
 // Full WCS for the literal-trig kernels (dfr_pix2world / dfr_world2pix).
@@ -41,6 +43,8 @@ struct SkyDev {
     double c1, c2, ra0, dec0;               // radians
     double cd[4], cdi[4];                   // CD and its inverse (deg/px, px/deg)
     Poly   a, b, ap, bp;
+    int32_t inv_exact;                      // DFR_SIP_INVERSE_EXACT: world2pix inverts a/b by iteration
+    int32_t pad_;
 };
 
 // ---- host side (dfr_host.cpp) ---------------------------------------------

@@ -67,9 +67,15 @@ world2pix_kernel(const SkyDev *__restrict__ wp, const double *__restrict__ ra_de
     const double up = -r * sp, vp = r * cp;
     double u = w.cdi[0] * up + w.cdi[1] * vp;
     double v = w.cdi[2] * up + w.cdi[3] * vp;
-    const double f = poly_eval(w.ap, u, v), g = poly_eval(w.bp, u, v);
-    u += f;
-    v += g;
+    if (w.inv_exact) {                                           // DFR_SIP_INVERSE_EXACT: invert A/B
+        const double U = u, V = v;
+        invert_sip([&](double p, double q) { return poly_eval(w.a, p, q); },
+                   [&](double p, double q) { return poly_eval(w.b, p, q); }, U, V, u, v);
+    } else {
+        const double f = poly_eval(w.ap, u, v), g = poly_eval(w.bp, u, v);
+        u += f;
+        v += g;
+    }
     x[k] = u + w.c1;
     y[k] = v + w.c2;
 }

@@ -37,6 +37,15 @@ struct ProfileEvents {
     bool enabled;
 };
 
+// Per-call constants that the first setup kernel copies from mapped pinned host memory into device
+// scratch (a copy-engine upload would put a cross-engine dependency in front of every call:
+// measured +8 us per C2 step). src == nullptr: nothing to copy.
+struct ConstsCopy {
+    const void *src = nullptr;          // device-visible address of the pinned staging buffer
+    void *dst = nullptr;                // device scratch
+    size_t bytes = 0;                   // multiple of 16
+};
+
 struct TiledParams {
     const float *src;
     float *out;
@@ -74,12 +83,12 @@ struct Prepared {
 
 cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const SourceDev *srcdev,
                       const SourceDev *srchost, int ony, int onx, cudaStream_t st,
-                      int32_t *host_stats, int stats_add, Scratch &sc, TiledParams &P);
+                      int32_t *host_stats, int stats_add, Scratch &sc, TiledParams &P, const ConstsCopy &cc);
 void free_scratch(Scratch &sc, cudaStream_t st);
 cudaError_t prepare_tiled(const float *src, int n, int sny, int snx, const TargetDev &tgt,
                           const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx,
                           int order, cudaStream_t st, int32_t *host_stats, int stats_add, Prepared &R,
-                          int span_tiles = CTA_T /* the staged box serves span_tiles x span_tiles tiles */,
+                          const ConstsCopy &cc, int span_tiles = CTA_T /* the staged box serves span_tiles x span_tiles tiles */,
                           size_t max_box_bytes = kMaxBoxBytes);
 
 cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
@@ -88,17 +97,18 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
                                    int ony, int onx, int order, float *out, cudaStream_t st,
                                    int32_t *host_stats /* 3 ints the setup kernel can write (mapped host or device memory), or NULL */,
                                    int stats_add /* 0: store the totals, 1: atomically add them (streaming) */,
-                                   TiledStats *stats, ProfileEvents *prof, int edge = DFR_EDGE_AREA,
+                                   TiledStats *stats, ProfileEvents *prof, const ConstsCopy &cc, int edge = DFR_EDGE_AREA,
                                    float *foot = nullptr /* DEVICE [n][ony][onx] footprint array, or NULL */);
 // dfr_reproject_stack: sum / wsum accumulated over the n exposures in one kernel.
 cudaError_t launch_tiled_stack(const float *src, int n, int sny, int snx, const TargetDev &tgt,
                                const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx, int order,
                                const float *dev_weights, float *sum, float *wsum, int accumulate,
-                               cudaStream_t st, int32_t *host_stats, int stats_add, TiledStats *stats, ProfileEvents *prof);
+                               cudaStream_t st, int32_t *host_stats, int stats_add, TiledStats *stats, ProfileEvents *prof,
+                               const ConstsCopy &cc);
 cudaError_t launch_stack_add(float *a, const float *b, long long n, cudaStream_t st);
 cudaError_t launch_stack_finalize(const float *sum, const float *wsum, long long npix, float *mean, cudaStream_t st);
 cudaError_t launch_tiled_coords(int n, int sny, int snx, const TargetDev &tgt,
                                 const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx, int order,
-                                double *x, double *y, cudaStream_t st);
+                                double *x, double *y, cudaStream_t st, const ConstsCopy &cc);
 
 }  // namespace dfr

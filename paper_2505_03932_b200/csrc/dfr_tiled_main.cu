@@ -11,6 +11,7 @@
 //                         staged box or touch the image rim, and all pixels of EXACT
 //                         tiles, take the exact/global-gather code of dfr_device.cuh.
 #include <algorithm>
+#include <atomic>
 #include <cstring>
 
 #include "dfr_tiled_device.cuh"
@@ -223,18 +224,31 @@ static cudaError_t launch_main(const TiledParams &P, const TargetDev &tgt, const
                                size_t smem, cudaStream_t st)
 {
     auto kern = tiled_reproject_kernel<ORDER, STAGE, EDGE>;
-    if (STAGE) {      // per device, cheap: set every time
-        cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxBoxBytes);
-        if (err != cudaSuccess) return err;
-    }
     if (P.ctas_y > 65535) return cudaErrorInvalidConfiguration;
     TiledParams Q = P;
     if (STAGE) {
-        int dev = 0, sms = 0, per_sm = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess &&
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 32 * CTA_T * CTA_T, smem) == cudaSuccess)
-            Q.prefetch_dist = sms * per_sm / 2;     // measured on B200, C2: flat optimum between 1/2 and 3/4 of a wave
+        // per (kernel, device): the shared-memory opt-in once, the resident-CTA count per box size
+        // (the occupancy query costs microseconds of host time per call otherwise)
+        constexpr int kDevs = 64, kSlots = kMaxBoxBytes / 1024 + 2;
+        static std::atomic<int> per_sm_cache[kDevs][kSlots];       // 0 = unknown; indexed by KB of box
+        static std::atomic<bool> opted_in[kDevs];
+        int dev = 0;
+        cudaError_t err = cudaGetDevice(&dev);
+        if (err != cudaSuccess) return err;
+        const int d = (dev >= 0 && dev < kDevs) ? dev : 0, slot = (int)std::min<size_t>((smem + 1023) / 1024, kSlots - 1);
+        if (!opted_in[d].load(std::memory_order_acquire) || dev != d) {
+            if ((err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxBoxBytes)) != cudaSuccess) return err;
+            opted_in[d].store(true, std::memory_order_release);
+        }
+        int waves = per_sm_cache[d][slot].load(std::memory_order_relaxed);
+        if (waves == 0 || dev != d) {
+            int sms = 0, per_sm = 0;
+            if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess &&
+                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 32 * CTA_T * CTA_T, (size_t)slot * 1024) == cudaSuccess)
+                waves = sms * per_sm;
+            per_sm_cache[d][slot].store(waves, std::memory_order_relaxed);
+        }
+        Q.prefetch_dist = waves / 2;        // measured on B200, C2: flat optimum between 1/2 and 3/4 of a wave
 #ifdef DFR_DEV_HOOKS                                                 // A-B timing builds only (never the shipped library)
         static const char *pd = std::getenv("DFR_PREFETCH");
         if (pd) Q.prefetch_dist = std::atoi(pd);
@@ -254,11 +268,11 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
                                    const SourceDev *srchost,
                                    int ony, int onx, int order, float *out, cudaStream_t st,
                                    int32_t *host_stats, int stats_add, TiledStats *stats, ProfileEvents *prof,
-                                   int edge, float *foot)
+                                   const ConstsCopy &cc, int edge, float *foot)
 {
     Prepared R;
     if (prof && prof->enabled) cudaEventRecord(prof->setup_begin, st);
-    cudaError_t err = prepare_tiled(src, n, sny, snx, tgt, srcdev, srchost, ony, onx, order, st, host_stats, stats_add, R);
+    cudaError_t err = prepare_tiled(src, n, sny, snx, tgt, srcdev, srchost, ony, onx, order, st, host_stats, stats_add, R, cc);
     if (err != cudaSuccess) { free_scratch(R.sc, st); return err; }
     R.P.out = out;
     if (prof && prof->enabled) cudaEventRecord(prof->main_begin, st);
@@ -290,13 +304,13 @@ cudaError_t launch_tiled_reproject(const float *src, int n, int sny, int snx,
 
 cudaError_t launch_tiled_coords(int n, int sny, int snx, const TargetDev &tgt,
                                 const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx, int order,
-                                double *x, double *y, cudaStream_t st)
+                                double *x, double *y, cudaStream_t st, const ConstsCopy &cc)
 {
     (void)order;
     TiledParams P;
     std::memset(&P, 0, sizeof P);
     Scratch sc;
-    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, srchost, ony, onx, st, nullptr, 0, sc, P);
+    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, srchost, ony, onx, st, nullptr, 0, sc, P, cc);
     if (err == cudaSuccess) {
         for (int e0 = 0; e0 < n && err == cudaSuccess; e0 += 65535) {
             P.e0 = e0;

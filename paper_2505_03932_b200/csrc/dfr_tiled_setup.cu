@@ -67,10 +67,13 @@ static FitConsts make_fit_consts()
 // ---------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128)
 target_nodes_kernel(const __grid_constant__ TargetDev tgt, const __grid_constant__ FitConsts fc,
-                    int ctas_x, int ctas, double2 *__restrict__ uv, int32_t *__restrict__ counters)
+                    int ctas_x, int ctas, double2 *__restrict__ uv, int32_t *__restrict__ counters,
+                    const uint4 *__restrict__ cc_src, uint4 *__restrict__ cc_dst, int cc_n16)
 {
     // tile counters + ticket of the setup kernel start from zero (no memset in the stream)
     if (blockIdx.x == 0 && threadIdx.x < 4) counters[threadIdx.x] = 0;
+    // the call's constants (per-exposure maps, weights): mapped pinned host memory -> device scratch
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < cc_n16; k += gridDim.x * blockDim.x) cc_dst[k] = cc_src[k];
     // sample points of the 64x64 CTA tiles (the parent fit of tile_setup_kernel)
     pdl_trigger();                                  // the setup kernel may stage its constants meanwhile
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
@@ -92,7 +95,7 @@ __host__ __device__ constexpr int tri_off(int n, int p) { return p * (n + 1) - (
 // The reciprocal is a float seed + two Newton steps (c is O(1) for any valid point);
 // invalid points (c <= 0, NaN) come out as NaN.
 template <int N>
-__device__ __forceinline__ void source_xy_sm(const double *__restrict__ sm, double U, double V,
+__device__ __forceinline__ void source_xy_sm(const double *__restrict__ sm, bool inv_exact, double U, double V,
                                              double &x, double &y)
 {
     const double a = fma(sm[0], U, fma(sm[1], V, sm[2]));
@@ -108,8 +111,16 @@ __device__ __forceinline__ void source_xy_sm(const double *__restrict__ sm, doub
     x = us + sm[9];
     y = vs + sm[10];
     if (N > 0) {
-        x += poly_eval_fixed<N>(sm + 11, us, vs);
-        y += poly_eval_fixed<N>(sm + 11 + tri(N), us, vs);
+        if (inv_exact) {                         // DFR_SIP_INVERSE_EXACT: sm holds A, B; solve at this sample point
+            double u, v;
+            invert_sip([&](double p, double q) { return poly_eval_fixed<N>(sm + 11, p, q); },
+                       [&](double p, double q) { return poly_eval_fixed<N>(sm + 11 + tri(N), p, q); }, us, vs, u, v);
+            x = u + sm[9];
+            y = v + sm[10];
+        } else {
+            x += poly_eval_fixed<N>(sm + 11, us, vs);
+            y += poly_eval_fixed<N>(sm + 11 + tri(N), us, vs);
+        }
     }
 }
 
@@ -118,7 +129,7 @@ __device__ __forceinline__ void source_xy_sm(const double *__restrict__ sm, doub
 // then VERIFIED against the exact map at 9 other points (centre, T4 extrema on the axes, corners).
 // uvf(k) returns the target-side (U, V) of sample point k. C[4q + p] = coefficient of s^p t^q.
 template <int N, class UVF>
-__device__ __forceinline__ bool fit_cubic(const double *__restrict__ sm, const FitConsts &fc, UVF uvf,
+__device__ __forceinline__ bool fit_cubic(const double *__restrict__ sm, bool inv_exact, const FitConsts &fc, UVF uvf,
                                           double (&Cx)[16], double (&Cy)[16])
 {
     double Rx[4][4], Ry[4][4];                  // [node row b][power of s]
@@ -129,7 +140,7 @@ __device__ __forceinline__ bool fit_cubic(const double *__restrict__ sm, const F
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
             const double2 q = uvf(4 * b + a);
-            source_xy_sm<N>(sm, q.x, q.y, xs[a], ys[a]);
+            source_xy_sm<N>(sm, inv_exact, q.x, q.y, xs[a], ys[a]);
             nanacc = fma(xs[a], 0.0, fma(ys[a], 0.0, nanacc));
         }
 #pragma unroll
@@ -150,7 +161,7 @@ __device__ __forceinline__ bool fit_cubic(const double *__restrict__ sm, const F
     for (int k = 16; k < NPTS; ++k) {
         const double2 q = uvf(k);
         double x, y;
-        source_xy_sm<N>(sm, q.x, q.y, x, y);
+        source_xy_sm<N>(sm, inv_exact, q.x, q.y, x, y);
         const double ss = fc.pts[k][0], tt = fc.pts[k][1];
         double px = 0.0, py = 0.0;
 #pragma unroll
@@ -266,6 +277,9 @@ tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ 
 {
     __shared__ double sm[11 + 2 * tri(N)];
     const int e = e0 + blockIdx.y;
+    pdl_trigger();                                  // the main kernel's launch may overlap this one
+    pdl_wait();                                     // the node table and the call's constants are complete
+    const bool inv_exact = N > 0 && srcdev[e].inv_exact != 0;
     {
         const SourceDev &s = srcdev[e];
         for (int k = threadIdx.x; k < 11 + 2 * tri(N); k += blockDim.x) {
@@ -285,15 +299,13 @@ tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ 
             sm[k] = v;
         }
     }
-    pdl_trigger();                                  // the main kernel's launch may overlap this one
     __syncthreads();
-    pdl_wait();                                     // the node table is complete
     const int c = blockIdx.x * kSetupThreads + threadIdx.x;
     int nflag[3] = {0, 0, 0};
     if (c < ctas) {
         const int cty = c / ctas_x, ctx = c - cty * ctas_x;
         double Px[16], Py[16];                      // parent cubic, unit = 32 px
-        const bool parent = fit_cubic<N>(sm, fc, [&](int k) { return __ldg(uv + (size_t)k * ctas + c); }, Px, Py);
+        const bool parent = fit_cubic<N>(sm, inv_exact, fc, [&](int k) { return __ldg(uv + (size_t)k * ctas + c); }, Px, Py);
         int box_x = kNoBox, box_y = kNoBox;
 #pragma unroll 1
         for (int sub = 0; sub < CTA_T * CTA_T; ++sub) {
@@ -317,7 +329,7 @@ tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ 
                 }
             } else {
                 const double cx0 = ttx * TS + kCentre, cy0 = tty * TS + kCentre;
-                good = fit_cubic<N>(sm, fc, [&](int k) {
+                good = fit_cubic<N>(sm, inv_exact, fc, [&](int k) {
                     double U, V;
                     target_uv(tgt, cx0 + kHalf * fc.pts[k][0], cy0 + kHalf * fc.pts[k][1], U, V);
                     return make_double2(U, V);
@@ -410,7 +422,7 @@ static bool probe_extent(const TargetDev &tgt, const SourceDev *hs, int n, int o
 
 cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const SourceDev *srcdev,
                              const SourceDev *srchost, int ony, int onx, cudaStream_t st,
-                             int32_t *host_stats, int stats_add, Scratch &sc, TiledParams &P)
+                             int32_t *host_stats, int stats_add, Scratch &sc, TiledParams &P, const ConstsCopy &cc)
 {
     static const FitConsts fc = make_fit_consts();
     P.n = n; P.sny = sny; P.snx = snx; P.ony = ony; P.onx = onx;
@@ -434,7 +446,9 @@ cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const Sourc
     sc.counters = reinterpret_cast<int32_t *>(base + b_uv + b_recs + b_box);
     P.recs = sc.recs;
     P.cta_box = sc.cta_box;
-    target_nodes_kernel<<<(ctas * NPTS + 127) / 128, 128, 0, st>>>(tgt, fc, P.ctas_x, ctas, sc.uv, sc.counters);
+    target_nodes_kernel<<<(ctas * NPTS + 127) / 128, 128, 0, st>>>(tgt, fc, P.ctas_x, ctas, sc.uv, sc.counters,
+                                                                   static_cast<const uint4 *>(cc.src), static_cast<uint4 *>(cc.dst),
+                                                                   cc.src ? (int)(cc.bytes / 16) : 0);
     if ((err = cudaGetLastError()) != cudaSuccess) return err;
     // SIP order class of the batch: inverse polynomials are zero-padded up to N
     int maxo = 0;
@@ -463,12 +477,12 @@ void free_scratch(Scratch &sc, cudaStream_t st)
 cudaError_t prepare_tiled(const float *src, int n, int sny, int snx, const TargetDev &tgt,
                                  const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx,
                                  int order, cudaStream_t st, int32_t *host_stats, int stats_add, Prepared &R,
-                                 int span_tiles, size_t max_box_bytes)
+                                 const ConstsCopy &cc, int span_tiles, size_t max_box_bytes)
 {
     std::memset(&R.P, 0, sizeof R.P);
     std::memset(&R.tmap, 0, sizeof R.tmap);
     R.P.src = src;
-    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, srchost, ony, onx, st, host_stats, stats_add, R.sc, R.P);
+    cudaError_t err = run_setup(n, sny, snx, tgt, srcdev, srchost, ony, onx, st, host_stats, stats_add, R.sc, R.P, cc);
     if (err != cudaSuccess) return err;
     // ---- staging decision: box size from a host probe; TMA needs 16-byte rows
     double ex, ey;

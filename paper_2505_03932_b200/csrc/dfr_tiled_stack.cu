@@ -372,13 +372,14 @@ static cudaError_t launch_stack(TiledParams P, const TargetDev &tgt, const CUten
 cudaError_t launch_tiled_stack(const float *src, int n, int sny, int snx, const TargetDev &tgt,
                                const SourceDev *srcdev, const SourceDev *srchost, int ony, int onx, int order,
                                const float *dev_weights, float *sum, float *wsum, int accumulate,
-                               cudaStream_t st, int32_t *host_stats, int stats_add, TiledStats *stats, ProfileEvents *prof)
+                               cudaStream_t st, int32_t *host_stats, int stats_add, TiledStats *stats, ProfileEvents *prof,
+                               const ConstsCopy &cc)
 {
     Prepared R;
     if (prof && prof->enabled) cudaEventRecord(prof->setup_begin, st);
     // the staged boxes are per 32x32 tile (one per warp)
     cudaError_t err = prepare_tiled(src, n, sny, snx, tgt, srcdev, srchost, ony, onx, order, st, host_stats, stats_add, R,
-                                    1, kStackMaxBoxBytes);
+                                    cc, 1, kStackMaxBoxBytes);
     if (err != cudaSuccess) { free_scratch(R.sc, st); return err; }
     StackParams S;
     S.weights = dev_weights; S.sum = sum; S.wsum = wsum; S.partial = nullptr; S.ticket = nullptr;

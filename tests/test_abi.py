@@ -165,3 +165,23 @@ def test_shard_range_is_a_partition_and_matches_the_python_rule(P):
         P.dfr_shard_range(10, 0, 0)
     with pytest.raises(P.DfrError):
         P.dfr_shard_range(10, 4, 4)
+
+
+def test_exact_inverse_sentinel_validation(P):
+    """DFR_SIP_INVERSE_EXACT (-1) is accepted only for ap_order and bp_order together."""
+    L = P.lib()
+    w = S.make_wcs(8, 8, 1.0, 2.0, 0.0, S.PIXSCALE)
+    src, out = C.c_void_p(0x10000), C.c_void_p(0x90000)
+
+    def call(ap, bp, a=2):
+        s = P.pack_wcs(w)
+        s.a_order = s.b_order = a
+        s.a[2 * 10 + 0] = 1e-6
+        s.ap_order, s.bp_order = ap, bp
+        arr = (P.DfrWCS * 1)(s)
+        # an aliasing output stops the call after validation (no CUDA needed)
+        return L.dfr_reproject_ex(src, 1, 8, 8, arr, C.byref(P.pack_wcs(w)), 8, 8, 1, C.c_void_p(0x10000 + 64), None, 0)
+
+    assert call(-1, -1) == -7                      # valid WCS: reaches the alias check
+    assert call(0, 0) == -7
+    assert call(-1, 0) == -4 and call(3, -1) == -4 and call(-2, -2) == -4

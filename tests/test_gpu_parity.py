@@ -641,3 +641,86 @@ def test_nearest_ties_round_half_even_on_both_paths(P):
         mixed2 = oracle.interp(img, np.ceil(xo - 1e-6).ravel(), np.floor(yo).ravel(), 0).reshape(96, 128)
         okx = (x == lo) | (x == hi) | (x == mixed1) | (x == mixed2) | np.isnan(x)
         assert okx[inside].all(), (sx, sy)
+
+
+def test_fit_acceptance_adversarial_sweep(P):
+    """The tiled path accepts a tile's cubic fit after comparing it with the exact map at 9 check
+    points (FIT_TOL = 2e-6 px): a spot check, not a bound. This seeded sweep searches for a
+    geometry where an ACCEPTED tile is wrong anyway: SIP orders 2-9 on either side with
+    amplitudes 1e-6 ... 1e-2 (up to tens of pixels of distortion), scale ratios 0.5-2, any
+    rotation, tangent points up to degrees apart, declinations up to the poles. Everywhere
+    |tiled - exact| must stay below 1e-5 px (design for <= 1e-5 px; the
+    north_star tolerance is 1e-4 px), whatever mix of FAST / EXACT tiles the setup kernel chose."""
+    rng = np.random.default_rng(777)
+    worst, worst_case, n_fast, n_exact = 0.0, None, 0, 0
+    for case in range(240):
+        n_src = int(rng.integers(160, 420)) // 4 * 4
+        n_out = int(rng.integers(160, 420))
+        dec0 = [rng.uniform(-60, 60), rng.uniform(80, 89.9), -rng.uniform(80, 89.9), 89.999][case % 4]
+        ra0 = rng.uniform(0, 360)
+        sep = 10 ** rng.uniform(-4, 0.5) * S.PIXSCALE * 200            # tangent points 0.02 ... 600 px apart
+        pa = rng.uniform(0, 2 * np.pi)
+        ratio = 2 ** rng.uniform(-1, 1)
+        src = S.make_wcs(n_src, n_src, ra0, dec0, rng.uniform(0, 360), S.PIXSCALE)
+        dra = sep * np.sin(pa) / max(np.cos(np.radians(dec0)), 1e-3)
+        tgt = S.make_wcs(n_out, n_out, ra0 + dra, min(max(dec0 + sep * np.cos(pa), -89.9999), 89.9999),
+                         rng.uniform(0, 360), S.PIXSCALE * ratio)
+        if case % 5:
+            S.add_sip(src, int(rng.integers(2, 10)), n_src / 2.0, rng, amp=10 ** rng.uniform(-6, -2))
+        if case % 3:
+            S.add_sip(tgt, int(rng.integers(2, 10)), n_out / 2.0, rng, amp=10 ** rng.uniform(-6, -2))
+        xa, ya = P.dfr_src_coords([src], tgt, (n_src, n_src), (n_out, n_out), 1, path=P.PATH_AUTO)
+        img = torch.zeros((1, n_src, n_src), dtype=torch.float32, device="cuda")
+        P.dfr_reproject(img, [src], tgt, (n_out, n_out), 1)
+        st = P.dfr_last_stats()
+        xe, ye = P.dfr_src_coords([src], tgt, (n_src, n_src), (n_out, n_out), 1, path=P.PATH_EXACT)
+        assert torch.equal(torch.isfinite(xa), torch.isfinite(xe)), case
+        # only coordinates that can matter: within 4 px of the source image
+        near = torch.isfinite(xe) & (xe > -4) & (xe < n_src + 3) & (ye > -4) & (ye < n_src + 3)
+        if bool(near.any()):
+            d = float(torch.maximum((xa - xe).abs()[near].max(), (ya - ye).abs()[near].max()))
+            if d > worst:
+                worst, worst_case = d, (case, st, dec0, ratio, src.a_order, tgt.a_order)
+        n_fast += st["tiles_fast"]
+        n_exact += st["tiles_exact"]
+    print("fit sweep: worst |tiled - exact| =", worst, "px at", worst_case, "; tiles fast / exact:", n_fast, n_exact)
+    assert n_fast > 5000 and worst <= 1e-5
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_exact_inverse_sip_on_device(P, path):
+    """§8(f) f4, device side: a source WCS with A/B but no AP/BP, ap_order = bp_order =
+    DFR_SIP_INVERSE_EXACT: the library inverts the forward distortion itself. Oracle = the literal
+    chain without inverse SIP (O6-O8) followed by the DEFINITION of the inverse distortion,
+    oracle/sip_inverse.py: newton_inverse (pin I1). A ~9 px distortion: a fitted order-3 AP/BP
+    is 0.1 px off here (pin I3), the exact inverse must meet the 1e-4 px bar."""
+    from oracle import sip_inverse as SI
+    src, tgt = S.stress_sip_pair()
+    bare = src.copy()
+    bare.ap_order = bare.bp_order = 0
+    bare.ap, bare.bp = np.zeros((10, 10)), np.zeros((10, 10))
+    exact = bare.copy()
+    exact.ap_order = exact.bp_order = -1
+    n = 1024
+    rng = np.random.default_rng(44)
+    img = S.make_image(n, n, 400, rng)
+    xo, yo = oracle.src_coords(tgt, bare, n, n)              # U + crpix - 1: no inverse distortion applied
+    u, v = SI.newton_inverse(bare, xo - (bare.crpix[0] - 1.0), yo - (bare.crpix[1] - 1.0))
+    xo, yo = u + (bare.crpix[0] - 1.0), v + (bare.crpix[1] - 1.0)
+    xg, yg = P.dfr_src_coords([exact], tgt, (n, n), (n, n), 1, path=PATHS[path])
+    st = PR.check_coords(xg[0].cpu().numpy(), yg[0].cpu().numpy(), xo, yo, bare)
+    xb, _ = P.dfr_src_coords([bare], tgt, (n, n), (n, n), 1, path=PATHS[path])
+    assert float((xb[0] - xg[0]).abs().max()) > 1.0           # the inverse distortion is pixels, not noise
+    for order in (0, 1, 3):
+        out = P.dfr_reproject(torch.from_numpy(img[None]).cuda(), [exact], tgt, (n, n), order, path=PATHS[path])
+        ref = oracle.interp(img, xo.ravel(), yo.ravel(), order).reshape(n, n).astype(np.float32)
+        PR.check_image(out[0].cpu().numpy(), ref, xo, yo, img, order)
+    if path == "auto":
+        assert P.dfr_last_stats()["tiles_fast"] > 900
+    # the sky entry point inverts as well: world2pix(pix2world(x)) = x to 1e-9 px without any AP/BP
+    x = torch.from_numpy(rng.uniform(0, n - 1, 5000)).cuda()
+    y = torch.from_numpy(rng.uniform(0, n - 1, 5000)).cuda()
+    ra, dec = P.dfr_pix2world(exact, x, y)
+    xr, yr = P.dfr_world2pix(exact, ra, dec)
+    assert float((xr - x).abs().max()) < 1e-7 and float((yr - y).abs().max()) < 1e-7
+    print("exact inverse", path, st)
