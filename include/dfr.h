@@ -92,7 +92,7 @@ typedef enum dfr_status {
 } dfr_status;
 
 /* Path selection for dfr_reproject_ex / dfr_src_coords_ex.
- *   AUTO  : tiled fast path where its verified error bound holds, exact
+ *   AUTO  : tiled fast path where its per-tile fit passes a 9-point spot check, exact
  *           per-pixel path elsewhere (what dfr_reproject uses).
  *   EXACT : every pixel through the per-pixel fp64 map, direct gathers.
  *   TILED : as AUTO (kept distinct so tests can assert the fast path ran). */

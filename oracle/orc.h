@@ -18,7 +18,8 @@
  * Readings that no available source can pin against the real package
  * ("parity unpinned"): G3 SIP sign (+, Shupe 2005), G6 footprint edge
  * (half-open pixel-area union), G7 bicubic kernel (Keys a = -0.75),
- * G14 NaN in the source image. See DESIGN.md §3.
+ * G19 the literal zero-pad / identity rule. (G14, NaN pixels in the source, is
+ * pinned by the S6 stack pin and the interpolation pins.) See DESIGN.md §3.
  */
 #ifndef ORC_H
 #define ORC_H

@@ -37,7 +37,9 @@ def wcs_from_header(header, shape=None, inverse_order=None) -> DfrWCS:
     CRPIXi, CRVALi; CDi_j, or PCi_j (default identity) with CDELTi, or CDELTi
     with CROTA2; A_ORDER/A_p_q, B_, AP_, BP_. If forward SIP terms are present
     without AP/BP, the inverse is fitted by dfr_wcs_fit_inverse_sip over `shape` (ny, nx)
-    (default NAXIS2, NAXIS1) at `inverse_order` (default min(9, A_ORDER + 2)).
+    (default NAXIS2, NAXIS1) at `inverse_order` (default min(9, A_ORDER + 2));
+    inverse_order="exact" marks the WCS DFR_SIP_INVERSE_EXACT instead: the library then inverts
+    A/B itself by iteration (no fit, no truncation error).
     Rejected: any other projection, LONPOLE != 180, transposed axes."""
     c1, c2 = str(_get(header, "CTYPE1", "RA---TAN")).strip(), str(_get(header, "CTYPE2", "DEC--TAN")).strip()
     if not (c1 in ("RA---TAN", "RA---TAN-SIP") and c2 in ("DEC--TAN", "DEC--TAN-SIP")):
@@ -71,7 +73,9 @@ def wcs_from_header(header, shape=None, inverse_order=None) -> DfrWCS:
         for p in range(order + 1):
             for q in range(order + 1 - p):
                 arr[p * 10 + q] = float(_get(header, f"{key}_{p}_{q}", 0.0))
-    if (w.a_order or w.b_order) and not (w.ap_order or w.bp_order):
+    if (w.a_order or w.b_order) and not (w.ap_order or w.bp_order) and inverse_order == "exact":
+        w.ap_order = w.bp_order = -1                            # DFR_SIP_INVERSE_EXACT
+    elif (w.a_order or w.b_order) and not (w.ap_order or w.bp_order):
         ny, nx = shape if shape is not None else (_get(header, "NAXIS2"), _get(header, "NAXIS1"))
         if ny is None or nx is None:
             raise HeaderError("forward SIP without AP/BP: the image shape is needed to fit the inverse")

@@ -26,18 +26,34 @@ def _headers():
             + [os.path.join(ROOT, "include", "dfr.h")])
 
 
-def _obj(src):
-    return os.path.join(OBJ, os.path.basename(src)[:-3] + ".o")
+def _obj(src, objdir=OBJ):
+    return os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
 
 
-def compile_command(src, extra=()):
+def compile_command(src, extra=(), objdir=OBJ):
     return [NVCC, *ARCH, "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
             "-I" + os.path.join(ROOT, "include"), "-I" + os.path.join(PKG, "csrc"),
-            *extra, "-c", src, "-o", _obj(src)]
+            *extra, "-c", src, "-o", _obj(src, objdir)]
 
 
-def link_command():
-    return [NVCC, *ARCH, "-shared", "-o", SO, *[_obj(s) for s in sources()]]
+def link_command(so=SO, objdir=OBJ):
+    return [NVCC, *ARCH, "-shared", "-o", so, *[_obj(s, objdir) for s in sources()]]
+
+
+# The instrumented library of tests/bounds_check.py: every staged shared-memory gather checks its
+# address against the box it may read (csrc/dfr_tiled_device.cuh, DFR_BOUNDS_CHECK). Never loaded
+# by the package itself.
+SO_CHECKED = os.path.join(PKG, "libdfr_checked.so")
+
+
+def build_checked(selftest: bool = False, verbose: bool = False) -> str:
+    objdir = os.path.join(PKG, "csrc", "build_checked")
+    os.makedirs(objdir, exist_ok=True)
+    extra = ["-DDFR_BOUNDS_CHECK"] + (["-DDFR_BOUNDS_SELFTEST"] if selftest else [])
+    with ThreadPoolExecutor(max_workers=8) as ex:
+        list(ex.map(lambda s: _run(compile_command(s, extra, objdir), verbose), sources()))
+    _run(link_command(SO_CHECKED, objdir), verbose)
+    return SO_CHECKED
 
 
 def _run(cmd, verbose):
@@ -66,4 +82,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 if __name__ == "__main__":
     import sys
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--checked" in sys.argv:
+        print(build_checked(selftest="--selftest" in sys.argv, verbose="-v" in sys.argv))
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -115,27 +115,43 @@ struct CallConsts {
     }
 };
 
-// by_kernel: leave the upload to the tiled path's first kernel (K.cc); otherwise enqueue a copy.
+// How the constants reach the device. Up to kInlineCopyBytes: a cudaMemcpyAsync from PAGEABLE memory
+// (the runtime takes the bytes before returning and needs no copy-engine transfer for them: the
+// cheapest form measured — a copy from pinned memory put a copy-engine -> compute dependency in front
+// of every call, +8 us per C2 step). Above it such a copy would block the host until the stream
+// drains, so the pinned, device-mapped staging ring is used and, on the tiled path (by_kernel), the
+// first setup kernel reads the constants from it (K.cc); the other paths enqueue a pinned copy.
+constexpr size_t kInlineCopyBytes = 48 * 1024;
+static thread_local std::vector<char> t_inline;      // pageable staging of the small case
+
 static int upload_consts(DevCtx *c, int32_t n, const dfr_wcs *sw, const dfr_wcs *tw, bool with_weights,
                          const float *weights, cudaStream_t st, bool by_kernel, CallConsts &K)
 {
     make_target(tw, &K.tgt);
     const size_t b_src = sizeof(SourceDev) * (size_t)n;
     const size_t bytes = (b_src + (with_weights ? sizeof(float) * (size_t)n : 0) + 15) & ~(size_t)15;
-    cudaError_t err = stage_acquire(c, bytes, &K.slot);
-    if (err != cudaSuccess) return cuda_fail(err, "pinned staging buffer");
-    SourceDev *h = static_cast<SourceDev *>(K.slot->host);
+    const bool small = bytes <= kInlineCopyBytes;
+    cudaError_t err;
+    char *stage;
+    if (small) {
+        if (t_inline.size() < bytes) t_inline.resize(bytes);
+        stage = t_inline.data();
+    } else {
+        if ((err = stage_acquire(c, bytes, &K.slot)) != cudaSuccess) return cuda_fail(err, "pinned staging buffer");
+        stage = static_cast<char *>(K.slot->host);
+    }
+    SourceDev *h = reinterpret_cast<SourceDev *>(stage);
     for (int32_t e = 0; e < n; ++e) make_source(tw, &sw[e], &h[e]);
     if (with_weights) {
-        float *hw = reinterpret_cast<float *>(static_cast<char *>(K.slot->host) + b_src);
+        float *hw = reinterpret_cast<float *>(stage + b_src);
         for (int32_t e = 0; e < n; ++e) hw[e] = weights ? weights[e] : 1.0f;
     }
     if ((err = scratch_alloc(&K.block, bytes, st)) != cudaSuccess) return cuda_fail(err, "scratch allocation (constants)");
-    if (by_kernel) {
+    if (!small && by_kernel) {
         K.cc.src = K.slot->dev;
         K.cc.dst = K.block;
         K.cc.bytes = bytes;
-    } else if ((err = cudaMemcpyAsync(K.block, K.slot->host, bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) {
+    } else if ((err = cudaMemcpyAsync(K.block, stage, bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) {
         K.finish(st);
         return cuda_fail(err, "cudaMemcpyAsync(constants)");
     }

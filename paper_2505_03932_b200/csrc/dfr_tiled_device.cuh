@@ -92,17 +92,56 @@ template <bool STAGE> struct GatherSrc {
     const float *gbase;              // !STAGE: global address of element (0, 0)
 };
 
+#ifdef DFR_BOUNDS_CHECK
+// Checked build (never shipped): compute-sanitizer is not available on the GPU pool, so the
+// unchecked gathers of the packed loops are verified by an instrumented build instead. Every staged
+// load checks its address against the box the current warp may read — set by the kernels with
+// dfr_chk_set: the CTA's box (reproject) or the warp's own box (stack) — and against 4-byte
+// alignment; violations are counted in dfr_oob_count and the load is redirected to the box start.
+// dfr_dev_oob_main() / dfr_dev_oob_stack() (extern "C") return and clear the counts.
+static __device__ unsigned long long dfr_oob_count;
+__device__ __forceinline__ uint2 &dfr_chk_range()
+{
+    __shared__ uint2 r[8];
+    return r[(threadIdx.x >> 5) & 7];
+}
+__device__ __forceinline__ void dfr_chk_set(uint32_t lo, uint32_t hi)
+{
+#ifdef DFR_BOUNDS_SELFTEST                      // negative control: declare a box 256 bytes long
+    hi = hi > lo + 256u ? lo + 256u : hi;
+#endif
+    dfr_chk_range() = make_uint2(lo, hi);
+    __syncwarp();
+}
+__device__ __forceinline__ uint32_t dfr_chk(uint32_t a)
+{
+    const uint2 r = dfr_chk_range();
+    if (a < r.x || a + 4u > r.y || (a & 3u)) {
+        atomicAdd(&dfr_oob_count, 1ull);
+        return r.x;
+    }
+    return a;
+}
+#else
+__device__ __forceinline__ void dfr_chk_set(uint32_t, uint32_t) {}
+__device__ __forceinline__ uint32_t dfr_chk(uint32_t a) { return a; }
+#endif
+
 __device__ __forceinline__ float lds_f32(uint32_t a)
 {
     float v;
-    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(dfr_chk(a)));
     return v;
 }
 __device__ __forceinline__ float lds_f32_4(uint32_t a)
 {
+#ifdef DFR_BOUNDS_CHECK
+    return lds_f32(a + 4u);
+#else
     float v;
     asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v) : "r"(a));
     return v;
+#endif
 }
 
 // One pixel of a FAST tile: floor/rint by a magic add, range test, gather, interpolate.

@@ -115,11 +115,25 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
     if (!active) return;
     TileHead H;
     H.flag = flag; H.ix0 = ix0; H.iy0 = iy0; H.bx0 = bx0; H.by0 = by0; H.bx1 = bx1; H.by1 = by1; H.deg = deg;
+    dfr_chk_set(has_box ? smem_u32(box) : 0u, has_box ? smem_u32(box) + (uint32_t)(P.BW * P.BH * sizeof(float)) : 0u);
     StoreSink sink;
     sink.orow = P.out + ((size_t)e * P.ony + (size_t)tty * TS) * P.onx + (ttx * TS + lane);
     sink.opitch = (size_t)P.onx;
     warp_tile<ORDER, STAGE, EDGE>(P, tgt, e, ttx, tty, lane, H, X, Y, smem_u32(box), ox, oy, sink);
 }
+
+#ifdef DFR_BOUNDS_CHECK
+}  // namespace dfr
+extern "C" unsigned long long dfr_dev_oob_main()
+{
+    unsigned long long v = 0, zero = 0;
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(&v, dfr::dfr_oob_count, sizeof v);
+    cudaMemcpyToSymbol(dfr::dfr_oob_count, &zero, sizeof zero);
+    return v;
+}
+namespace dfr {
+#endif
 
 // coordinates the tiled path uses (dfr_src_coords): same records, same polynomial code
 __global__ void __launch_bounds__(32 * CTA_T * CTA_T)

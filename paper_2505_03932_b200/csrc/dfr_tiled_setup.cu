@@ -267,19 +267,26 @@ __device__ __forceinline__ int emit_tile(double (&Cx)[16], double (&Cy)[16], boo
 // shared memory took 21-23 us — more waves of a latency-bound kernel — so this stays.)
 constexpr int kSetupThreads = 128;
 
-template <int N>
+// INV: the batch contains DFR_SIP_INVERSE_EXACT sources (a separate instantiation, so the common
+// kernel is compiled exactly as without that feature: as a run-time flag alone it cost 6 us per call).
+template <int N, bool INV>
 __global__ void __launch_bounds__(kSetupThreads)
 tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ srcdev,
                   const __grid_constant__ TargetDev tgt, const __grid_constant__ FitConsts fc, int e0,
                   int tiles_x, int tiles_y, int ctas_x, int ctas, int sny, int snx,
                   TileRec *__restrict__ recs, int2 *__restrict__ cta_box, int32_t *__restrict__ counters,
-                  int total_blocks, int32_t *__restrict__ host_stats, int stats_add)
+                  int total_blocks, int32_t *__restrict__ host_stats, int stats_add, int late_consts)
 {
     __shared__ double sm[11 + 2 * tri(N)];
     const int e = e0 + blockIdx.y;
-    pdl_trigger();                                  // the main kernel's launch may overlap this one
-    pdl_wait();                                     // the node table and the call's constants are complete
-    const bool inv_exact = N > 0 && srcdev[e].inv_exact != 0;
+    // The exposure's constants -> shared memory. When they were uploaded by a copy earlier in the
+    // stream they are staged BEFORE waiting for the node kernel (this kernel's launch overlaps it);
+    // when the node kernel itself brings them in (late_consts), after.
+    if (late_consts) {
+        pdl_trigger();
+        pdl_wait();
+    }
+    const bool inv_exact = INV && N > 0 && srcdev[e].inv_exact != 0;
     {
         const SourceDev &s = srcdev[e];
         for (int k = threadIdx.x; k < 11 + 2 * tri(N); k += blockDim.x) {
@@ -299,7 +306,9 @@ tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ 
             sm[k] = v;
         }
     }
+    if (!late_consts) pdl_trigger();                // the main kernel's launch may overlap this one
     __syncthreads();
+    if (!late_consts) pdl_wait();                   // the node table is complete
     const int c = blockIdx.x * kSetupThreads + threadIdx.x;
     int nflag[3] = {0, 0, 0};
     if (c < ctas) {
@@ -452,17 +461,26 @@ cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const Sourc
     if ((err = cudaGetLastError()) != cudaSuccess) return err;
     // SIP order class of the batch: inverse polynomials are zero-padded up to N
     int maxo = 0;
-    for (int e = 0; e < n; ++e) maxo = std::max(maxo, std::max(srchost[e].ap.order, srchost[e].bp.order));
+    bool inv = false;
+    for (int e = 0; e < n; ++e) {
+        maxo = std::max(maxo, std::max(srchost[e].ap.order, srchost[e].bp.order));
+        inv = inv || srchost[e].inv_exact != 0;
+    }
     const unsigned bx = (unsigned)((ctas + kSetupThreads - 1) / kSetupThreads);
     const long long total_blocks = (long long)bx * n;
     if (total_blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     for (int e0 = 0; e0 < n; e0 += 65535) {
         const dim3 grid(bx, (unsigned)std::min(n - e0, 65535));
-        if (maxo == 0) err = launch_pdl(tile_setup_kernel<0>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
-        else if (maxo <= 3) err = launch_pdl(tile_setup_kernel<3>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
-        else if (maxo <= 4) err = launch_pdl(tile_setup_kernel<4>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
-        else if (maxo <= 5) err = launch_pdl(tile_setup_kernel<5>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
-        else err = launch_pdl(tile_setup_kernel<9>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks, host_stats, stats_add);
+#define DFR_SETUP(NN, II)                                                                                           \
+    launch_pdl(tile_setup_kernel<NN, II>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, \
+               P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks,       \
+               host_stats, stats_add, cc.src ? 1 : 0)
+        if (maxo == 0) err = DFR_SETUP(0, false);
+        else if (maxo <= 3) err = inv ? DFR_SETUP(3, true) : DFR_SETUP(3, false);
+        else if (maxo <= 4) err = inv ? DFR_SETUP(4, true) : DFR_SETUP(4, false);
+        else if (maxo <= 5) err = inv ? DFR_SETUP(5, true) : DFR_SETUP(5, false);
+        else err = inv ? DFR_SETUP(9, true) : DFR_SETUP(9, false);
+#undef DFR_SETUP
         if (err != cudaSuccess) return err;
     }
     return cudaSuccess;

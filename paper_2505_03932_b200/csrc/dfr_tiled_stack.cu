@@ -236,6 +236,7 @@ tiled_stack_kernel(const __grid_constant__ TiledParams P, const __grid_constant_
                 mbar_wait(bar, phase);
                 phase ^= 1u;
             }
+            dfr_chk_set(has_box ? box_smem : 0u, has_box ? box_smem + box_bytes : 0u);
             warp_tile<ORDER, STAGE>(P, tgt, e, ttx, tty, lane, H, X, Y, box_smem, ox, oy, sink);
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             __syncwarp();                                   // every lane is done with the box
@@ -297,6 +298,19 @@ tiled_stack_kernel(const __grid_constant__ TiledParams P, const __grid_constant_
     if (warp == 0)
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kStackCols) : "memory");
 }
+
+#ifdef DFR_BOUNDS_CHECK
+}  // namespace dfr
+extern "C" unsigned long long dfr_dev_oob_stack()
+{
+    unsigned long long v = 0, zero = 0;
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(&v, dfr::dfr_oob_count, sizeof v);
+    cudaMemcpyToSymbol(dfr::dfr_oob_count, &zero, sizeof zero);
+    return v;
+}
+namespace dfr {
+#endif
 
 __global__ void stack_finalize_kernel(const float *__restrict__ sum, const float *__restrict__ wsum,
                                       long long npix, float *__restrict__ mean)

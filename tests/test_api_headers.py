@@ -81,6 +81,9 @@ def test_missing_inverse_is_fitted(A):
         h = header_of(w, 512, 512, inverse=False)
         del h["NAXIS1"]
         A.wcs_from_header(h)
+    # inverse_order="exact": no fit; the library inverts A/B itself (DFR_SIP_INVERSE_EXACT)
+    e = A.wcs_from_header(header_of(w, 512, 512, inverse=False), inverse_order="exact")
+    assert e.ap_order == -1 and e.bp_order == -1 and e.a_order == 3
 
 
 @pytest.mark.gpu
