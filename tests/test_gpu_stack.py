@@ -172,3 +172,20 @@ def test_stack_many_exposures_few_tiles(P):
     P.dfr_reproject_stack(src, srcs, tgt, (on, on), 1, weights=wts, sum=s0, wsum=w0, accumulate=True)
     assert torch.equal(w0, c + 1.0) and torch.allclose(s0, s + 3.0, rtol=1e-6, atol=1e-3)
     print("stack many", st)
+
+
+def test_stack_is_deterministic_run_to_run(P):
+    """Every output pixel has one owner (or, with exposure chunks, a fixed order of partial sums):
+    the same call must give the same BITS every time, for a chunked launch (few tiles, many
+    exposures) and for an unchunked one (many tiles)."""
+    for n, npx, out_px in ((12, 256, 200), (3, 512, 2048)):
+        w = S.config2(batch=n, n=npx, nstars=100)
+        tgt = S.make_wcs(out_px, out_px, 150.0, 2.0, 0.3, S.PIXSCALE * npx / out_px)
+        src = torch.from_numpy(w.images).cuda()
+        wts = np.linspace(0.3, 1.7, n).astype(np.float32)         # not exactly representable sums
+        ref_s, ref_w = P.dfr_reproject_stack(src, w.src_wcs, tgt, (out_px, out_px), 1, weights=wts)
+        ref_s, ref_w = ref_s.clone(), ref_w.clone()
+        for _ in range(4):
+            s, c = P.dfr_reproject_stack(src, w.src_wcs, tgt, (out_px, out_px), 1, weights=wts)
+            assert torch.equal(s, ref_s) and torch.equal(c, ref_w)
+        assert float(ref_w.max()) > 0
