@@ -115,27 +115,25 @@ struct CallConsts {
     }
 };
 
-// How the constants reach the device. Up to kInlineCopyBytes: a cudaMemcpyAsync from PAGEABLE memory
-// (the runtime takes the bytes before returning and needs no copy-engine transfer for them: the
-// cheapest form measured — a copy from pinned memory put a copy-engine -> compute dependency in front
-// of every call, +8 us per C2 step). Above it such a copy would block the host until the stream
-// drains, so the pinned, device-mapped staging ring is used and, on the tiled path (by_kernel), the
-// first setup kernel reads the constants from it (K.cc); the other paths enqueue a pinned copy.
-constexpr size_t kInlineCopyBytes = 48 * 1024;
-static thread_local std::vector<char> t_inline;      // pageable staging of the small case
-
+// How the constants reach the device (the tiled path: by_kernel). Never by a copy-engine transfer
+// in front of the kernels (measured: +8 us per C2 step for the cross-engine dependency) and never
+// from pageable memory (the runtime does not always take the bytes before returning: reusing the
+// buffer made 2 of 8 test runs fail). Up to kInlineConstsBytes (three exposures) they ride in the
+// parameters of the first setup kernel; larger sets are written to the thread's pinned, device-mapped
+// staging ring and read from there by that kernel. Either way the kernel copies them to device
+// scratch for the kernels that follow. The other paths (exact, sky) enqueue a copy from the ring.
 static int upload_consts(DevCtx *c, int32_t n, const dfr_wcs *sw, const dfr_wcs *tw, bool with_weights,
                          const float *weights, cudaStream_t st, bool by_kernel, CallConsts &K)
 {
     make_target(tw, &K.tgt);
     const size_t b_src = sizeof(SourceDev) * (size_t)n;
     const size_t bytes = (b_src + (with_weights ? sizeof(float) * (size_t)n : 0) + 15) & ~(size_t)15;
-    const bool small = bytes <= kInlineCopyBytes;
+    const bool small = by_kernel && bytes <= kInlineConstsBytes;
     cudaError_t err;
     char *stage;
+    static thread_local char t_small[kInlineConstsBytes];
     if (small) {
-        if (t_inline.size() < bytes) t_inline.resize(bytes);
-        stage = t_inline.data();
+        stage = t_small;
     } else {
         if ((err = stage_acquire(c, bytes, &K.slot)) != cudaSuccess) return cuda_fail(err, "pinned staging buffer");
         stage = static_cast<char *>(K.slot->host);
@@ -147,10 +145,12 @@ static int upload_consts(DevCtx *c, int32_t n, const dfr_wcs *sw, const dfr_wcs 
         for (int32_t e = 0; e < n; ++e) hw[e] = weights ? weights[e] : 1.0f;
     }
     if ((err = scratch_alloc(&K.block, bytes, st)) != cudaSuccess) return cuda_fail(err, "scratch allocation (constants)");
-    if (!small && by_kernel) {
+    K.cc.dst = K.block;
+    K.cc.bytes = bytes;
+    if (small) {
+        K.cc.inline_src = stage;
+    } else if (by_kernel) {
         K.cc.src = K.slot->dev;
-        K.cc.dst = K.block;
-        K.cc.bytes = bytes;
     } else if ((err = cudaMemcpyAsync(K.block, stage, bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) {
         K.finish(st);
         return cuda_fail(err, "cudaMemcpyAsync(constants)");

@@ -41,9 +41,14 @@ struct ProfileEvents {
 // scratch (a copy-engine upload would put a cross-engine dependency in front of every call:
 // measured +8 us per C2 step). src == nullptr: nothing to copy.
 struct ConstsCopy {
-    const void *src = nullptr;          // device-visible address of the pinned staging buffer
+    const void *src = nullptr;          // device-visible address of the pinned staging buffer, or
+    const void *inline_src = nullptr;   // HOST address of at most kInlineConstsBytes that ride in the kernel parameters
     void *dst = nullptr;                // device scratch
     size_t bytes = 0;                   // multiple of 16
+};
+constexpr size_t kInlineConstsBytes = 3 * 1024;     // three exposures' constants: single frames, small batches
+struct InlineConsts {
+    uint4 q[kInlineConstsBytes / 16];
 };
 
 struct TiledParams {

@@ -23,9 +23,14 @@ namespace dfr {
 // ---------------------------------------------------------------------------------
 // constants of the fit
 // ---------------------------------------------------------------------------------
+constexpr int SUP_T = 2;               // a super-tile is SUP_T x SUP_T CTA tiles (128 x 128 px)
+constexpr int kSupLanes = 16;          // = its 4 x 4 tiles = the 16 nodes = the 16 check points: one lane each
+constexpr int kSupEdge = TS * CTA_T * SUP_T;
+
 struct FitConsts {
     double W[4][4];            // monomial coefficients of the Lagrange basis: L_a(s) = sum_p W[p][a] s^p
     double pts[NPTS][2];       // sample points (s, t) in [-1, 1]^2; pixel offset = 16 s
+    double sup[2 * kSupLanes][2];  // the 128x128 super-tile fit: 16 nodes, then 16 check points
 };
 
 static FitConsts make_fit_consts()
@@ -59,6 +64,12 @@ static FitConsts make_fit_consts()
         f.pts[16 + k][0] = chk[k][0];
         f.pts[16 + k][1] = chk[k][1];
     }
+    // super-tile: the same nodes; 16 check points = the 9 above + the 4 edge mid-points (|T4| = 1 in
+    // one direction, 0 offset in the other) + 3 interior points off every symmetry line
+    for (int k = 0; k < 16; ++k) { f.sup[k][0] = f.pts[k][0]; f.sup[k][1] = f.pts[k][1]; }
+    const double more[7][2] = {{1, 0}, {-1, 0}, {0, 1}, {0, -1}, {h, -0.38}, {-0.38, h}, {-0.55, -0.8}};
+    for (int k = 0; k < 9; ++k) { f.sup[16 + k][0] = chk[k][0]; f.sup[16 + k][1] = chk[k][1]; }
+    for (int k = 0; k < 7; ++k) { f.sup[25 + k][0] = more[k][0]; f.sup[25 + k][1] = more[k][1]; }
     return f;
 }
 
@@ -68,22 +79,26 @@ static FitConsts make_fit_consts()
 __global__ void __launch_bounds__(128)
 target_nodes_kernel(const __grid_constant__ TargetDev tgt, const __grid_constant__ FitConsts fc,
                     int ctas_x, int ctas, double2 *__restrict__ uv, int32_t *__restrict__ counters,
-                    const uint4 *__restrict__ cc_src, uint4 *__restrict__ cc_dst, int cc_n16)
+                    const uint4 *__restrict__ cc_src, uint4 *__restrict__ cc_dst, int cc_n16,
+                    const __grid_constant__ InlineConsts ic)
 {
     // tile counters + ticket of the setup kernel start from zero (no memset in the stream)
     if (blockIdx.x == 0 && threadIdx.x < 4) counters[threadIdx.x] = 0;
     // the call's constants (per-exposure maps, weights): mapped pinned host memory -> device scratch
-    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < cc_n16; k += gridDim.x * blockDim.x) cc_dst[k] = cc_src[k];
+    // (small sets ride in this kernel's parameters: cc_src == nullptr)
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < cc_n16; k += gridDim.x * blockDim.x)
+        cc_dst[k] = cc_src ? cc_src[k] : ic.q[k];
     // sample points of the 64x64 CTA tiles (the parent fit of tile_setup_kernel)
     pdl_trigger();                                  // the setup kernel may stage its constants meanwhile
+    // (ctas_x, ctas) here count SUPER-tiles
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= ctas * NPTS) return;
-    const int c = idx / NPTS, k = idx - c * NPTS;
-    constexpr double edge = TS * CTA_T;
+    if (idx >= ctas * 2 * kSupLanes) return;
+    const int c = idx / (2 * kSupLanes), k = idx - c * (2 * kSupLanes);
+    constexpr double edge = kSupEdge;
     const double cx0 = (c % ctas_x) * edge + 0.5 * (edge - 1), cy0 = (c / ctas_x) * edge + 0.5 * (edge - 1);
     double U, V;
-    target_uv(tgt, cx0 + 0.5 * edge * fc.pts[k][0], cy0 + 0.5 * edge * fc.pts[k][1], U, V);
-    uv[(size_t)k * ctas + c] = make_double2(U, V);          // [point][CTA tile]: coalesced for the setup kernel
+    target_uv(tgt, cx0 + 0.5 * edge * fc.sup[k][0], cy0 + 0.5 * edge * fc.sup[k][1], U, V);
+    uv[(size_t)k * ctas + c] = make_double2(U, V);          // [point][super-tile]
 }
 
 // Triangle size and row offset of an order-N packed polynomial (see Poly).
@@ -178,12 +193,13 @@ __device__ __forceinline__ bool fit_cubic(const double *__restrict__ sm, bool in
 
 // p(s0 + s'/2) as a cubic in s': the re-centring of a parent cubic (unit = 32 px) on one of
 // its halves (unit = 16 px). Exact up to fp64 rounding.
-__device__ __forceinline__ void shift_half(double &c0, double &c1, double &c2, double &c3, double s0)
+__device__ __forceinline__ void shift_quarter(double &c0, double &c1, double &c2, double &c3, double s0)
 {
+    // p(s0 + s'/4) as a cubic in s': a 128-px parent (unit = 64 px) re-centred on a 32-px tile (unit = 16 px)
     const double d0 = fma(s0, fma(s0, fma(s0, c3, c2), c1), c0);
-    const double d1 = 0.5 * fma(s0, fma(3.0 * s0, c3, 2.0 * c2), c1);
-    const double d2 = 0.25 * fma(3.0 * s0, c3, c2);
-    c0 = d0; c1 = d1; c2 = d2; c3 = 0.125 * c3;
+    const double d1 = 0.25 * fma(s0, fma(3.0 * s0, c3, 2.0 * c2), c1);
+    const double d2 = 0.0625 * fma(3.0 * s0, c3, c2);
+    c0 = d0; c1 = d1; c2 = d2; c3 = 0.015625 * c3;
 }
 
 // The record of one 32x32 tile from its cubic (unit = 16 px about the tile centre):
@@ -255,25 +271,33 @@ __device__ __forceinline__ int emit_tile(double (&Cx)[16], double (&Cy)[16], boo
     return flag;
 }
 
-// One thread per (64x64 CTA tile, exposure); a block is 128 consecutive CTA tiles of ONE
-// exposure, so the exposure's constants are staged once in shared memory and every
-// coefficient read is a broadcast LDS. Two levels:
-//   1. the cubic is fitted and verified over the whole 64x64 CTA tile (25 map evaluations);
-//      if it holds, the four 32x32 tile records are its exact re-centrings (no more map
-//      evaluations) — 4x less fp64 work than fitting each tile;
-//   2. if it does not (strongly curved maps), each 32x32 tile gets its own fit, with the
+// Sixteen lanes per (128x128 super-tile, exposure) — its 4 x 4 tiles, its 16 interpolation nodes and
+// its 16 check points, one of each per lane. A block is 8 consecutive super-tiles of ONE exposure, so
+// the exposure's constants are staged once in shared memory and every coefficient read is a
+// broadcast LDS. Two levels:
+//   1. every lane evaluates the exact map (a3-a6) at one Chebyshev node; the tensor-product cubic over
+//      the whole super-tile comes out of two rounds of 4-lane shuffles (Lagrange -> monomial along s,
+//      then along t), is gathered by all lanes, and is compared with the exact map at 16 other points
+//      (one per lane: centre, T4 extrema on the axes, corners, edge mid-points, three generic points);
+//      if it holds everywhere, each lane re-centres it on its own 32x32 tile — no further map
+//      evaluations: 2 per lane instead of the 25 (+ fit) a tile of its own would need;
+//   2. if it does not (strongly curved maps), each lane fits its own tile from 25 points with the
 //      target side (a1-a2) evaluated on the fly; a tile whose own fit fails is EXACT.
-// (Measured on B200, C2: 16.8 us; four threads per CTA tile sharing the parent fit through
-// shared memory took 21-23 us — more waves of a latency-bound kernel — so this stays.)
+// Round 1 ran one thread per 64x64 tile (a serial chain of ~2600 fp64 operations, 17 us on C2, and as
+// long for a single frame, where the GPU was nearly empty); here the chain is ~400 operations.
 constexpr int kSetupThreads = 128;
+constexpr int kSupPerBlock = kSetupThreads / kSupLanes;
 
-// INV: the batch contains DFR_SIP_INVERSE_EXACT sources (a separate instantiation, so the common
-// kernel is compiled exactly as without that feature: as a run-time flag alone it cost 6 us per call).
+__device__ __forceinline__ double shfl16(double v, int src_lane_in_group)
+{
+    return __shfl_sync(0xffffffffu, v, src_lane_in_group, kSupLanes);
+}
+
 template <int N, bool INV>
 __global__ void __launch_bounds__(kSetupThreads)
 tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ srcdev,
                   const __grid_constant__ TargetDev tgt, const __grid_constant__ FitConsts fc, int e0,
-                  int tiles_x, int tiles_y, int ctas_x, int ctas, int sny, int snx,
+                  int tiles_x, int tiles_y, int ctas_x, int ctas_y, int sups_x, int nsup, int sny, int snx,
                   TileRec *__restrict__ recs, int2 *__restrict__ cta_box, int32_t *__restrict__ counters,
                   int total_blocks, int32_t *__restrict__ host_stats, int stats_add, int late_consts)
 {
@@ -309,49 +333,103 @@ tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ 
     if (!late_consts) pdl_trigger();                // the main kernel's launch may overlap this one
     __syncthreads();
     if (!late_consts) pdl_wait();                   // the node table is complete
-    const int c = blockIdx.x * kSetupThreads + threadIdx.x;
-    int nflag[3] = {0, 0, 0};
-    if (c < ctas) {
-        const int cty = c / ctas_x, ctx = c - cty * ctas_x;
-        double Px[16], Py[16];                      // parent cubic, unit = 32 px
-        const bool parent = fit_cubic<N>(sm, inv_exact, fc, [&](int k) { return __ldg(uv + (size_t)k * ctas + c); }, Px, Py);
-        int box_x = kNoBox, box_y = kNoBox;
-#pragma unroll 1
-        for (int sub = 0; sub < CTA_T * CTA_T; ++sub) {
-            const int ttx = ctx * CTA_T + (sub % CTA_T), tty = cty * CTA_T + (sub / CTA_T);
-            if (ttx >= tiles_x || tty >= tiles_y) continue;
-            double Cx[16], Cy[16];
-            bool good = true;
-            if (parent) {
-                const double s0 = (sub % CTA_T) ? 0.5 : -0.5, t0 = (sub / CTA_T) ? 0.5 : -0.5;
+
+    const int l = threadIdx.x & (kSupLanes - 1);                // lane of the group: node / check point / tile
+    const int a = l & 3, b = l >> 2;
+    const int sidx_raw = blockIdx.x * kSupPerBlock + (threadIdx.x / kSupLanes);
+    const bool live = sidx_raw < nsup;                          // dead groups compute on super-tile 0 and write nothing
+    const int sidx = live ? sidx_raw : 0;
+    const int sy = sidx / sups_x, sx = sidx - sy * sups_x;
+
+    // ---- level 1: one node per lane, the fit through shuffles
+    double xs, ys;
+    {
+        const double2 q = __ldg(uv + (size_t)l * nsup + sidx);
+        source_xy_sm<N>(sm, inv_exact, q.x, q.y, xs, ys);
+    }
+    double Rx = 0.0, Ry = 0.0;                                  // row b, power a of s
 #pragma unroll
-                for (int k = 0; k < 16; ++k) { Cx[k] = Px[k]; Cy[k] = Py[k]; }
+    for (int k = 0; k < 4; ++k) {
+        const double w = fc.W[a][k];
+        Rx = fma(w, shfl16(xs, (b << 2) | k), Rx);
+        Ry = fma(w, shfl16(ys, (b << 2) | k), Ry);
+    }
+    double cxl = 0.0, cyl = 0.0;                                // coefficient of s^a t^b
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {       // along s, each power of t
-                    shift_half(Cx[4 * q], Cx[4 * q + 1], Cx[4 * q + 2], Cx[4 * q + 3], s0);
-                    shift_half(Cy[4 * q], Cy[4 * q + 1], Cy[4 * q + 2], Cy[4 * q + 3], s0);
-                }
+    for (int k = 0; k < 4; ++k) {
+        const double w = fc.W[b][k];
+        cxl = fma(w, shfl16(Rx, (k << 2) | a), cxl);
+        cyl = fma(w, shfl16(Ry, (k << 2) | a), cyl);
+    }
+    double Cx[16], Cy[16];                                      // C[4q + p]: s^p t^q, unit = 64 px
 #pragma unroll
-                for (int pp = 0; pp < 4; ++pp) {    // along t, each power of s
-                    shift_half(Cx[pp], Cx[4 + pp], Cx[8 + pp], Cx[12 + pp], t0);
-                    shift_half(Cy[pp], Cy[4 + pp], Cy[8 + pp], Cy[12 + pp], t0);
-                }
-            } else {
-                const double cx0 = ttx * TS + kCentre, cy0 = tty * TS + kCentre;
-                good = fit_cubic<N>(sm, inv_exact, fc, [&](int k) {
-                    double U, V;
-                    target_uv(tgt, cx0 + kHalf * fc.pts[k][0], cy0 + kHalf * fc.pts[k][1], U, V);
-                    return make_double2(U, V);
-                }, Cx, Cy);
-            }
-            int bx0, by0;
-            const int flag = emit_tile(Cx, Cy, good, sny, snx,
-                                       recs + ((size_t)e * tiles_x * tiles_y + (size_t)tty * tiles_x + ttx), bx0, by0);
-            ++nflag[flag];
-            if (flag == TILE_FAST) { box_x = min(box_x, bx0); box_y = min(box_y, by0); }
+    for (int k = 0; k < 16; ++k) {
+        Cx[k] = shfl16(cxl, k);
+        Cy[k] = shfl16(cyl, k);
+    }
+    bool ok;
+    {
+        const double2 q = __ldg(uv + (size_t)(kSupLanes + l) * nsup + sidx);
+        double x, y;
+        source_xy_sm<N>(sm, inv_exact, q.x, q.y, x, y);
+        const double ss = fc.sup[kSupLanes + l][0], tt = fc.sup[kSupLanes + l][1];
+        double px = 0.0, py = 0.0;
+#pragma unroll
+        for (int qq = 3; qq >= 0; --qq) {
+            const double rx = fma(fma(fma(Cx[4 * qq + 3], ss, Cx[4 * qq + 2]), ss, Cx[4 * qq + 1]), ss, Cx[4 * qq]);
+            const double ry = fma(fma(fma(Cy[4 * qq + 3], ss, Cy[4 * qq + 2]), ss, Cy[4 * qq + 1]), ss, Cy[4 * qq]);
+            px = fma(px, tt, rx);
+            py = fma(py, tt, ry);
         }
-        // origin of the CTA tile's staged box = min over its FAST tiles (kNoBox: none)
-        cta_box[(size_t)e * ctas + c] = make_int2(box_x, box_y);
+        // false on NaN; a NaN at a node poisons every coefficient, hence every lane's comparison
+        ok = (fabs(px - x) <= (double)FIT_TOL) && (fabs(py - y) <= (double)FIT_TOL);
+    }
+    const unsigned votes = __ballot_sync(0xffffffffu, ok);
+    const bool parent = ((votes >> (threadIdx.x & 16)) & 0xffffu) == 0xffffu;
+
+    // ---- this lane's tile
+    const int ttx = (sx * SUP_T * CTA_T) + a, tty = (sy * SUP_T * CTA_T) + b;
+    const bool mine = live && ttx < tiles_x && tty < tiles_y;
+    bool good = true;
+    if (parent) {
+        const double s0 = 0.5 * a - 0.75, t0 = 0.5 * b - 0.75;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {           // along s, each power of t
+            shift_quarter(Cx[4 * q], Cx[4 * q + 1], Cx[4 * q + 2], Cx[4 * q + 3], s0);
+            shift_quarter(Cy[4 * q], Cy[4 * q + 1], Cy[4 * q + 2], Cy[4 * q + 3], s0);
+        }
+#pragma unroll
+        for (int pp = 0; pp < 4; ++pp) {        // along t, each power of s
+            shift_quarter(Cx[pp], Cx[4 + pp], Cx[8 + pp], Cx[12 + pp], t0);
+            shift_quarter(Cy[pp], Cy[4 + pp], Cy[8 + pp], Cy[12 + pp], t0);
+        }
+    } else if (mine) {
+        // ---- level 2: this tile's own fit, target side on the fly
+        const double cx0 = ttx * TS + kCentre, cy0 = tty * TS + kCentre;
+        good = fit_cubic<N>(sm, inv_exact, fc, [&](int k) {
+            double U, V;
+            target_uv(tgt, cx0 + kHalf * fc.pts[k][0], cy0 + kHalf * fc.pts[k][1], U, V);
+            return make_double2(U, V);
+        }, Cx, Cy);
+    }
+    int nflag[3] = {0, 0, 0};
+    int box_x = kNoBox, box_y = kNoBox;
+    if (mine) {
+        int bx0, by0;
+        const int flag = emit_tile(Cx, Cy, good, sny, snx,
+                                   recs + ((size_t)e * tiles_x * tiles_y + (size_t)tty * tiles_x + ttx), bx0, by0);
+        ++nflag[flag];
+        if (flag == TILE_FAST) { box_x = bx0; box_y = by0; }
+    }
+    // origin of each CTA tile's staged box = min over its 2 x 2 FAST tiles (kNoBox: none)
+    box_x = min(box_x, __shfl_xor_sync(0xffffffffu, box_x, 1));
+    box_y = min(box_y, __shfl_xor_sync(0xffffffffu, box_y, 1));
+    box_x = min(box_x, __shfl_xor_sync(0xffffffffu, box_x, 4));
+    box_y = min(box_y, __shfl_xor_sync(0xffffffffu, box_y, 4));
+    if (live && (a & 1) == 0 && (b & 1) == 0) {
+        const int ctx = sx * SUP_T + (a >> 1), cty = sy * SUP_T + (b >> 1);
+        if (ctx < ctas_x && cty < ctas_y)
+            cta_box[(size_t)e * ctas_x * ctas_y + (size_t)cty * ctas_x + ctx] = make_int2(box_x, box_y);
     }
     // tile statistics: per-warp sums -> device counters; the last block of the last launch
     // (ticket) writes the totals straight into the caller's mapped host memory, so
@@ -445,7 +523,8 @@ cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const Sourc
     const int ctas = P.ctas_x * P.ctas_y;
     // one stream-ordered allocation from the library's pool, carved up (256-byte aligned pieces)
     auto up = [](size_t b) { return (b + 255) & ~(size_t)255; };
-    const size_t b_uv = up(sizeof(double2) * (size_t)ctas * NPTS), b_recs = up(sizeof(TileRec) * (size_t)ntile * n),
+    const int sups_x = (P.ctas_x + SUP_T - 1) / SUP_T, sups_y = (P.ctas_y + SUP_T - 1) / SUP_T, nsup = sups_x * sups_y;
+    const size_t b_uv = up(sizeof(double2) * (size_t)nsup * 2 * kSupLanes), b_recs = up(sizeof(TileRec) * (size_t)ntile * n),
                  b_box = up(sizeof(int2) * (size_t)ctas * n), b_cnt = up(4 * sizeof(int32_t));
     if ((err = scratch_alloc(&sc.block, b_uv + b_recs + b_box + b_cnt, st)) != cudaSuccess) return err;
     char *base = static_cast<char *>(sc.block);
@@ -455,9 +534,11 @@ cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const Sourc
     sc.counters = reinterpret_cast<int32_t *>(base + b_uv + b_recs + b_box);
     P.recs = sc.recs;
     P.cta_box = sc.cta_box;
-    target_nodes_kernel<<<(ctas * NPTS + 127) / 128, 128, 0, st>>>(tgt, fc, P.ctas_x, ctas, sc.uv, sc.counters,
+    static thread_local InlineConsts ic;            // kernel parameters are copied at launch
+    if (cc.inline_src) std::memcpy(&ic, cc.inline_src, cc.bytes);
+    target_nodes_kernel<<<(nsup * 2 * kSupLanes + 127) / 128, 128, 0, st>>>(tgt, fc, sups_x, nsup, sc.uv, sc.counters,
                                                                    static_cast<const uint4 *>(cc.src), static_cast<uint4 *>(cc.dst),
-                                                                   cc.src ? (int)(cc.bytes / 16) : 0);
+                                                                   (cc.src || cc.inline_src) ? (int)(cc.bytes / 16) : 0, ic);
     if ((err = cudaGetLastError()) != cudaSuccess) return err;
     // SIP order class of the batch: inverse polynomials are zero-padded up to N
     int maxo = 0;
@@ -466,15 +547,16 @@ cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const Sourc
         maxo = std::max(maxo, std::max(srchost[e].ap.order, srchost[e].bp.order));
         inv = inv || srchost[e].inv_exact != 0;
     }
-    const unsigned bx = (unsigned)((ctas + kSetupThreads - 1) / kSetupThreads);
+    const unsigned bx = (unsigned)((nsup + kSupPerBlock - 1) / kSupPerBlock);
     const long long total_blocks = (long long)bx * n;
     if (total_blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     for (int e0 = 0; e0 < n; e0 += 65535) {
         const dim3 grid(bx, (unsigned)std::min(n - e0, 65535));
 #define DFR_SETUP(NN, II)                                                                                           \
     launch_pdl(tile_setup_kernel<NN, II>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, \
-               P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters, (int)total_blocks,       \
-               host_stats, stats_add, cc.src ? 1 : 0)
+               P.tiles_x, P.tiles_y, P.ctas_x, P.ctas_y, sups_x, nsup, sny, snx, sc.recs, sc.cta_box, sc.counters,         \
+               (int)total_blocks,                                                                                       \
+               host_stats, stats_add, (cc.src || cc.inline_src) ? 1 : 0)
         if (maxo == 0) err = DFR_SETUP(0, false);
         else if (maxo <= 3) err = inv ? DFR_SETUP(3, true) : DFR_SETUP(3, false);
         else if (maxo <= 4) err = inv ? DFR_SETUP(4, true) : DFR_SETUP(4, false);
