@@ -115,45 +115,72 @@ struct CallConsts {
     }
 };
 
-// How the constants reach the device (the tiled path: by_kernel). Never by a copy-engine transfer
-// in front of the kernels (measured: +8 us per C2 step for the cross-engine dependency) and never
-// from pageable memory (the runtime does not always take the bytes before returning: reusing the
-// buffer made 2 of 8 test runs fail). Up to kInlineConstsBytes (three exposures) they ride in the
-// parameters of the first setup kernel; larger sets are written to the thread's pinned, device-mapped
-// staging ring and read from there by that kernel. Either way the kernel copies them to device
-// scratch for the kernels that follow. The other paths (exact, sky) enqueue a copy from the ring.
+// How the constants reach the device (ConstsCopy, dfr_tiled.h). On the tiled path (by_kernel) never
+// by a copy-engine transfer in front of the kernels, and never from pageable memory (the runtime does
+// not always take the bytes before returning: reusing the buffer made 2 of 8 test runs fail).
+// The per-exposure constants are built in a thread-local host array (`hsrc`: the launchers read it for
+// the staging decision); then either PACKED (only the coefficients the batch's highest order needs)
+// into the parameters of the first setup kernel, which expands them on the device, or — batches too
+// large for that — written to the thread's pinned, device-mapped ring and read from there by that
+// kernel. The other paths (exact, sky) enqueue a copy from the ring.
+static int tri_count(int order) { return (order + 1) * (order + 2) / 2; }
+
 static int upload_consts(DevCtx *c, int32_t n, const dfr_wcs *sw, const dfr_wcs *tw, bool with_weights,
                          const float *weights, cudaStream_t st, bool by_kernel, CallConsts &K)
 {
     make_target(tw, &K.tgt);
     const size_t b_src = sizeof(SourceDev) * (size_t)n;
     const size_t bytes = (b_src + (with_weights ? sizeof(float) * (size_t)n : 0) + 15) & ~(size_t)15;
-    const bool small = by_kernel && bytes <= kInlineConstsBytes;
+    static thread_local std::vector<SourceDev> t_src;           // host copy (never handed to CUDA)
+    if (t_src.size() < (size_t)n) t_src.resize((size_t)n);
+    SourceDev *h = t_src.data();
+    int maxo = 0;
+    for (int32_t e = 0; e < n; ++e) {
+        make_source(tw, &sw[e], &h[e]);
+        maxo = std::max(maxo, std::max(h[e].ap.order, h[e].bp.order));
+    }
     cudaError_t err;
-    char *stage;
-    static thread_local char t_small[kInlineConstsBytes];
-    if (small) {
-        stage = t_small;
-    } else {
-        if ((err = stage_acquire(c, bytes, &K.slot)) != cudaSuccess) return cuda_fail(err, "pinned staging buffer");
-        stage = static_cast<char *>(K.slot->host);
-    }
-    SourceDev *h = reinterpret_cast<SourceDev *>(stage);
-    for (int32_t e = 0; e < n; ++e) make_source(tw, &sw[e], &h[e]);
-    if (with_weights) {
-        float *hw = reinterpret_cast<float *>(stage + b_src);
-        for (int32_t e = 0; e < n; ++e) hw[e] = weights ? weights[e] : 1.0f;
-    }
     if ((err = scratch_alloc(&K.block, bytes, st)) != cudaSuccess) return cuda_fail(err, "scratch allocation (constants)");
     K.cc.dst = K.block;
     K.cc.bytes = bytes;
-    if (small) {
-        K.cc.inline_src = stage;
-    } else if (by_kernel) {
-        K.cc.src = K.slot->dev;
-    } else if ((err = cudaMemcpyAsync(K.block, stage, bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) {
-        K.finish(st);
-        return cuda_fail(err, "cudaMemcpyAsync(constants)");
+    const int T = tri_count(maxo), stride = kPackedHead + 2 * T;
+    const size_t packed_bytes = ((size_t)n * stride * 8 + (with_weights ? 4 * (size_t)n : 0) + 15) & ~(size_t)15;
+    if (by_kernel && packed_bytes <= (size_t)kPackedMaxBytes) {
+        static thread_local std::vector<unsigned long long> t_pack;
+        t_pack.assign(packed_bytes / 8, 0ull);
+        for (int32_t e = 0; e < n; ++e) {
+            unsigned long long *r = t_pack.data() + (size_t)e * stride;
+            std::memcpy(r, h[e].m, 9 * 8);
+            std::memcpy(r + 9, &h[e].c1, 8);
+            std::memcpy(r + 10, &h[e].c2, 8);
+            r[11] = (unsigned long long)(h[e].ap.order & 0xff) | ((unsigned long long)(h[e].bp.order & 0xff) << 8) |
+                    ((unsigned long long)(h[e].inv_exact & 0xff) << 16);
+            std::memcpy(r + kPackedHead, h[e].ap.c, (size_t)tri_count(h[e].ap.order) * 8);      // rest stays zero
+            std::memcpy(r + kPackedHead + T, h[e].bp.c, (size_t)tri_count(h[e].bp.order) * 8);
+        }
+        if (with_weights) {
+            float *hw = reinterpret_cast<float *>(t_pack.data() + (size_t)n * stride);
+            for (int32_t e = 0; e < n; ++e) hw[e] = weights ? weights[e] : 1.0f;
+        }
+        K.cc.packed = t_pack.data();
+        K.cc.packed_bytes = (int)packed_bytes;
+        K.cc.n = n;
+        K.cc.T = T;
+        K.cc.nweights = with_weights ? n : 0;
+    } else {
+        if ((err = stage_acquire(c, bytes, &K.slot)) != cudaSuccess) { K.finish(st); return cuda_fail(err, "pinned staging buffer"); }
+        char *stage = static_cast<char *>(K.slot->host);
+        std::memcpy(stage, h, b_src);
+        if (with_weights) {
+            float *hw = reinterpret_cast<float *>(stage + b_src);
+            for (int32_t e = 0; e < n; ++e) hw[e] = weights ? weights[e] : 1.0f;
+        }
+        if (by_kernel) {
+            K.cc.mapped = K.slot->dev;
+        } else if ((err = cudaMemcpyAsync(K.block, stage, bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) {
+            K.finish(st);
+            return cuda_fail(err, "cudaMemcpyAsync(constants)");
+        }
     }
     K.hsrc = h;
     K.dsrc = static_cast<SourceDev *>(K.block);

@@ -37,18 +37,25 @@ struct ProfileEvents {
     bool enabled;
 };
 
-// Per-call constants that the first setup kernel copies from mapped pinned host memory into device
-// scratch (a copy-engine upload would put a cross-engine dependency in front of every call:
-// measured +8 us per C2 step). src == nullptr: nothing to copy.
+// Per-call constants (SourceDev x n, then float weights x nweights) reach device scratch through the
+// first setup kernel, never through the copy engine (a copy in front of the kernels is a
+// cross-engine dependency: measured +8 us per C2 step). Two routes:
+//   packed  : a compact form (only the polynomial coefficients the batch's highest order needs) rides
+//             in the kernel's PARAMETERS and is expanded on the device — up to kPackedMaxBytes;
+//   mapped  : the full-size block sits in pinned, device-mapped host memory and is read from there.
 struct ConstsCopy {
-    const void *src = nullptr;          // device-visible address of the pinned staging buffer, or
-    const void *inline_src = nullptr;   // HOST address of at most kInlineConstsBytes that ride in the kernel parameters
-    void *dst = nullptr;                // device scratch
-    size_t bytes = 0;                   // multiple of 16
+    const void *packed = nullptr;       // HOST: packed form (see pack_consts in dfr_api.cu), or
+    const void *mapped = nullptr;       // device-visible address of the full-size block in the pinned ring
+    void *dst = nullptr;                // device scratch, `bytes` long
+    size_t bytes = 0;                   // full size, multiple of 16
+    int packed_bytes = 0, n = 0, T = 0, nweights = 0;      // packed: exposures, coefficients per polynomial, weights
+    bool any() const { return packed || mapped; }
 };
-constexpr size_t kInlineConstsBytes = 3 * 1024;     // three exposures' constants: single frames, small batches
-struct InlineConsts {
-    uint4 q[kInlineConstsBytes / 16];
+constexpr int kPackedSmallBytes = 3 * 1024;      // single frames: keeps the parameter block of the common launch small
+constexpr int kPackedMaxBytes = 28 * 1024;       // kernel parameters hold 32 764 bytes in all
+constexpr int kPackedHead = 12;                  // doubles per exposure before the coefficients: m[9], c1, c2, header
+template <int BYTES> struct PackedConsts {
+    uint4 q[BYTES / 16];
 };
 
 struct TiledParams {

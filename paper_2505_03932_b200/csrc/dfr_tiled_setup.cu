@@ -76,22 +76,56 @@ static FitConsts make_fit_consts()
 // ---------------------------------------------------------------------------------
 // setup kernels (fp64)
 // ---------------------------------------------------------------------------------
+// Expansion of the packed constants (ConstsCopy, dfr_tiled.h): word j of the full-size block.
+__device__ __forceinline__ unsigned long long expand_word(const unsigned long long *__restrict__ pk, int stride, int T, int j)
+{
+    constexpr int W = (int)(sizeof(SourceDev) / 8);             // 124 words per exposure
+    const int e = j / W, k = j - e * W;
+    const unsigned long long *r = pk + (size_t)e * stride;
+    const unsigned long long hdr = r[11];                        // ap.order | bp.order << 8 | inv_exact << 16
+    if (k < 11) return r[k];
+    if (k == 11) return hdr & 0xffull;                           // Poly ap: { int32 order, int32 pad }
+    if (k < 67) return (k - 12 < T) ? r[kPackedHead + (k - 12)] : 0ull;
+    if (k == 67) return (hdr >> 8) & 0xffull;
+    if (k < 123) return (k - 68 < T) ? r[kPackedHead + T + (k - 68)] : 0ull;
+    return (hdr >> 16) & 0xffull;                                // { int32 inv_exact, int32 pad }
+}
+
+template <int BYTES>
 __global__ void __launch_bounds__(128)
 target_nodes_kernel(const __grid_constant__ TargetDev tgt, const __grid_constant__ FitConsts fc,
                     int ctas_x, int ctas, double2 *__restrict__ uv, int32_t *__restrict__ counters,
-                    const uint4 *__restrict__ cc_src, uint4 *__restrict__ cc_dst, int cc_n16,
-                    const __grid_constant__ InlineConsts ic)
+                    const uint4 *__restrict__ cc_mapped, void *__restrict__ cc_dst, int cc_bytes,
+                    int pk_n, int pk_T, int pk_nw, const __grid_constant__ PackedConsts<BYTES> pk, int wide)
 {
     // tile counters + ticket of the setup kernel start from zero (no memset in the stream)
     if (blockIdx.x == 0 && threadIdx.x < 4) counters[threadIdx.x] = 0;
-    // the call's constants (per-exposure maps, weights): mapped pinned host memory -> device scratch
-    // (small sets ride in this kernel's parameters: cc_src == nullptr)
-    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < cc_n16; k += gridDim.x * blockDim.x)
-        cc_dst[k] = cc_src ? cc_src[k] : ic.q[k];
-    // sample points of the 64x64 CTA tiles (the parent fit of tile_setup_kernel)
+    // the call's constants (per-exposure maps, weights) -> device scratch
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+    if (cc_mapped) {
+        for (int k = tid; k < cc_bytes / 16; k += nth) static_cast<uint4 *>(cc_dst)[k] = cc_mapped[k];
+    } else if (pk_n > 0) {
+        const unsigned long long *src = reinterpret_cast<const unsigned long long *>(pk.q);
+        const int stride = kPackedHead + 2 * pk_T, words = pk_n * (int)(sizeof(SourceDev) / 8);
+        for (int j = tid; j < words; j += nth) static_cast<unsigned long long *>(cc_dst)[j] = expand_word(src, stride, pk_T, j);
+        const float *w = reinterpret_cast<const float *>(src + (size_t)pk_n * stride);
+        float *wd = reinterpret_cast<float *>(static_cast<char *>(cc_dst) + (size_t)pk_n * sizeof(SourceDev));
+        for (int j = tid; j < pk_nw; j += nth) wd[j] = w[j];
+    }
     pdl_trigger();                                  // the setup kernel may stage its constants meanwhile
-    // (ctas_x, ctas) here count SUPER-tiles
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (wide) {
+        // sample points of the 64x64 CTA tiles (tile_setup_wide_kernel): (ctas_x, ctas) count CTA tiles
+        if (idx >= ctas * NPTS) return;
+        const int c = idx / NPTS, k = idx - c * NPTS;
+        constexpr double edge = TS * CTA_T;
+        const double cx0 = (c % ctas_x) * edge + 0.5 * (edge - 1), cy0 = (c / ctas_x) * edge + 0.5 * (edge - 1);
+        double U, V;
+        target_uv(tgt, cx0 + 0.5 * edge * fc.pts[k][0], cy0 + 0.5 * edge * fc.pts[k][1], U, V);
+        uv[(size_t)k * ctas + c] = make_double2(U, V);          // [point][CTA tile]: coalesced for the setup kernel
+        return;
+    }
+    // (ctas_x, ctas) here count SUPER-tiles
     if (idx >= ctas * 2 * kSupLanes) return;
     const int c = idx / (2 * kSupLanes), k = idx - c * (2 * kSupLanes);
     constexpr double edge = kSupEdge;
@@ -193,6 +227,14 @@ __device__ __forceinline__ bool fit_cubic(const double *__restrict__ sm, bool in
 
 // p(s0 + s'/2) as a cubic in s': the re-centring of a parent cubic (unit = 32 px) on one of
 // its halves (unit = 16 px). Exact up to fp64 rounding.
+__device__ __forceinline__ void shift_half(double &c0, double &c1, double &c2, double &c3, double s0)
+{
+    const double d0 = fma(s0, fma(s0, fma(s0, c3, c2), c1), c0);
+    const double d1 = 0.5 * fma(s0, fma(3.0 * s0, c3, 2.0 * c2), c1);
+    const double d2 = 0.25 * fma(3.0 * s0, c3, c2);
+    c0 = d0; c1 = d1; c2 = d2; c3 = 0.125 * c3;
+}
+
 __device__ __forceinline__ void shift_quarter(double &c0, double &c1, double &c2, double &c3, double s0)
 {
     // p(s0 + s'/4) as a cubic in s': a 128-px parent (unit = 64 px) re-centred on a 32-px tile (unit = 16 px)
@@ -286,6 +328,7 @@ __device__ __forceinline__ int emit_tile(double (&Cx)[16], double (&Cy)[16], boo
 // Round 1 ran one thread per 64x64 tile (a serial chain of ~2600 fp64 operations, 17 us on C2, and as
 // long for a single frame, where the GPU was nearly empty); here the chain is ~400 operations.
 constexpr int kSetupThreads = 128;
+constexpr long long kWideThreshold = 16384;      // (CTA tiles x exposures) from which tile_setup_wide_kernel is used
 constexpr int kSupPerBlock = kSetupThreads / kSupLanes;
 
 __device__ __forceinline__ double shfl16(double v, int src_lane_in_group)
@@ -453,6 +496,126 @@ tile_setup_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ 
     }
 }
 
+// The WIDE form of the setup kernel, for launches that fill the GPU (C2: 32 768 CTA tiles):
+// one thread per (64x64 CTA tile, exposure); a block is 128 consecutive CTA tiles of ONE
+// exposure, so the exposure's constants are staged once in shared memory and every
+// coefficient read is a broadcast LDS. Two levels:
+//   1. the cubic is fitted and verified over the whole 64x64 CTA tile (25 map evaluations);
+//      if it holds, the four 32x32 tile records are its exact re-centrings (no more map
+//      evaluations) — 4x less fp64 work than fitting each tile;
+//   2. if it does not (strongly curved maps), each 32x32 tile gets its own fit, with the
+//      target side (a1-a2) evaluated on the fly; a tile whose own fit fails is EXACT.
+// Measured on B200, C2: 19.3 us under ncu against 25.7 us for the cooperative kernel above, whose
+// strength is its short serial chain when the grid is small (single frames).
+
+// INV: the batch contains DFR_SIP_INVERSE_EXACT sources (a separate instantiation, so the common
+// kernel is compiled exactly as without that feature: as a run-time flag alone it cost 6 us per call).
+template <int N, bool INV>
+__global__ void __launch_bounds__(kSetupThreads)
+tile_setup_wide_kernel(const double2 *__restrict__ uv, const SourceDev *__restrict__ srcdev,
+                  const __grid_constant__ TargetDev tgt, const __grid_constant__ FitConsts fc, int e0,
+                  int tiles_x, int tiles_y, int ctas_x, int ctas, int sny, int snx,
+                  TileRec *__restrict__ recs, int2 *__restrict__ cta_box, int32_t *__restrict__ counters,
+                  int total_blocks, int32_t *__restrict__ host_stats, int stats_add, int late_consts)
+{
+    __shared__ double sm[11 + 2 * tri(N)];
+    const int e = e0 + blockIdx.y;
+    // The exposure's constants -> shared memory. When they were uploaded by a copy earlier in the
+    // stream they are staged BEFORE waiting for the node kernel (this kernel's launch overlaps it);
+    // when the node kernel itself brings them in (late_consts), after.
+    if (late_consts) {
+        pdl_trigger();
+        pdl_wait();
+    }
+    const bool inv_exact = INV && N > 0 && srcdev[e].inv_exact != 0;
+    {
+        const SourceDev &s = srcdev[e];
+        for (int k = threadIdx.x; k < 11 + 2 * tri(N); k += blockDim.x) {
+            double v;
+            if (k < 9) v = s.m[k];
+            else if (k == 9) v = s.c1;
+            else if (k == 10) v = s.c2;
+            else {
+                // slot of the order-N layout -> (p, q) -> slot of the stored order-n layout
+                const int t = (k - 11) % tri(N);
+                const Poly &P = (k - 11) < tri(N) ? s.ap : s.bp;
+                int p = 0;
+                while (p < N && tri_off(N, p + 1) <= t) ++p;
+                const int q = t - tri_off(N, p), n = P.order;
+                v = (p + q <= n) ? P.c[tri_off(n, p) + q] : 0.0;
+            }
+            sm[k] = v;
+        }
+    }
+    if (!late_consts) pdl_trigger();                // the main kernel's launch may overlap this one
+    __syncthreads();
+    if (!late_consts) pdl_wait();                   // the node table is complete
+    const int c = blockIdx.x * kSetupThreads + threadIdx.x;
+    int nflag[3] = {0, 0, 0};
+    if (c < ctas) {
+        const int cty = c / ctas_x, ctx = c - cty * ctas_x;
+        double Px[16], Py[16];                      // parent cubic, unit = 32 px
+        const bool parent = fit_cubic<N>(sm, inv_exact, fc, [&](int k) { return __ldg(uv + (size_t)k * ctas + c); }, Px, Py);
+        int box_x = kNoBox, box_y = kNoBox;
+#pragma unroll 1
+        for (int sub = 0; sub < CTA_T * CTA_T; ++sub) {
+            const int ttx = ctx * CTA_T + (sub % CTA_T), tty = cty * CTA_T + (sub / CTA_T);
+            if (ttx >= tiles_x || tty >= tiles_y) continue;
+            double Cx[16], Cy[16];
+            bool good = true;
+            if (parent) {
+                const double s0 = (sub % CTA_T) ? 0.5 : -0.5, t0 = (sub / CTA_T) ? 0.5 : -0.5;
+#pragma unroll
+                for (int k = 0; k < 16; ++k) { Cx[k] = Px[k]; Cy[k] = Py[k]; }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {       // along s, each power of t
+                    shift_half(Cx[4 * q], Cx[4 * q + 1], Cx[4 * q + 2], Cx[4 * q + 3], s0);
+                    shift_half(Cy[4 * q], Cy[4 * q + 1], Cy[4 * q + 2], Cy[4 * q + 3], s0);
+                }
+#pragma unroll
+                for (int pp = 0; pp < 4; ++pp) {    // along t, each power of s
+                    shift_half(Cx[pp], Cx[4 + pp], Cx[8 + pp], Cx[12 + pp], t0);
+                    shift_half(Cy[pp], Cy[4 + pp], Cy[8 + pp], Cy[12 + pp], t0);
+                }
+            } else {
+                const double cx0 = ttx * TS + kCentre, cy0 = tty * TS + kCentre;
+                good = fit_cubic<N>(sm, inv_exact, fc, [&](int k) {
+                    double U, V;
+                    target_uv(tgt, cx0 + kHalf * fc.pts[k][0], cy0 + kHalf * fc.pts[k][1], U, V);
+                    return make_double2(U, V);
+                }, Cx, Cy);
+            }
+            int bx0, by0;
+            const int flag = emit_tile(Cx, Cy, good, sny, snx,
+                                       recs + ((size_t)e * tiles_x * tiles_y + (size_t)tty * tiles_x + ttx), bx0, by0);
+            ++nflag[flag];
+            if (flag == TILE_FAST) { box_x = min(box_x, bx0); box_y = min(box_y, by0); }
+        }
+        // origin of the CTA tile's staged box = min over its FAST tiles (kNoBox: none)
+        cta_box[(size_t)e * ctas + c] = make_int2(box_x, box_y);
+    }
+    // tile statistics: per-warp sums -> device counters; the last block of the last launch
+    // (ticket) writes the totals straight into the caller's mapped host memory, so
+    // dfr_last_stats needs neither a memset nor a copy in the stream
+#pragma unroll
+    for (int f = 0; f < 3; ++f) {
+        const int w = __reduce_add_sync(0xffffffffu, nflag[f]);
+        if ((threadIdx.x & 31) == 0 && w) atomicAdd(&counters[f], w);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0 && host_stats) {
+        __threadfence();
+        if (atomicAdd(&counters[3], 1) == total_blocks - 1) {
+            __threadfence();
+            for (int f = 0; f < 3; ++f) {
+                const int32_t v = *(volatile int32_t *)&counters[f];
+                if (stats_add) atomicAdd(&host_stats[f], v);     // streaming calls: device-side totals
+                else host_stats[f] = v;
+            }
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------
@@ -524,7 +687,10 @@ cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const Sourc
     // one stream-ordered allocation from the library's pool, carved up (256-byte aligned pieces)
     auto up = [](size_t b) { return (b + 255) & ~(size_t)255; };
     const int sups_x = (P.ctas_x + SUP_T - 1) / SUP_T, sups_y = (P.ctas_y + SUP_T - 1) / SUP_T, nsup = sups_x * sups_y;
-    const size_t b_uv = up(sizeof(double2) * (size_t)nsup * 2 * kSupLanes), b_recs = up(sizeof(TileRec) * (size_t)ntile * n),
+    // which setup kernel: the wide one (a thread per 64x64 tile) when the launch fills the GPU anyway,
+    // the cooperative one (16 lanes per 128x128 super-tile, short serial chain) otherwise
+    const bool wide = (long long)ctas * n >= kWideThreshold;
+    const size_t b_uv = up(sizeof(double2) * std::max((size_t)nsup * 2 * kSupLanes, (size_t)ctas * NPTS)), b_recs = up(sizeof(TileRec) * (size_t)ntile * n),
                  b_box = up(sizeof(int2) * (size_t)ctas * n), b_cnt = up(4 * sizeof(int32_t));
     if ((err = scratch_alloc(&sc.block, b_uv + b_recs + b_box + b_cnt, st)) != cudaSuccess) return err;
     char *base = static_cast<char *>(sc.block);
@@ -534,11 +700,22 @@ cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const Sourc
     sc.counters = reinterpret_cast<int32_t *>(base + b_uv + b_recs + b_box);
     P.recs = sc.recs;
     P.cta_box = sc.cta_box;
-    static thread_local InlineConsts ic;            // kernel parameters are copied at launch
-    if (cc.inline_src) std::memcpy(&ic, cc.inline_src, cc.bytes);
-    target_nodes_kernel<<<(nsup * 2 * kSupLanes + 127) / 128, 128, 0, st>>>(tgt, fc, sups_x, nsup, sc.uv, sc.counters,
-                                                                   static_cast<const uint4 *>(cc.src), static_cast<uint4 *>(cc.dst),
-                                                                   (cc.src || cc.inline_src) ? (int)(cc.bytes / 16) : 0, ic);
+    {
+        const unsigned nb = (unsigned)(((wide ? ctas * NPTS : nsup * 2 * kSupLanes) + 127) / 128);
+        const int nx_ = wide ? P.ctas_x : sups_x, nn_ = wide ? ctas : nsup;
+        const uint4 *mp = static_cast<const uint4 *>(cc.mapped);
+        if (cc.packed && cc.packed_bytes > kPackedSmallBytes) {
+            static thread_local PackedConsts<kPackedMaxBytes> pk;         // kernel parameters are copied at launch
+            std::memcpy(&pk, cc.packed, (size_t)cc.packed_bytes);
+            target_nodes_kernel<kPackedMaxBytes><<<nb, 128, 0, st>>>(tgt, fc, nx_, nn_, sc.uv, sc.counters, mp, cc.dst,
+                                                                     (int)cc.bytes, cc.n, cc.T, cc.nweights, pk, wide ? 1 : 0);
+        } else {
+            static thread_local PackedConsts<kPackedSmallBytes> pk;
+            if (cc.packed) std::memcpy(&pk, cc.packed, (size_t)cc.packed_bytes);
+            target_nodes_kernel<kPackedSmallBytes><<<nb, 128, 0, st>>>(tgt, fc, nx_, nn_, sc.uv, sc.counters, mp, cc.dst,
+                                                                       (int)cc.bytes, cc.packed ? cc.n : 0, cc.T, cc.nweights, pk, wide ? 1 : 0);
+        }
+    }
     if ((err = cudaGetLastError()) != cudaSuccess) return err;
     // SIP order class of the batch: inverse polynomials are zero-padded up to N
     int maxo = 0;
@@ -547,16 +724,18 @@ cudaError_t run_setup(int n, int sny, int snx, const TargetDev &tgt, const Sourc
         maxo = std::max(maxo, std::max(srchost[e].ap.order, srchost[e].bp.order));
         inv = inv || srchost[e].inv_exact != 0;
     }
-    const unsigned bx = (unsigned)((nsup + kSupPerBlock - 1) / kSupPerBlock);
+    const unsigned bx = wide ? (unsigned)((ctas + kSetupThreads - 1) / kSetupThreads) : (unsigned)((nsup + kSupPerBlock - 1) / kSupPerBlock);
     const long long total_blocks = (long long)bx * n;
     if (total_blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     for (int e0 = 0; e0 < n; e0 += 65535) {
         const dim3 grid(bx, (unsigned)std::min(n - e0, 65535));
 #define DFR_SETUP(NN, II)                                                                                           \
-    launch_pdl(tile_setup_kernel<NN, II>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt, fc, e0, \
-               P.tiles_x, P.tiles_y, P.ctas_x, P.ctas_y, sups_x, nsup, sny, snx, sc.recs, sc.cta_box, sc.counters,         \
-               (int)total_blocks,                                                                                       \
-               host_stats, stats_add, (cc.src || cc.inline_src) ? 1 : 0)
+    (wide ? launch_pdl(tile_setup_wide_kernel<NN, II>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev,  \
+                       tgt, fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, ctas, sny, snx, sc.recs, sc.cta_box, sc.counters,     \
+                       (int)total_blocks, host_stats, stats_add, cc.any() ? 1 : 0)                                        \
+          : launch_pdl(tile_setup_kernel<NN, II>, grid, dim3(kSetupThreads), 0, st, (const double2 *)sc.uv, srcdev, tgt,  \
+                       fc, e0, P.tiles_x, P.tiles_y, P.ctas_x, P.ctas_y, sups_x, nsup, sny, snx, sc.recs, sc.cta_box,     \
+                       sc.counters, (int)total_blocks, host_stats, stats_add, cc.any() ? 1 : 0))
         if (maxo == 0) err = DFR_SETUP(0, false);
         else if (maxo <= 3) err = inv ? DFR_SETUP(3, true) : DFR_SETUP(3, false);
         else if (maxo <= 4) err = inv ? DFR_SETUP(4, true) : DFR_SETUP(4, false);
