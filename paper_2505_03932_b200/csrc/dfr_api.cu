@@ -715,6 +715,8 @@ int dfr_reproject_host_multi(const float *src_host, int32_t n, int32_t src_ny, i
                                        order, out_host + out_px * lo, std::min(batch, hi - lo));
             if (r.rc != DFR_OK) r.error = last_error_cstr();
             for (int q = 0; q < 4; ++q) r.stats[q] = g_stats_acc[q];
+            g_last = LastCall();
+            release_thread_contexts();              // this thread ends here: nothing of it may stay behind
         });
     for (std::thread &t : workers) t.join();
     for (int q = 0; q < 4; ++q) g_stats_acc[q] = 0;
@@ -756,6 +758,8 @@ int dfr_stack_host_multi(const float *src_host, int32_t n, int32_t src_ny, int32
                                    std::min(batch, hi - lo), &partial[(size_t)k]);
             if (r.rc != DFR_OK) r.error = last_error_cstr();
             for (int q = 0; q < 4; ++q) r.stats[q] = g_stats_acc[q];
+            g_last = LastCall();
+            release_thread_contexts();              // this thread ends here: nothing of it may stay behind
         });
     for (std::thread &t : workers) t.join();
     for (int q = 0; q < 4; ++q) g_stats_acc[q] = 0;

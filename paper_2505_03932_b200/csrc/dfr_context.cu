@@ -133,6 +133,18 @@ cudaError_t stage_done(PinnedSlot *slot, cudaStream_t st)
     return cudaEventRecord(slot->copied, st);
 }
 
+void release_thread_contexts()
+{
+    int prev = 0;
+    const bool have = cudaGetDevice(&prev) == cudaSuccess;
+    for (DevCtx *c : t_ctx) {
+        cudaSetDevice(c->dev);
+        destroy_ctx(c);
+    }
+    t_ctx.clear();
+    if (have) cudaSetDevice(prev);
+}
+
 void release_current_device()
 {
     int dev = 0;

@@ -50,5 +50,9 @@ cudaError_t stage_done(PinnedSlot *slot, cudaStream_t st);
 
 // dfr_release: free what this thread keeps for the current device and trim the scratch pool.
 void release_current_device();
+// Free every context of the calling thread (all devices). For the library's own short-lived
+// worker threads (the *_multi entry points), whose work has been synchronised: without it every
+// such thread would leave its events and pinned staging memory behind.
+void release_thread_contexts();
 
 }  // namespace dfr

@@ -724,3 +724,23 @@ def test_exact_inverse_sip_on_device(P, path):
     xr, yr = P.dfr_world2pix(exact, ra, dec)
     assert float((xr - x).abs().max()) < 1e-7 and float((yr - y).abs().max()) < 1e-7
     print("exact inverse", path, st)
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_exact_inverse_that_cannot_converge_gives_nan(P, path):
+    """DFR_SIP_INVERSE_EXACT on a distortion whose gradient exceeds 1 (no fixed point to converge
+    to): the documented outcome is NaN coordinates, hence NaN pixels — not a hang, not garbage.
+    Near CRPIX, where the gradient is small, the solve still converges."""
+    n = 256
+    src = S.make_wcs(n, n, 150.0, 2.0, 0.0, S.PIXSCALE)
+    src.a_order = src.b_order = 2
+    src.a[2][0] = 2e-2                       # dA/du = 0.04 u: > 1 beyond 25 px from CRPIX
+    src.ap_order = src.bp_order = -1
+    tgt = S.make_wcs(n, n, 150.0, 2.0, 0.0, S.PIXSCALE)
+    x, y = P.dfr_src_coords([src], tgt, (n, n), (n, n), 1, path=PATHS[path])
+    x = x[0].cpu().numpy()
+    assert np.isnan(x[:, :60]).all() and np.isnan(x[:, 200:]).all()
+    centre = x[120:136, 124:132]
+    assert np.isfinite(centre).all()
+    out = P.dfr_reproject(torch.ones((1, n, n), device="cuda"), [src], tgt, (n, n), 1, path=PATHS[path])
+    assert bool(torch.isnan(out[0, :, :60]).all()) and bool((out[0, 120:136, 124:132] == 1).all())
