@@ -744,3 +744,77 @@ def test_exact_inverse_that_cannot_converge_gives_nan(P, path):
     assert np.isfinite(centre).all()
     out = P.dfr_reproject(torch.ones((1, n, n), device="cuda"), [src], tgt, (n, n), 1, path=PATHS[path])
     assert bool(torch.isnan(out[0, :, :60]).all()) and bool((out[0, 120:136, 124:132] == 1).all())
+
+
+def test_maximum_frame_size_index_arithmetic(P):
+    """Frames at the size limit of the ABI (ny * nx < 2^31 pixels: 46340 x 46340 = 8.6 GB each way):
+    every byte offset above 4 GB, every element index near 2^31. The source is a linear ramp built
+    on the device, which bilinear interpolation reproduces exactly (pin P10), so the expected value
+    of a pixel is the ramp at the ORACLE's source coordinate: 400 000 sampled output pixels
+    (including the four corners and the last rows) computed one by one through the oracle's sky
+    entry points, plus the NaN mask."""
+    n = 46340
+    free, _ = torch.cuda.mem_get_info()
+    if free < 20 * 2 ** 30:
+        pytest.skip("needs 20 GB of free device memory")
+    ax, ay, c0 = 0.25, 0.5, 7.0
+    src = torch.empty((1, n, n), dtype=torch.float32, device="cuda")
+    xs = torch.arange(n, dtype=torch.float32, device="cuda")
+    for j0 in range(0, n, 4096):                                   # row blocks: no second full-size temporary
+        j1 = min(n, j0 + 4096)
+        src[0, j0:j1] = c0 + ax * xs[None, :] + ay * torch.arange(j0, j1, dtype=torch.float32, device="cuda")[:, None]
+    sw = S.make_wcs(n, n, 150.0, 2.0, 0.0, S.PIXSCALE)
+    tw = S.make_wcs(n, n, 150.02, 1.99, 0.4, S.PIXSCALE)          # ~25 px shift, 0.4 deg: NaN wedges on all sides
+    out = P.dfr_reproject(src, [sw], tw, (n, n), 1)
+    torch.cuda.synchronize()
+    st = P.dfr_last_stats()
+    assert st["tiles_fast"] + st["tiles_exact"] + st["tiles_empty"] == ((n + 31) // 32) ** 2
+    rng = np.random.default_rng(4634)
+    ii = np.concatenate([rng.integers(0, n, 399990), [0, n - 1, 0, n - 1, n - 1, n - 2, 1, n - 1, n // 2, n - 1]]).astype(np.float64)
+    jj = np.concatenate([rng.integers(0, n, 399990), [0, 0, n - 1, n - 1, n - 2, n - 1, n - 1, 1, n - 1, n // 2]]).astype(np.float64)
+    ra, dec = oracle.pix2world(tw, ii, jj)
+    xo, yo = oracle.world2pix(sw, ra, dec)
+    got = out[0][torch.from_numpy(jj.astype(np.int64)).cuda(), torch.from_numpy(ii.astype(np.int64)).cuda()].cpu().numpy()
+    inside = (xo >= -0.5) & (xo < n - 0.5) & (yo >= -0.5) & (yo < n - 0.5)
+    band = PR.edge_band(xo, yo, n, n)
+    assert np.array_equal(np.isnan(got)[~band], ~inside[~band])
+    # edge replication: the ramp is evaluated at the coordinate clamped to the pixel-centre hull
+    want = c0 + ax * np.clip(xo, 0, n - 1) + ay * np.clip(yo, 0, n - 1)
+    ok = inside & ~band
+    dr = ax * (n - 1) + ay * (n - 1)
+    err = np.abs(got[ok] - want[ok])
+    # 1e-5 x DR = 0.35; what is actually expected: coordinate error (<= 1e-4 px) x slope + float32 rounding of the ramp (ulp 0.004)
+    assert err.max() <= 0.01, err.max()
+    assert 0.9 < ok.mean() < 1.0 and err.max() <= PR.VALUE_TOL * dr
+    del out, src
+
+
+def test_more_exposures_than_one_grid_dimension(P):
+    """n > 65535 exposures in one call: the exposure index no longer fits grid.y / grid.z, so the
+    launchers cut the batch; every exposure must still get its own WCS and its own image."""
+    n, npx = 66000, 8
+    rng = np.random.default_rng(66)
+    imgs = rng.normal(100.0, 5.0, (n, npx, npx)).astype(np.float32)
+    base = S.make_wcs(npx, npx, 150.0, 2.0, 0.0, S.PIXSCALE)
+    tgt = S.make_wcs(npx, npx, 150.0, 2.0, 0.0, S.PIXSCALE)
+    ws = (P.DfrWCS * n)()
+    proto = P.pack_wcs(base)
+    shifts = rng.integers(-2, 3, (n, 2))
+    for k in range(n):
+        ws[k] = proto
+        ws[k].crpix[0] = base.crpix[0] + float(shifts[k, 0])
+        ws[k].crpix[1] = base.crpix[1] + float(shifts[k, 1])
+    src = torch.from_numpy(imgs).cuda()
+    out = P.dfr_reproject(src, ws, tgt, (npx, npx), 0).cpu().numpy()
+    for k in (0, 1, 65534, 65535, 65536, 65999):
+        dx, dy = int(shifts[k, 0]), int(shifts[k, 1])              # source pixel = target pixel + shift
+        want = np.full((npx, npx), np.nan, dtype=np.float32)
+        for j in range(npx):
+            for i in range(npx):
+                if 0 <= i + dx < npx and 0 <= j + dy < npx:
+                    want[j, i] = imgs[k, j + dy, i + dx]
+        assert np.array_equal(np.nan_to_num(out[k], nan=-1), np.nan_to_num(want, nan=-1)), k
+    s, c = P.dfr_reproject_stack(src, ws, tgt, (npx, npx), 0)
+    valid = ~np.isnan(out)
+    assert np.array_equal(c.cpu().numpy(), valid.sum(0).astype(np.float32))
+    assert np.allclose(s.cpu().numpy(), np.where(valid, out, 0).astype(np.float64).sum(0), rtol=1e-4)
