@@ -189,11 +189,14 @@ int dfr_shard_range(int32_t n, int32_t parts, int32_t k, int32_t *lo, int32_t *h
  *   wsum[j][i] (+)= sum over the same e of weights[e]
  * where v_e is what dfr_reproject would store for exposure e, and exposure e
  * contributes to a pixel only where v_e is not NaN (inside its footprint and no
- * NaN under the taps). Accumulation is float32. Large batches are split into exposure
- * chunks whose partial sums are combined with atomic adds, so the last bits of `sum` may
- * differ from run to run; `wsum` is exact whenever the weights' partial sums are.
+ * NaN under the taps). Accumulation is float32, in exposure order within one kernel pass;
+ * every output pixel has one owner (small outputs are cut into exposure chunks whose partial
+ * sums are added in chunk order), so the same call gives the same bits on every run. `wsum` is
+ * exact whenever the weights' partial sums are (it is the sum of a per-tile and a per-pixel part).
+ * With accumulate = 1 the batch is added by plain read-modify-write: do not run two such calls on
+ * the same sum / wsum concurrently on different streams.
  *   src_batch, src_wcs, tgt_wcs, out_ny/nx, order : as dfr_reproject
- *   weights    : HOST float32[n], or NULL for 1.0 each (must be finite)
+ *   weights    : HOST float32[n], or NULL for 1.0 each (must be finite: DFR_ERR_WEIGHT)
  *   sum, wsum  : DEVICE float32 [out_ny][out_nx] each; must not overlap src_batch
  *                or each other
  *   accumulate : 0 = both arrays are overwritten; 1 = the batch is added to their
