@@ -51,8 +51,9 @@ def kernel_source_hash():
     import hashlib
     h = hashlib.sha256()
     csrc = os.path.join(ROOT, "paper_2505_03932_b200", "csrc")
-    for f in sorted(glob.glob(os.path.join(csrc, "*.cu")) + glob.glob(os.path.join(csrc, "*.cuh"))
-                    + glob.glob(os.path.join(csrc, "*.h"))):
+    # the KERNEL sources: what the captured DRAM traffic depends on (not the host-side API files)
+    for f in sorted(glob.glob(os.path.join(csrc, "dfr_tiled*")) + [os.path.join(csrc, "dfr_device.cuh"),
+                                                                    os.path.join(csrc, "dfr_internal.h")]):
         h.update(os.path.basename(f).encode())
         h.update(open(f, "rb").read())
     return h.hexdigest()[:16]
