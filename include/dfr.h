@@ -154,6 +154,40 @@ int dfr_reproject_ex(const float *src_batch, int32_t n, int32_t src_ny, int32_t 
                      int32_t out_ny, int32_t out_nx, int32_t order,
                      float *out, void *stream, int32_t path);
 
+/* dfr_reproject for callers that must not trigger a device allocation.
+ *
+ * Every other entry point draws per-call scratch from a CUDA memory pool and keeps events and
+ * pinned staging memory per host thread. Two kinds of caller cannot live with that: code that
+ * shares the GPU with something that already owns all of its memory (a framework's caching
+ * allocator grown to the whole card, a reduction pipeline that reserved HBM for the night's
+ * frames), where the library's first allocation may simply fail; and real-time loops (quick-look
+ * reduction between read-outs) that cannot risk the device-wide synchronisation cudaMalloc /
+ * cudaFree may imply. This entry point calls no cudaMalloc, cudaFree, cudaMallocAsync, pool,
+ * event, stream or pinned-memory routine. The only scratch its kernel needs, the table of
+ * per-exposure constants, is a fixed array inside the library image:
+ *   limit : n <= DFR_NOALLOC_MAX_EXPOSURES per call (more -> DFR_ERR_SHAPE, nothing written);
+ *   cost  : DFR_NOALLOC_MAX_EXPOSURES x 992 B = 63 488 B on every GPU that loads libdfr, held
+ *           from load until the process exits, used or not.
+ * What it computes: steps a1-a9 of SURVEY.md §8(a) through the exact
+ * per-pixel fp64 map with direct gathers — the same arithmetic as dfr_reproject_ex(...,
+ * DFR_PATH_EXACT), bit for bit, area footprint rule. It is slower than the tiled path of
+ * dfr_reproject (that path's scratch grows with the output size and does not fit a fixed array).
+ * Arguments, layouts, asynchrony and validation errors are those of dfr_reproject; the caller
+ * owns and passes src_batch and out as usual.
+ * First call per device: the first call made with a given device current looks up the array's
+ * device address (cudaGetSymbolAddress, which also makes the runtime load the library's device
+ * code there) and remembers it. Make that first call during set-up, outside any stream capture.
+ * Sharing: all calls on a device use the same array, which keeps the previous call's contents;
+ * each call overwrites the n entries it reads before reading them, so nothing needs clearing and
+ * calls issued on ONE stream are safe back to back. Two calls that can overlap on the GPU
+ * (different streams, or different host threads, same device) race on the array: the later
+ * call's constants may replace the earlier call's while its kernel still runs. Serialise them. */
+#define DFR_NOALLOC_MAX_EXPOSURES 64
+int dfr_reproject_noalloc(const float *src_batch, int32_t n, int32_t src_ny, int32_t src_nx,
+                          const dfr_wcs *src_wcs, const dfr_wcs *tgt_wcs,
+                          int32_t out_ny, int32_t out_nx, int32_t order,
+                          float *out, void *stream);
+
 /* End-to-end form with HOST buffers (">1000 exposures"; SURVEY.md
  * §8(a) a10): src_host [n][src_ny][src_nx] and out_host [n][out_ny][out_nx]
  * are HOST float32 arrays (pinned memory gives full PCIe rate, pageable

@@ -21,6 +21,7 @@ EDGE_AREA, EDGE_PAPER = 0, 1
 _ORDER_NAMES = {"nearest": 0, "nearest-neighbor": 0, "bilinear": 1, "bicubic": 3}
 
 EXPORTS = ["dfr_reproject", "dfr_reproject_edge", "dfr_reproject_ex", "dfr_reproject_fp", "dfr_reproject_host",
+           "dfr_reproject_noalloc",
            "dfr_reproject_host_multi", "dfr_reproject_stack", "dfr_shard_range", "dfr_release",
            "dfr_stack_finalize", "dfr_stack_host", "dfr_stack_host_multi", "dfr_pix2world",
            "dfr_world2pix", "dfr_src_coords", "dfr_wcs_set_pc_cdelt", "dfr_wcs_fit_inverse_sip", "dfr_last_stats",
@@ -58,6 +59,7 @@ def lib():
         i32, i64 = C.c_int32, C.c_int64
         L.dfr_reproject.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, vp]
         L.dfr_reproject_ex.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, vp, i32]
+        L.dfr_reproject_noalloc.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, vp]
         L.dfr_reproject_edge.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, i32, fp, vp]
         L.dfr_reproject_fp.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, i32, fp, fp, vp]
         L.dfr_reproject_host.argtypes = [fp, i32, i32, i32, wp, wp, i32, i32, i32, fp, i32]
@@ -176,6 +178,38 @@ def dfr_reproject(src_batch, src_wcs, tgt_wcs, shape_out=None, order=BILINEAR, o
             _check(lib().dfr_reproject_ex(src_batch.data_ptr(), n, sny, snx, ws, C.byref(tw), ony, onx,
                                           _order(order), out.data_ptr(), _stream_ptr(stream), int(path)))
     return out if fp_t is None else (out, fp_t)
+
+
+NOALLOC_MAX_EXPOSURES = 64          # DFR_NOALLOC_MAX_EXPOSURES (include/dfr.h)
+
+
+def dfr_reproject_noalloc(src_batch, src_wcs, tgt_wcs, out, order=BILINEAR, stream=None):
+    """dfr_reproject_noalloc (include/dfr.h): the exact per-pixel reprojection for callers that
+    cannot afford a device allocation inside the call — the GPU's memory already belongs to
+    another allocator, or the call sits in a real-time loop where cudaMalloc / cudaFree (and the
+    device-wide synchronisation they may bring) are off limits. The library allocates nothing:
+    its constants table is a fixed 63 488-byte array in the library image, hence at most
+    NOALLOC_MAX_EXPOSURES exposures per call. Neither does this wrapper: `out`, a CUDA float32
+    [n][out_ny][out_nx] tensor, is the caller's and gives shape_out. Results equal
+    dfr_reproject(..., path=PATH_EXACT). Make the first call on a device during set-up (it looks
+    up the array's address); calls that may overlap on the GPU share the table and race."""
+    import torch
+    if src_batch.dim() == 2:
+        src_batch = src_batch[None]
+    _need_cuda(src_batch, torch.float32, "src_batch")
+    _need_cuda(out, torch.float32, "out")
+    n, sny, snx = src_batch.shape
+    if out.dim() != 3 or out.shape[0] != n:
+        raise ValueError("out must be [n][out_ny][out_nx]")
+    ws = pack_wcs_array(src_wcs)
+    if len(ws) != n:
+        raise ValueError("one source WCS per exposure")
+    tw = pack_wcs(tgt_wcs)
+    with torch.cuda.device(src_batch.device):
+        _check(lib().dfr_reproject_noalloc(src_batch.data_ptr(), n, sny, snx, ws, C.byref(tw),
+                                           int(out.shape[1]), int(out.shape[2]), _order(order),
+                                           out.data_ptr(), _stream_ptr(stream)))
+    return out
 
 
 def dfr_reproject_host(src_host, src_wcs, tgt_wcs, shape_out=None, order=BILINEAR, out_host=None,
