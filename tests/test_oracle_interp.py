@@ -308,3 +308,54 @@ def test_f4_paper_mode_rejects_bicubic_and_nearest_matches_area_rule():
     val, _ = oracle.interp_paper(img, x, y, 0)
     area = oracle.interp(img, x, y, 0)
     assert np.array_equal(np.isnan(val), np.isnan(area)) and np.array_equal(np.nan_to_num(val), np.nan_to_num(area))
+
+
+# ------------------------------------------------- G14: NaN source pixels under the 16 bicubic taps
+def test_g14_bicubic_nan_reach_is_exactly_the_4x4_taps():
+    """Reading G14: a NaN source pixel poisons a sample iff it lies under one of the
+    taps read — for bicubic the edge-replicated 4x4 neighbourhood floor(x)-1 .. floor(x)+2, including
+    taps whose Keys weight is zero (integer coordinates: IEEE 0 x NaN = NaN). Pinned twice:
+    (i) against a hand-counted neighbourhood written as index logic only, on a lattice that contains
+    every integer and quarter-integer coordinate; (ii) mask and finite values against torch-CPU
+    float64 grid_sample(bicubic, border, align_corners=True) at generic coordinates (torch
+    un-normalises the grid, which may move an exact integer by an ulp, so integers are left to (i))."""
+    rng = np.random.default_rng(14)
+    ny, nx = 12, 14
+    img = rng.normal(100.0, 20.0, (ny, nx)).astype(np.float32)      # the oracle reads float32 images (G14)
+    holes = [(5, 6), (0, 0), (11, 9), (7, 13)]                 # interior, corner, bottom edge, right edge
+    for r, c in holes:
+        img[r, c] = np.nan
+    # (i) hand count
+    xs = np.arange(-2, 4 * nx - 2 + 1) / 4.0                     # -0.5 .. nx - 0.5 in quarter steps
+    ys = np.arange(-2, 4 * ny - 2 + 1) / 4.0
+    xs, ys = xs[xs < nx - 0.5], ys[ys < ny - 0.5]
+    X, Y = np.meshgrid(xs, ys)
+    got = oracle.interp(img, X.ravel(), Y.ravel(), 3).reshape(X.shape)
+    want = np.zeros(X.shape, dtype=bool)
+    for j, y in enumerate(ys):
+        rows = {min(max(int(math.floor(y)) + d, 0), ny - 1) for d in (-1, 0, 1, 2)}
+        for i, x in enumerate(xs):
+            cols = {min(max(int(math.floor(x)) + d, 0), nx - 1) for d in (-1, 0, 1, 2)}
+            want[j, i] = any(r in rows and c in cols for r, c in holes)
+    assert np.array_equal(np.isnan(got), want)
+    # an interior hole is reached from exactly 4 x 4 unit cells: 16 quarter-lattice points each
+    near = (X >= 4) & (X < 8) & (Y >= 3) & (Y < 7)               # cells whose taps include (5, 6)
+    assert want[near].all() and int(near.sum()) == 16 * 16
+    ring = (X >= 3) & (X < 9) & (Y >= 2) & (Y < 8) & ~near
+    assert not want[ring].any()
+    # at integer coordinates the taps at -1 and +2 have weight zero and still count
+    k = np.argmin(np.abs(xs - 4.0)), np.argmin(np.abs(ys - 4.0))
+    assert xs[k[0]] == 4.0 and ys[k[1]] == 4.0 and np.isnan(got[k[1], k[0]])      # (5, 6) is tap (+2, +1): weight 0 along x
+    # (ii) torch float64 grid_sample at generic coordinates
+    x = rng.uniform(-0.5, nx - 0.5 - 1e-9, 6000)
+    y = rng.uniform(-0.5, ny - 0.5 - 1e-9, 6000)
+    keep = (np.abs(x - np.rint(x)) > 1e-6) & (np.abs(y - np.rint(y)) > 1e-6)
+    x, y = x[keep], y[keep]
+    got = oracle.interp(img, x, y, 3)
+    grid = torch.from_numpy(np.stack([2.0 * x / (nx - 1) - 1.0, 2.0 * y / (ny - 1) - 1.0], axis=-1)).reshape(1, 1, -1, 2)
+    ref = torch.nn.functional.grid_sample(torch.from_numpy(img.astype(np.float64)).reshape(1, 1, ny, nx), grid, mode="bicubic",
+                                          padding_mode="border", align_corners=True).reshape(-1).numpy()
+    assert np.array_equal(np.isnan(got), np.isnan(ref))
+    ok = ~np.isnan(ref)
+    assert 0.2 < ok.mean() < 0.95
+    assert np.max(np.abs(got[ok] - ref[ok])) < 1e-10
