@@ -56,8 +56,8 @@ extern "C" {
  *   u + A(u, v) = U,  v + B(u, v) = V
  * for (u, v) in fp64 by fixed-point iteration to 1e-11 px (at most 32 steps: distortions whose
  * gradient exceeds ~0.4 do not converge and give NaN). Exact where a fitted AP/BP is only as good
- * as its order allows. On the tiled path the solve runs at the 25 sample points of a tile, not
- * per pixel. */
+ * as its order allows. On the tiled path the solve runs at the sample points of the per-tile fit
+ * (16 nodes + 16 check points per 128 x 128 output pixels, or 25 per tile), not per pixel. */
 #define DFR_SIP_INVERSE_EXACT (-1)
 
 /* Packed WCS parameter set. POD, no pointers,
@@ -92,8 +92,9 @@ typedef enum dfr_status {
 } dfr_status;
 
 /* Path selection for dfr_reproject_ex / dfr_src_coords_ex.
- *   AUTO  : tiled fast path where its per-tile fit passes a 9-point spot check, exact
- *           per-pixel path elsewhere (what dfr_reproject uses).
+ *   AUTO  : tiled fast path where its per-tile cubic fit passes a spot check against the exact
+ *           map (16 check points per 128 x 128 output pixels; 9 per tile on the refit level),
+ *           exact per-pixel path elsewhere (what dfr_reproject uses).
  *   EXACT : every pixel through the per-pixel fp64 map, direct gathers.
  *   TILED : as AUTO (kept distinct so tests can assert the fast path ran). */
 enum { DFR_PATH_AUTO = 0, DFR_PATH_EXACT = 1, DFR_PATH_TILED = 2 };
@@ -306,7 +307,11 @@ int dfr_wcs_fit_inverse_sip(dfr_wcs *w, int32_t order, int32_t nx, int32_t ny, d
 
 /* Counters of the last dfr_reproject* call on this thread (HOST):
  * stats[0] = tiles on the fast path, [1] = tiles on the exact path,
- * [2] = tiles entirely outside the footprint, [3] = kernels launched. */
+ * [2] = tiles entirely outside the footprint, [3] = kernels launched.
+ * The counters and the event that guards them exist once per (host thread, device), not per
+ * stream: they describe the last call only if this thread's calls on that device were issued on
+ * ONE stream. With calls in flight on several streams an earlier call may finish later and
+ * overwrite them. The same holds for dfr_profile_last. Outputs are never affected. */
 int dfr_last_stats(int64_t stats[4]);
 
 /* Timing hooks used by bench.py: when enabled (per host thread), dfr_reproject*

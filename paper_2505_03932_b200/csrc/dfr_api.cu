@@ -74,6 +74,10 @@ static cudaError_t stream_stats_begin(DevCtx *c)
     cudaError_t err;
     if (!c->stream_totals && (err = cudaMalloc((void **)&c->stream_totals, 4 * sizeof(int32_t))) != cudaSuccess) return err;
     if ((err = cudaMemset(c->stream_totals, 0, 4 * sizeof(int32_t))) != cudaSuccess) return err;
+    // A device memset returns before it has run, and the pipeline's streams are non-blocking (nothing
+    // orders them after the legacy stream): wait here, once per streaming call, so the setup kernels'
+    // atomicAdd into stream_totals cannot land before the zeros do.
+    if ((err = cudaStreamSynchronize(nullptr)) != cudaSuccess) return err;
     for (int k = 0; k < 4; ++k) g_stats_acc[k] = 0;
     g_last.pending = false;
     g_accumulate = true;
@@ -93,8 +97,8 @@ static void stream_stats_end(DevCtx *c)
 // ---- per-call constants -------------------------------------------------------------------
 // Host constants -> one stream-ordered device block [SourceDev x n | float weights x n], staged
 // through the thread's pinned ring (dfr_context.h) so the upload never blocks the host. `hsrc`
-// stays valid until kRingSlots - 1 further calls on this thread and device: long enough for the
-// launchers, which read it for the staging decision only.
+// points into a thread-local host array that the NEXT call on this thread overwrites: valid for the
+// launchers of this call, which read it for the staging decision only.
 struct CallConsts {
     TargetDev tgt;
     const SourceDev *hsrc = nullptr;

@@ -1,15 +1,24 @@
 // dfr_tiled_setup.cu — setup kernels of the tiled fast path and the host
 // side they share with the main kernels (scratch, staging decision, tensor map).
 //
-//   target_nodes_kernel   (fp64) a1-a2 at 25 sample points per 64x64 CTA tile — shared by
-//                         the whole batch, as SURVEY.md §8(a) a10 notes.
-//   tile_setup_kernel     (fp64) a3-a6 at those points per (exposure, CTA tile); fits the
-//                         cubic through 16 Chebyshev nodes, checks it against the exact
-//                         map at 9 other points, re-centres it on the four 32x32 tiles
-//                         (or refits each tile when the 64x64 fit fails), bounds each
-//                         tile's source footprint rigorously, classifies it FAST / EXACT /
-//                         EMPTY, picks the dj degree the main kernel must keep, and
-//                         reduces the origin of the CTA tile's staged box.
+//   target_nodes_kernel      (fp64) a1-a2 at the sample points — shared by the whole batch, as
+//                            SURVEY.md §8(a) a10 notes: 16 nodes + 16 check points per 128x128
+//                            super-tile for the cooperative kernel, 25 points per 64x64 CTA tile
+//                            for the wide one.
+//   tile_setup_kernel        (fp64, the default) cooperative: 16 lanes per 128x128 super-tile, one
+//                            node, one check point and one 32x32 tile each. a3-a6 at the 16
+//                            Chebyshev nodes, bicubic fit through shuffles, compared with the exact
+//                            map at 16 other points (centre, T4 extrema on the axes, corners, edge
+//                            mid-points, three generic points); if accepted, every lane re-centres
+//                            the cubic on its own tile; if not, every lane fits its own tile from
+//                            25 points (16 nodes + 9 check points), and a tile whose own fit fails
+//                            is classified EXACT.
+//   tile_setup_wide_kernel   (fp64) the round-1 form, a thread per 64x64 CTA tile (25 points: 16
+//                            nodes + 9 check points, refit per 32x32 tile when the 64x64 fit
+//                            fails); chosen by run_setup when the launch fills the GPU anyway.
+//   Both then bound each tile's source footprint rigorously, classify it FAST / EXACT / EMPTY,
+//   pick the dj degree the main kernel must keep, and reduce the origin of the CTA tile's
+//   staged box.
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
@@ -626,16 +635,16 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
 
 static EncodeTiledFn get_encode()
 {
-    static EncodeTiledFn fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
+    // function-local static initialiser: run once, and every thread that gets here meanwhile waits for
+    // it (the *_multi entry points start several worker threads that all reach this on first use)
+    static const EncodeTiledFn fn = []() -> EncodeTiledFn {
         void *p = nullptr;
         cudaDriverEntryPointQueryResult q;
         if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
             q == cudaDriverEntryPointSuccess)
-            fn = (EncodeTiledFn)p;
-    }
+            return (EncodeTiledFn)p;
+        return nullptr;
+    }();
     return fn;
 }
 

@@ -1,7 +1,9 @@
 // dfr_tiled_stack.cu — fused reproject-and-stack (dfr_reproject_stack).
 #include <algorithm>
 #include <cmath>
+#include <atomic>
 #include <cstring>
+#include <mutex>
 
 #include "dfr_tiled_device.cuh"
 
@@ -338,17 +340,42 @@ static cudaError_t launch_stack(TiledParams P, const TargetDev &tgt, const CUten
     P.rec_off = 0;
     const size_t smem = (size_t)kStackWarps * P.stage_bytes;
     P.e0 = 0;
-    cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    // Per (kernel, device), once: the shared-memory opt-in to the constant maximum (never to this call's
+    // own size — the attribute is per function and device, so two host threads stacking on one device
+    // with different box sizes would otherwise lower each other's limit between set and launch) and the
+    // resource figures the resident-CTA estimate below needs (no runtime queries on later calls).
+    struct DevInfo {
+        std::atomic<int> ready{0};
+        int sms = 0, smem_sm = 0, regs_sm = 0, static_smem = 0, regs = 0;
+    };
+    constexpr int kDevs = 64;
+    constexpr size_t kMaxSmem = (size_t)kStackWarps * ((kStackMaxBoxBytes + 127) & ~(size_t)127);
+    static DevInfo info[kDevs];
+    static std::mutex info_mu;
+    if (smem > kMaxSmem) return cudaErrorInvalidValue;
+    int dev = 0;
+    cudaError_t err = cudaGetDevice(&dev);
     if (err != cudaSuccess) return err;
+    DevInfo uncached;                                    // device ordinals beyond the table: queried every call
+    DevInfo *I = (dev >= 0 && dev < kDevs) ? &info[dev] : &uncached;
+    if (!I->ready.load(std::memory_order_acquire)) {
+        std::lock_guard<std::mutex> lock(info_mu);
+        if (!I->ready.load(std::memory_order_relaxed)) {
+            cudaFuncAttributes fa;
+            err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
+            if (err == cudaSuccess) err = cudaDeviceGetAttribute(&I->sms, cudaDevAttrMultiProcessorCount, dev);
+            if (err == cudaSuccess) err = cudaFuncGetAttributes(&fa, kern);
+            if (err == cudaSuccess) err = cudaDeviceGetAttribute(&I->smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
+            if (err == cudaSuccess) err = cudaDeviceGetAttribute(&I->regs_sm, cudaDevAttrMaxRegistersPerMultiprocessor, dev);
+            if (err != cudaSuccess) return err;
+            I->static_smem = (int)fa.sharedSizeBytes;
+            I->regs = fa.numRegs;
+            I->ready.store(1, std::memory_order_release);
+        }
+    }
     // resident CTAs per SM from the kernel's own resources: shared memory, registers, TMEM columns
-    int dev = 0, sms = 0, smem_sm = 0, regs_sm = 0;
-    cudaFuncAttributes fa;
-    err = cudaGetDevice(&dev);
-    if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (err == cudaSuccess) err = cudaFuncGetAttributes(&fa, kern);
-    if (err == cudaSuccess) err = cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
-    if (err == cudaSuccess) err = cudaDeviceGetAttribute(&regs_sm, cudaDevAttrMaxRegistersPerMultiprocessor, dev);
-    if (err != cudaSuccess) return err;
+    const int sms = I->sms, smem_sm = I->smem_sm, regs_sm = I->regs_sm;
+    struct { size_t sharedSizeBytes; int numRegs; } fa = {(size_t)I->static_smem, I->regs};
     int per_sm = std::min(512 / kStackCols, 32);
     per_sm = (int)std::min<long long>(per_sm, smem_sm / (long long)(smem + fa.sharedSizeBytes + 1024));
     per_sm = std::max(1, std::min(per_sm, regs_sm / std::max(1, ((fa.numRegs + 7) & ~7) * kStackThreads)));

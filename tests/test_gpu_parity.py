@@ -644,8 +644,9 @@ def test_nearest_ties_round_half_even_on_both_paths(P):
 
 
 def test_fit_acceptance_adversarial_sweep(P):
-    """The tiled path accepts a tile's cubic fit after comparing it with the exact map at 9 check
-    points (FIT_TOL = 2e-6 px): a spot check, not a bound. This seeded sweep searches for a
+    """The tiled path accepts a cubic fit after comparing it with the exact map at check points
+    (16 per 128x128 super-tile, 9 per 32x32 tile on the refit level; FIT_TOL = 2e-6 px): a spot
+    check, not a bound. This seeded sweep searches for a
     geometry where an ACCEPTED tile is wrong anyway: SIP orders 2-9 on either side with
     amplitudes 1e-6 ... 1e-2 (up to tens of pixels of distortion), scale ratios 0.5-2, any
     rotation, tangent points up to degrees apart, declinations up to the poles. Everywhere
