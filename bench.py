@@ -260,7 +260,7 @@ def run_stack(args):
                          "setup_kernels_ms": statistics.mean(m[0] for m in ms), "algorithmic_bytes_per_launch": alg,
                          "note": "issue-bound, not HBM-bound: see DESIGN.md §6.5"},
             "cpu_baseline": None, "e2e": None, "gpu_launches": int(stats["kernels"]) * args.steps,
-            "clocks": sampler.summary()}
+            "clocks": clocks}
     print(json.dumps(line))
     return 0
 
@@ -369,6 +369,20 @@ def main():
     # ---- burst figure: K steps right after the warm-up, GPU otherwise idle (boost clocks)
     burst_ms, burst_steps = timed(args.steps)
     burst_ms = max_over_ranks(burst_ms, device="cuda")
+    # the dominant kernel in the same regime: single profiled steps with the GPU idle in between
+    kern_burst = None
+    if path == P.PATH_AUTO:
+        ms = []
+        for _ in range(min(args.steps, 10)):
+            torch.cuda.synchronize()
+            time.sleep(0.02)                         # idle gap: every short series starts from boost clocks
+            for _ in range(5):
+                step()
+            P.dfr_profile_enable(True)
+            step()
+            ms.append(P.dfr_profile_last())
+            P.dfr_profile_enable(False)
+        kern_burst = {"setup_ms": statistics.mean(m[0] for m in ms), "main_ms": statistics.mean(m[1] for m in ms)}
     # ---- the timed region proper: K steps inside a sustained run of the same steps, CUDA events
     # on the launching (current) stream; clocks and throttle reasons sampled during it
     sampler = ClockSampler(local)
@@ -436,14 +450,35 @@ def main():
     dom_ms = kern_ms["main_ms"] if kern_ms else statistics.median(per_step)
     achieved = alg_bytes / (dom_ms * 1e-3) / 1e9
     traffic, traffic_src = ncu_traffic("tiled_reproject_kernel<1,1,0>") if kern_ms else (None, None)
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s",
+    # `bound`: which of the two explains how the kernel's duration changes between the regimes. Limited
+    # by the SM clock domain (issue slots / FMA pipe), its duration scales with 1 / SM clock: kernel_ms x
+    # sm_mhz is the same in the sustained leg (median clock sampled under load) and the burst leg (short
+    # series from an idle GPU: taken at sm_max_mhz), ratio 1. Limited by HBM, the duration is the same in
+    # both and the ratio is sm_mhz / sm_max_mhz. The nearer hypothesis is reported; with no clock
+    # difference (< 3 %) the two cannot be told apart and the label stays "hbm", the stricter peak.
+    clocks = sampler.summary()
+    bound, bound_rule = "hbm", None
+    if kern_burst and clocks and clocks.get("sm_mhz") and clocks.get("sm_max_mhz"):
+        r_clk = clocks["sm_mhz"] / clocks["sm_max_mhz"]
+        r_cyc = (dom_ms * clocks["sm_mhz"]) / (kern_burst["main_ms"] * clocks["sm_max_mhz"])
+        if r_clk < 0.97:
+            bound = "sm" if abs(r_cyc - 1.0) < abs(r_cyc - r_clk) else "hbm"
+        bound_rule = (f"(kernel_ms x sm_mhz) sustained / burst = {r_cyc:.3f}; 1.000 if the duration follows the SM "
+                      f"clock ('sm'), {r_clk:.3f} = sm_mhz / sm_max_mhz if it does not ('hbm'); nearer one reported")
+    roofline = {"bound": bound, "bound_rule": bound_rule, "achieved": achieved, "peak": hbm, "unit": "GB/s",
                 "frac": achieved / hbm, "frac_upper": upper_bytes / (dom_ms * 1e-3) / 1e9 / hbm,
                 "frac_whole_call": alg_bytes / (statistics.median(per_step) * 1e-3) / 1e9 / hbm,
                 "traffic": traffic, "traffic_source": traffic_src, "peak_source": which,
                 "kernel": "tiled_reproject_kernel<1,1,0>" if kern_ms else "whole dfr_reproject call",
                 "kernel_ms": dom_ms, "setup_kernels_ms": kern_ms["setup_ms"] if kern_ms else None,
                 "algorithmic_bytes_per_launch": alg_bytes, "source_pixels_touched": touched,
-                "upper_bound_bytes_per_launch": upper_bytes}
+                "upper_bound_bytes_per_launch": upper_bytes,
+                # the same K steps / the same kernel right after the warm-up on an idle GPU (boost clocks)
+                "kernel_ms_burst": kern_burst["main_ms"] if kern_burst else None,
+                "setup_kernels_ms_burst": kern_burst["setup_ms"] if kern_burst else None,
+                "frac_burst": alg_bytes / (kern_burst["main_ms"] * 1e-3) / 1e9 / hbm if kern_burst else None,
+                "ms_per_step_burst": burst_ms / args.steps,
+                "value_burst": out_mpix * world * args.steps / (burst_ms * 1e-3)}
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -477,7 +512,7 @@ def main():
                               "`value` is measured inside a sustained run, where the power cap lowers the SM clock"},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
             "gpu_launches": int(stats["kernels"]) * args.steps,
-            "clocks": sampler.summary()}
+            "clocks": clocks}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

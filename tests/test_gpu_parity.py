@@ -168,16 +168,21 @@ def test_sip_order_9(P):
 
 def test_config2_batch_full_size(P):
     """configs[2] at full size in the launch configuration bench.py times (batch 32 in one
-    call): ALL 32 exposures element by element (mask + values, tests/parity.py), plus 40 000
+    call): ALL 32 exposures element by element (coordinates of the tiled path, mask, values;
+    tests/parity.py), plus 40 000
     sampled pixels computed one by one through the oracle's sky entry points
     (pix2world -> world2pix -> interp: a second route through the oracle)."""
     w = S.config2()
     out = run_gpu(P, w, 1, 0)
     st = P.dfr_last_stats()
     sny, snx = w.images.shape[1:]
-    fr, worst = [], 0.0
+    fr, worst, worst_c = [], 0.0, 0.0
     for e in range(32):
+        if e % 4 == 0:       # the kernels' own coordinates (PAPER.md:101-121), 4 exposures x 2 x 33.5 MB at a time
+            xg, yg = P.dfr_src_coords(w.src_wcs[e:e + 4], w.tgt_wcs, (sny, snx), w.shape_out, 1, path=0)
+            xg, yg = xg.cpu().numpy(), yg.cpu().numpy()
         xo, yo = oracle.src_coords(w.tgt_wcs, w.src_wcs[e], *w.shape_out)
+        worst_c = max(worst_c, PR.check_coords(xg[e % 4], yg[e % 4], xo, yo, w.src_wcs[e])["max"])
         ref = oracle.interp(w.images[e], xo.ravel(), yo.ravel(), 1).reshape(w.shape_out).astype(np.float32)
         r = PR.check_image(out[e], ref, xo, yo, w.images[e], 1)
         fr.append(r["nan_frac"])
@@ -195,7 +200,7 @@ def test_config2_batch_full_size(P):
         assert np.array_equal(np.isnan(got)[~band], np.isnan(ref)[~band])
         ok = ~np.isnan(got) & ~np.isnan(ref)
         assert np.max(np.abs(got[ok] - ref[ok])) <= PR.VALUE_TOL * PR.dyn_range(w.images[e])
-    print("C2 stats", st, "worst value error", worst, "x DR, mean NaN fraction", np.mean(fr))
+    print("C2 stats", st, "worst value error", worst, "x DR, worst coordinate error", worst_c, "px, mean NaN fraction", np.mean(fr))
 
 
 def test_config3_three_orders(P):
@@ -213,13 +218,17 @@ def test_config4_stream_sample(P):
     src = torch.from_numpy(w.images).pin_memory()
     out = P.dfr_reproject_host(src, w.src_wcs, w.tgt_wcs, w.shape_out, 1, batch=2)
     out = out.numpy()
-    inside = []
+    inside, worst_c = [], 0.0
     for t in range(len(idx)):
         xo, yo = oracle.src_coords(w.tgt_wcs, w.src_wcs[t], *w.shape_out)
+        xg, yg = P.dfr_src_coords([w.src_wcs[t]], w.tgt_wcs, w.images.shape[1:], w.shape_out, 1, path=0)
+        worst_c = max(worst_c, PR.check_coords(xg[0].cpu().numpy(), yg[0].cpu().numpy(), xo, yo, w.src_wcs[t])["max"])
+        del xg, yg
         ref = oracle.interp(w.images[t], xo.ravel(), yo.ravel(), 1).reshape(w.shape_out).astype(np.float32)
         r = PR.check_image(out[t], ref, xo, yo, w.images[t], 1)
         inside.append(1 - r["nan_frac"])
     assert abs(np.mean(inside) - 0.25) < 0.01
+    print("C4 worst coordinate error", worst_c, "px")
     # same result from the device-buffer entry point
     dev = P.dfr_reproject(torch.from_numpy(w.images[:2]).cuda(), w.src_wcs[:2], w.tgt_wcs, w.shape_out, 1)
     assert np.array_equal(np.nan_to_num(dev.cpu().numpy(), nan=-1), np.nan_to_num(out[:2], nan=-1))
