@@ -70,23 +70,26 @@ def ncu_traffic(kernel):
     return float(d["dram_bytes_read"]) + float(d["dram_bytes_write"]), d.get("summary")
 
 
-def source_pixels_touched(P, torch, src_wcs, tgt, src_shape, shape_out, chunk=4):
-    """Unique source pixels the bilinear taps of one step read (algorithmic
-    bytes = 4 B per output pixel + 4 B per unique source pixel touched), counted on the device
-    from the coordinates the kernels themselves use (dfr_src_coords), outside any timed region."""
+def source_pixels_touched(P, torch, src_wcs, tgt, src_shape, shape_out, chunk=4, order=1):
+    """Unique source pixels the taps of one step read (algorithmic bytes = 4 B
+    per output pixel + 4 B per unique source pixel touched), counted on the device from the
+    coordinates the kernels themselves use (dfr_src_coords), outside any timed region. Taps:
+    nearest the rounded pixel, bilinear floor + {0, 1}, bicubic floor + {-1 .. 2}, edge-replicated."""
     sny, snx = src_shape
     n = len(src_wcs)
     total = 0
+    taps = {0: (0,), 1: (0, 1), 3: (-1, 0, 1, 2)}[order]
     for e0 in range(0, n, chunk):
         ws = src_wcs[e0:e0 + chunk]
-        x, y = P.dfr_src_coords(ws, tgt, src_shape, shape_out, P.BILINEAR)
+        x, y = P.dfr_src_coords(ws, tgt, src_shape, shape_out, order)
         for k in range(len(ws)):
             xe, ye = x[k].reshape(-1), y[k].reshape(-1)
             ok = (xe >= -0.5) & (xe < snx - 0.5) & (ye >= -0.5) & (ye < sny - 0.5)
-            ix, iy = torch.floor(xe[ok]).long(), torch.floor(ye[ok]).long()
+            rnd = torch.round if order == 0 else torch.floor          # torch.round: half to even, as the kernels
+            ix, iy = rnd(xe[ok]).long(), rnd(ye[ok]).long()
             mask = torch.zeros(sny * snx, dtype=torch.bool, device=x.device)
-            for dy in (0, 1):
-                for dx in (0, 1):
+            for dy in taps:
+                for dx in taps:
                     mask[(iy + dy).clamp(0, sny - 1) * snx + (ix + dx).clamp(0, snx - 1)] = True
             total += int(mask.sum().item())
         del x, y
@@ -149,14 +152,14 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def time_oracle(w, n_exp, passes=1):
+def time_oracle(w, n_exp, passes=1, order=1):
     """The oracle as it stands on all host cores: `passes` passes over the first n_exp
     exposures, full frames. Returns (Mpix/s over all passes, wall seconds, threads used)."""
     import oracle
     oracle.build()
     t0 = time.perf_counter()
     for _ in range(passes):
-        oracle.reproject(w.images[:n_exp], w.src_wcs[:n_exp], w.tgt_wcs, w.shape_out, 1)
+        oracle.reproject(w.images[:n_exp], w.src_wcs[:n_exp], w.tgt_wcs, w.shape_out, order)
     dt = time.perf_counter() - t0
     mpix = passes * n_exp * w.shape_out[0] * w.shape_out[1] / 1e6
     return mpix / dt, dt, oracle.max_threads()
@@ -260,7 +263,222 @@ def run_stack(args):
                          "setup_kernels_ms": statistics.mean(m[0] for m in ms), "algorithmic_bytes_per_launch": alg,
                          "note": "issue-bound, not HBM-bound: see DESIGN.md §6.5"},
             "cpu_baseline": None, "e2e": None, "gpu_launches": int(stats["kernels"]) * args.steps,
-            "clocks": clocks}
+            "clocks": sampler.summary()}
+    print(json.dumps(line))
+    return 0
+
+
+ORDERS = {"nearest": 0, "bilinear": 1, "bicubic": 3}
+FLUSH_FLOATS = 128 * 1024 * 1024           # 512 MB > 126 MB L2, overwritten between timed steps
+
+
+def run_config(args):
+    """--config {0,1,3,4} [--order ...]: the other BASELINE.json configs through the same contract
+    line (roofline, cpu_baseline, e2e, clocks). Single frames (C0, C1, C3) fit the L2, so a 512 MB
+    buffer is overwritten between steps, outside the events that time them; every step is timed by
+    its own event pair on the launching stream and `ms_per_step` is their mean. configs[4] is the
+    stream of 1024 exposures onto a 4096^2 mosaic: `value` with the inputs resident in HBM (batches
+    of 32 per call), `e2e` through dfr_reproject_host from pinned host memory."""
+    import torch
+    import paper_2505_03932_b200 as P
+    P.lib()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    order = ORDERS[args.order]
+    cfg = args.config
+    hbm, which, _ = peaks()
+    flush = torch.empty(FLUSH_FLOATS, dtype=torch.float32, device="cuda")
+    if cfg == 4:
+        return run_config4(args, torch, P, order, hbm, which)
+    w = {0: S.config0, 1: S.config1, 3: S.config3}[cfg]()
+    if args.src_nx:                            # a source width that is not a multiple of 4: the non-staged path
+        keep = int(args.src_nx)
+        w = S.Workload(w.name, np.ascontiguousarray(w.images[:, :, :keep]), w.src_wcs, w.tgt_wcs, w.shape_out, w.orders)
+    n, (sny, snx), (ony, onx) = len(w.src_wcs), w.images.shape[1:], w.shape_out
+    src = torch.from_numpy(w.images).cuda()
+    out = torch.empty((n, ony, onx), dtype=torch.float32, device="cuda")
+    ws_arr, tw = P.pack_wcs_array(w.src_wcs), P.pack_wcs(w.tgt_wcs)
+    out_mpix = n * ony * onx / 1e6
+
+    def step():
+        P.dfr_reproject(src, ws_arr, tw, (ony, onx), order, out=out)
+
+    def flushed_steps(k, profile=False):
+        ms, kern = [], []
+        for _ in range(k):
+            flush.fill_(1.0)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            step()
+            b.record()
+            if profile:
+                kern.append(P.dfr_profile_last())
+            b.synchronize()
+            ms.append(a.elapsed_time(b))
+        return ms, kern
+
+    flushed_steps(args.warmup)
+    stats = P.dfr_last_stats()
+    sampler = ClockSampler(0)
+    sampler.start()
+    t_end = time.perf_counter() + args.load_seconds
+    while time.perf_counter() < t_end:
+        flushed_steps(20)
+    per_step, _ = flushed_steps(args.steps)
+    P.dfr_profile_enable(True)
+    _, kern = flushed_steps(min(args.steps, 10), profile=True)
+    P.dfr_profile_enable(False)
+    t_end = time.perf_counter() + 0.5 * args.load_seconds
+    while time.perf_counter() < t_end:
+        flushed_steps(20)
+    sampler.stop()
+    ms_step = statistics.mean(per_step)
+    tiled = stats["tiles_exact"] != -1
+    main_ms = statistics.mean(m[1] for m in kern) if tiled else ms_step
+    setup_ms = statistics.mean(m[0] for m in kern) if tiled else None
+    touched = source_pixels_touched(P, torch, w.src_wcs, w.tgt_wcs, (sny, snx), (ony, onx), order=order)
+    alg = 4.0 * n * ony * onx + 4.0 * touched
+    staged = 1 if (snx % 4 == 0) else 0
+    kname = f"tiled_reproject_kernel<{order},{staged},0>" if tiled else "exact_reproject_kernel"
+    traffic, traffic_src = ncu_traffic(kname)
+    roofline = {"bound": "hbm", "achieved": alg / (main_ms * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
+                "frac": alg / (main_ms * 1e-3) / 1e9 / hbm, "frac_whole_call": alg / (ms_step * 1e-3) / 1e9 / hbm,
+                "traffic": traffic, "traffic_source": traffic_src, "peak_source": which, "kernel": kname,
+                "kernel_ms": main_ms, "setup_kernels_ms": setup_ms, "algorithmic_bytes_per_launch": alg,
+                "source_pixels_touched": touched,
+                "note": "single frames: launch latency and the per-tile fit, not HBM, set the step time (DESIGN.md §8)"}
+    cpu = None
+    if not args.no_cpu_baseline:
+        v1, dt1, cores = time_oracle(w, n, 1, order)
+        passes = int(min(20, max(1, round(10.0 / max(dt1, 1e-3)))))
+        v, dt, cores = time_oracle(w, n, passes, order)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"the whole frame, {passes} pass(es) after one sizing pass ({dt:.1f} s wall)"}
+    e2e = None
+    if args.e2e_steps > 0:
+        hsrc = torch.from_numpy(w.images).pin_memory()
+        hout = torch.empty((n, ony, onx), dtype=torch.float32).pin_memory()
+        P.dfr_reproject_host(hsrc, ws_arr, tw, (ony, onx), order, out_host=hout)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            P.dfr_reproject_host(hsrc, ws_arr, tw, (ony, onx), order, out_host=hout)
+        el = time.perf_counter() - t0
+        a, b = hout, out.cpu()
+        both = ~torch.isnan(a) & ~torch.isnan(b)
+        dr = float(w.images.max() - w.images.min())
+        e2e = {"value": out_mpix * args.e2e_steps / el, "unit": UNIT, "h2d_bytes_per_step": int(w.images.nbytes),
+               "d2h_bytes_per_step": int(hout.numel() * 4), "steps": args.e2e_steps,
+               "api": "dfr_reproject_host, pinned host buffers",
+               "max_diff_vs_device_path_dr": float((a[both] - b[both]).abs().max()) / dr,
+               "mask_diff_vs_device_path": int((torch.isnan(a) != torch.isnan(b)).sum())}
+    line = {"metric": f"output Mpix/s reprojected (configs[{cfg}], {args.order})", "value": out_mpix / (ms_step * 1e-3),
+            "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"configs[{cfg}]: {n} x {sny}x{snx} -> {ony}x{onx}, {args.order}",
+                       "l2": "a 512 MB buffer is overwritten between timed steps (outside the events)",
+                       "nan_fraction": float(torch.isnan(out).float().mean().item()), "tiles": stats},
+            "ms_per_step_median": statistics.median(per_step), "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+            "gpu_launches": int(stats["kernels"]) * args.steps, "clocks": sampler.summary()}
+    print(json.dumps(line))
+    return 0
+
+
+def run_config4(args, torch, P, order, hbm, which):
+    """configs[4]: 1024 exposures (2048^2 each, own WCS, seeds [4, k]) onto a 4096^2 mosaic, 32 per call.
+    `--c4-images M` distinct images are generated (M = 1024: all of them; the default 128 bounds the
+    generation time, the WCSs are all distinct either way and exposure k reads image k mod M)."""
+    from concurrent.futures import ThreadPoolExecutor
+    n_exp, batch = args.c4_exposures, 32
+    m_img = max(batch, min(args.c4_images, n_exp) // batch * batch)        # a multiple of the batch
+    t0 = time.perf_counter()
+    tgt = S.config4_target()
+    hin = torch.empty((max(m_img, batch), NPIX, NPIX), dtype=torch.float32).pin_memory()
+    hin_np = hin.numpy()
+    wcs = [None] * n_exp
+
+    def produce(k):                                           # producer threads fill the pinned ring
+        img, wk = S.jittered_exposure([4, k], with_image=k < m_img, fast_image=True)
+        if k < m_img:
+            hin_np[k] = img
+        wcs[k] = wk
+
+    with ThreadPoolExecutor(max_workers=min(16, os.cpu_count() or 1)) as ex:
+        list(ex.map(produce, range(n_exp)))
+    gen_s = time.perf_counter() - t0
+    ony = onx = 4096
+    ws_all, tw = P.pack_wcs_array(wcs), P.pack_wcs(tgt)
+    ws_b = [P.pack_wcs_array(wcs[b0:b0 + batch]) for b0 in range(0, n_exp, batch)]
+    dsrc = hin.cuda()                                         # the M distinct images, resident in HBM
+    dout = torch.empty((batch, ony, onx), dtype=torch.float32, device="cuda")
+    out_mpix = n_exp * ony * onx / 1e6
+
+    def step():                                               # one pass over the whole stream
+        for b, b0 in enumerate(range(0, n_exp, batch)):
+            i0, nb = b0 % m_img, len(ws_b[b])
+            P.dfr_reproject(dsrc[i0:i0 + nb], ws_b[b], tw, (ony, onx), order, out=dout[:nb])
+
+    for _ in range(max(1, min(args.warmup, 3))):
+        step()
+    torch.cuda.synchronize()
+    stats = P.dfr_last_stats()
+    sampler = ClockSampler(0)
+    sampler.start()
+    steps = max(1, min(args.steps, 5))
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    ev[0].record()
+    for k in range(steps):
+        step()
+        ev[k + 1].record()
+    torch.cuda.synchronize()
+    total_ms = ev[0].elapsed_time(ev[-1])
+    P.dfr_profile_enable(True)
+    kern = []
+    for b in range(4):
+        P.dfr_reproject(dsrc[:batch], ws_b[b], tw, (ony, onx), order, out=dout)
+        kern.append(P.dfr_profile_last())
+    P.dfr_profile_enable(False)
+    sampler.stop()
+    main_ms = statistics.mean(m[1] for m in kern)
+    touched = source_pixels_touched(P, torch, wcs[:batch], tgt, (NPIX, NPIX), (ony, onx), order=order)
+    alg = 4.0 * batch * ony * onx + 4.0 * touched
+    roofline = {"bound": "hbm", "achieved": alg / (main_ms * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
+                "frac": alg / (main_ms * 1e-3) / 1e9 / hbm, "traffic": None, "traffic_source": "no ncu capture for this shape",
+                "peak_source": which, "kernel": f"tiled_reproject_kernel<{order},1,0>", "kernel_ms": main_ms,
+                "setup_kernels_ms": statistics.mean(m[0] for m in kern), "algorithmic_bytes_per_launch": alg,
+                "source_pixels_touched": touched,
+                "note": "per launch = one batch of 32 exposures (the first 32 of the stream); 3/4 of every output frame is "
+                        "outside the exposure's footprint and costs its NaN stores only"}
+    cpu = None
+    if not args.no_cpu_baseline:
+        w1 = S.Workload("c4-1", hin_np[:1], wcs[:1], tgt, (ony, onx), (order,))
+        v, dt, cores = time_oracle(w1, 1, 1, order)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"exposure 0 of the stream onto the whole 4096x4096 mosaic, one pass ({dt:.1f} s wall)"}
+    e2e = None
+    if args.e2e_steps > 0:
+        hout = torch.empty((batch, ony, onx), dtype=torch.float32).pin_memory()
+        P.dfr_reproject_host(hin[:batch], ws_b[0], tw, (ony, onx), order, out_host=hout, batch=8)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for b, b0 in enumerate(range(0, n_exp, batch)):
+            i0, nb = b0 % m_img, len(ws_b[b])
+            P.dfr_reproject_host(hin[i0:i0 + nb], ws_b[b], tw, (ony, onx), order, out_host=hout[:nb], batch=8)
+        el = time.perf_counter() - t0
+        e2e = {"value": out_mpix / el, "unit": UNIT, "h2d_bytes_per_step": int(n_exp * NPIX * NPIX * 4),
+               "d2h_bytes_per_step": int(n_exp * ony * onx * 4), "steps": 1, "exposures_per_s": n_exp / el,
+               "api": "dfr_reproject_host(batch=8), 32 exposures per call, pinned host buffers"}
+    line = {"metric": f"output Mpix/s reprojected (configs[4] stream, {args.order})",
+            "value": out_mpix * steps / (total_ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": steps,
+            "warmup": max(1, min(args.warmup, 3)), "ms_per_step": total_ms / steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "exposures_per_s": n_exp * steps / (total_ms * 1e-3),
+            "config": {"workload": f"configs[4]: {n_exp} x 2048^2 TAN-SIP3 -> 4096^2 mosaic, {args.order}, 32 exposures per call",
+                       "distinct_images": m_img, "generation_s": gen_s,
+                       "l2": "a batch reads 537 MB and writes 2147 MB > 126 MB L2 (no flush needed)", "tiles_last_batch": stats},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+            "gpu_launches": int(stats["kernels"]) * ((n_exp + batch - 1) // batch) * steps, "clocks": sampler.summary()}
     print(json.dumps(line))
     return 0
 
@@ -282,7 +500,18 @@ def main():
     ap.add_argument("--mode", default="reproject", choices=["reproject", "stack", "probes"],
                     help="stack: the fused reproject-and-stack entry point (SURVEY.md §8(f) f1) on the same "
                          "workload; probes: the register-only instruction-rate probes; neither is the headline metric")
+    ap.add_argument("--config", type=int, default=2, choices=[0, 1, 2, 3, 4],
+                    help="BASELINE.json config index; 2 (default) is the headline, the others print the same contract line")
+    ap.add_argument("--order", default="bilinear", choices=list(ORDERS), help="interpolation order of --config 0/1/3/4")
+    ap.add_argument("--src-nx", type=int, default=0,
+                    help="--config 0/1/3: crop the source to this width (e.g. one that is not a multiple of 4: "
+                         "rows TMA cannot describe, gathers go through L1 instead of a staged box)")
+    ap.add_argument("--c4-exposures", type=int, default=1024)
+    ap.add_argument("--c4-images", type=int, default=128, help="distinct images of the configs[4] stream (1024 = all)")
     args = ap.parse_args()
+    if args.config != 2 and args.impl == "ours" and args.mode == "reproject":
+        args.warmup = max(args.warmup, 3)
+        return run_config(args)
     if args.mode == "probes":
         # register-only instruction-rate probes (dfr_probe_rates): the measured ALU-side denominators
         import torch

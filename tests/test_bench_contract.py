@@ -59,6 +59,31 @@ def test_stack_line():
     assert 20.0 < d["config"]["depth_mean"] <= 32.0
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg,extra", [("0", ("--order", "bicubic")), ("1", ()), ("0", ("--src-nx", "254")),
+                                       ("4", ("--c4-exposures", "64", "--c4-images", "32"))])
+def test_other_configs_print_the_same_contract_line(cfg, extra):
+    """bench.py --config {0,1,3,4}: the configs the headline does not time, through the same keys
+    (C3 is left to the profiles/ run: its oracle leg alone takes a while)."""
+    torch = pytest.importorskip("torch")
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    d = run("--config", cfg, *extra, "--steps", "3", "--warmup", "3", "--e2e-steps", "1", "--load-seconds", "0.2")
+    assert BASE_KEYS | {"clocks"} <= set(d) and d["config"]["workload"].startswith(f"configs[{cfg}]")
+    r = d["roofline"]
+    assert r["kernel"].startswith("tiled_reproject_kernel") and 0 < r["frac"] < 1.2 and r["kernel_ms"] > 0
+    assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9 and r["source_pixels_touched"] > 0
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] > 0
+    e = d["e2e"]
+    assert 0 < e["value"] < d["value"] and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0
+    if cfg != "4":
+        assert e["max_diff_vs_device_path_dr"] <= 1e-5 and e["mask_diff_vs_device_path"] <= 8
+        assert ("<3," if "bicubic" in extra else "<1,") in r["kernel"]
+        assert (",0,0>" in r["kernel"]) == ("--src-nx" in extra)            # 254 columns: not staged
+    else:
+        assert d["exposures_per_s"] > 0 and e["exposures_per_s"] > 0 and d["config"]["distinct_images"] == 32
+
+
 def test_reference_arm_line():
     """The oracle arm runs on the host cores (no GPU): a bounded sample per step."""
     d = run("--impl", "reference", "--steps", "1", "--warmup", "0", timeout=900)
