@@ -318,6 +318,10 @@ def run_config(args):
             ms.append(a.elapsed_time(b))
         return ms, kern
 
+    if args.profile_runs:                      # the command ncu captures are taken from: plain launches, nothing else
+        flushed_steps(args.profile_runs)
+        print(json.dumps({"profile_runs": args.profile_runs, "config": cfg, "order": args.order, "tiles": P.dfr_last_stats()}))
+        return 0
     flushed_steps(args.warmup)
     stats = P.dfr_last_stats()
     sampler = ClockSampler(0)
@@ -435,8 +439,8 @@ def run_config4(args, torch, P, order, hbm, which):
     total_ms = ev[0].elapsed_time(ev[-1])
     P.dfr_profile_enable(True)
     kern = []
-    for b in range(4):
-        P.dfr_reproject(dsrc[:batch], ws_b[b], tw, (ony, onx), order, out=dout)
+    for b in range(min(4, len(ws_b))):
+        P.dfr_reproject(dsrc[:len(ws_b[b])], ws_b[b], tw, (ony, onx), order, out=dout[:len(ws_b[b])])
         kern.append(P.dfr_profile_last())
     P.dfr_profile_enable(False)
     sampler.stop()
@@ -506,6 +510,9 @@ def main():
     ap.add_argument("--src-nx", type=int, default=0,
                     help="--config 0/1/3: crop the source to this width (e.g. one that is not a multiple of 4: "
                          "rows TMA cannot describe, gathers go through L1 instead of a staged box)")
+    ap.add_argument("--profile-runs", type=int, default=0,
+                    help="--config 0/1/3: N plain launches (L2 flushed before each) and nothing else — no timing, no oracle: "
+                         "the command the ncu captures under profiles/ are taken from")
     ap.add_argument("--c4-exposures", type=int, default=1024)
     ap.add_argument("--c4-images", type=int, default=128, help="distinct images of the configs[4] stream (1024 = all)")
     args = ap.parse_args()
