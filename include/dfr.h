@@ -329,20 +329,6 @@ int dfr_profile_last(float ms[2]);
  * idle pipeline on it, and trims the scratch pool. Safe to call at any time between calls. */
 int dfr_release(void);
 
-/* Register-only instruction-rate probes (the ALU side of the roofline wants
- * MEASURED denominators). Runs one short kernel per class on the current device, every SM
- * loaded with 32 warps of independent chains, and writes into out[k] (HOST, n >=
- * DFR_PROBE_COUNT entries, k = DFR_PROBE_*) the thread-level INSTRUCTIONS retired per clock
- * per SM; a packed FFMA2 counts as one instruction (two fp32 FMAs). The three mixed classes
- * interleave two instruction kinds 1:1 and report their combined instruction rate: a rate
- * above either kind alone means the two do not share a pipe. Synchronous; ~50 ms. */
-enum { DFR_PROBE_FFMA = 0, DFR_PROBE_FFMA2 = 1, DFR_PROBE_FADD2_RM = 2, DFR_PROBE_DFMA = 3,
-       DFR_PROBE_IMAD = 4, DFR_PROBE_LOP3 = 5, DFR_PROBE_LDS = 6,
-       DFR_PROBE_FFMA_FFMA2 = 7, DFR_PROBE_FFMA2_IMAD = 8, DFR_PROBE_FFMA2_LOP3 = 9,
-       DFR_PROBE_FFMA_3REG = 10, DFR_PROBE_FFMA2_3REG = 11,   /* three distinct, changing register operands */
-       DFR_PROBE_COUNT = 12 };
-int dfr_probe_rates(double *out, int32_t n);
-
 const char *dfr_strerror(int code);
 const char *dfr_last_error(void);
 int dfr_version(void);           /* 10000*major + 100*minor + patch */

@@ -25,7 +25,7 @@ EXPORTS = ["dfr_reproject", "dfr_reproject_edge", "dfr_reproject_ex", "dfr_repro
            "dfr_reproject_host_multi", "dfr_reproject_stack", "dfr_shard_range", "dfr_release",
            "dfr_stack_finalize", "dfr_stack_host", "dfr_stack_host_multi", "dfr_pix2world",
            "dfr_world2pix", "dfr_src_coords", "dfr_wcs_set_pc_cdelt", "dfr_wcs_fit_inverse_sip", "dfr_last_stats",
-           "dfr_profile_enable", "dfr_profile_last", "dfr_probe_rates",
+           "dfr_profile_enable", "dfr_profile_last",
            "dfr_strerror", "dfr_last_error", "dfr_version"]
 
 
@@ -80,7 +80,6 @@ def lib():
         L.dfr_last_stats.argtypes = [C.POINTER(C.c_int64)]
         L.dfr_profile_enable.argtypes = [C.c_int]
         L.dfr_profile_last.argtypes = [C.POINTER(C.c_float)]
-        L.dfr_probe_rates.argtypes = [C.POINTER(C.c_double), i32]
         L.dfr_strerror.argtypes = [C.c_int]
         L.dfr_strerror.restype = C.c_char_p
         L.dfr_last_error.restype = C.c_char_p
@@ -408,10 +407,31 @@ PROBE_NAMES = ["FFMA", "FFMA2", "FADD2.RM", "DFMA", "IMAD", "LOP3", "LDS", "FFMA
                "FFMA 3-reg", "FFMA2 3-reg"]
 
 
+_probe_lib = None
+
+
+def probe_lib():
+    """libdfr_probe.so: the register-only instruction-rate probes, a measurement tool kept out of
+    libdfr and of include/dfr.h (csrc/probe/dfr_probe.cu). Only `bench.py --mode probes` uses it."""
+    global _probe_lib
+    if _probe_lib is None:
+        so = os.path.join(_PKG, "libdfr_probe.so")
+        if not os.path.exists(so):
+            raise ImportError(f"{so} missing: run `python -m paper_2505_03932_b200.build`")
+        L = C.CDLL(so)
+        L.dfr_probe_rates.argtypes = [C.POINTER(C.c_double), C.c_int]
+        L.dfr_probe_error.restype = C.c_char_p
+        _probe_lib = L
+    return _probe_lib
+
+
 def dfr_probe_rates() -> dict:
-    """dfr_probe_rates: thread-level instructions per clock per SM for each probe class."""
+    """Thread-level instructions per clock per SM for each probe class (libdfr_probe.so)."""
     out = (C.c_double * len(PROBE_NAMES))()
-    _check(lib().dfr_probe_rates(out, len(PROBE_NAMES)))
+    L = probe_lib()
+    rc = L.dfr_probe_rates(out, len(PROBE_NAMES))
+    if rc != 0:
+        raise DfrError(rc, L.dfr_probe_error().decode())
     return dict(zip(PROBE_NAMES, [float(v) for v in out]))
 
 

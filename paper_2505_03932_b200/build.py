@@ -56,6 +56,18 @@ def build_checked(selftest: bool = False, verbose: bool = False) -> str:
     return SO_CHECKED
 
 
+# The instruction-rate probes (csrc/probe/): a measurement tool, not part of libdfr or its ABI; its own
+# library, loaded only by `bench.py --mode probes`.
+SO_PROBE = os.path.join(PKG, "libdfr_probe.so")
+
+
+def build_probe(force: bool = False, verbose: bool = False) -> str:
+    srcs = sorted(glob.glob(os.path.join(PKG, "csrc", "probe", "*.cu")))
+    if force or not os.path.exists(SO_PROBE) or os.path.getmtime(SO_PROBE) < max(os.path.getmtime(s) for s in srcs):
+        _run([NVCC, *ARCH, "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC", "-shared", "-o", SO_PROBE, *srcs], verbose)
+    return SO_PROBE
+
+
 def _run(cmd, verbose):
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:
@@ -77,6 +89,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         os.remove(stray)
     if stale or not os.path.exists(SO) or os.path.getmtime(SO) < max(os.path.getmtime(o) for o in objs):
         _run(link_command(), verbose)
+    build_probe(force, verbose)
     return SO
 
 

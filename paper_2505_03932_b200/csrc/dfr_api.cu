@@ -887,14 +887,6 @@ int dfr_release(void)
     return DFR_OK;
 }
 
-int dfr_probe_rates(double *out, int32_t n)
-{
-    if (!out) { set_error("NULL pointer"); return DFR_ERR_NULL; }
-    if (n < DFR_PROBE_COUNT) { set_error("out needs %d entries", (int)DFR_PROBE_COUNT); return DFR_ERR_SHAPE; }
-    const cudaError_t err = probe_rates(out);
-    return err == cudaSuccess ? DFR_OK : cuda_fail(err, "probe kernels");
-}
-
 const char *dfr_strerror(int code)
 {
     switch (code) {

@@ -71,7 +71,4 @@ cudaError_t launch_pix2world(const SkyDev *w, const double *x, const double *y, 
 cudaError_t launch_world2pix(const SkyDev *w, const double *ra, const double *dec, int64_t npts,
                              double *x, double *y, cudaStream_t st);
 
-// register-only instruction-rate probes (dfr_probe.cu)
-cudaError_t probe_rates(double *out);
-
 }  // namespace dfr

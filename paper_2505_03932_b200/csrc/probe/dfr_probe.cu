@@ -1,4 +1,6 @@
-// dfr_probe.cu — register-only instruction-rate probes (dfr_probe_rates, include/dfr.h).
+// dfr_probe.cu — register-only instruction-rate probes. NOT part of libdfr or of include/dfr.h: a
+// measurement tool built into its own libdfr_probe.so, which only `bench.py --mode probes` loads
+// (through paper_2505_03932_b200.dfr_probe_rates).
 //
 // The roofline of SURVEY.md §8(d) has an ALU side whose denominator must be MEASURED on the
 // device ("register-only FMA micro-benchmark and the actual SM clock recorded"). These
@@ -10,7 +12,17 @@
 #include <algorithm>
 #include <vector>
 
-#include "dfr_internal.h"
+#include <cuda_runtime.h>
+
+// Probe classes: out[k] of dfr_probe_rates receives the thread-level INSTRUCTIONS retired per clock
+// per SM (every SM loaded with 32 warps of independent chains); a packed FFMA2 counts as one
+// instruction (two fp32 FMAs). The three mixed classes interleave two instruction kinds 1:1 and
+// report their combined rate: a rate above either kind alone means the two do not share a pipe.
+enum { DFR_PROBE_FFMA = 0, DFR_PROBE_FFMA2 = 1, DFR_PROBE_FADD2_RM = 2, DFR_PROBE_DFMA = 3,
+       DFR_PROBE_IMAD = 4, DFR_PROBE_LOP3 = 5, DFR_PROBE_LDS = 6,
+       DFR_PROBE_FFMA_FFMA2 = 7, DFR_PROBE_FFMA2_IMAD = 8, DFR_PROBE_FFMA2_LOP3 = 9,
+       DFR_PROBE_FFMA_3REG = 10, DFR_PROBE_FFMA2_3REG = 11,   /* three distinct, changing register operands */
+       DFR_PROBE_COUNT = 12 };
 
 namespace dfr {
 
@@ -177,3 +189,15 @@ cudaError_t probe_rates(double *out /* [DFR_PROBE_COUNT] thread-instructions per
 }
 
 }  // namespace dfr
+
+// HOST out[n], n >= DFR_PROBE_COUNT. Synchronous, ~50 ms on the current device. Returns 0, -1 (NULL),
+// -2 (n too small) or -8 (CUDA failure: dfr_probe_error() has the text).
+static thread_local cudaError_t g_probe_err = cudaSuccess;
+extern "C" int dfr_probe_rates(double *out, int n)
+{
+    if (!out) return -1;
+    if (n < DFR_PROBE_COUNT) return -2;
+    g_probe_err = dfr::probe_rates(out);
+    return g_probe_err == cudaSuccess ? 0 : -8;
+}
+extern "C" const char *dfr_probe_error(void) { return cudaGetErrorString(g_probe_err); }

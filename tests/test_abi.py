@@ -146,7 +146,10 @@ def test_footprint_and_multi_device_validation_without_gpu(P):
     assert L.dfr_stack_host_multi(src, 2, 8, 8, arr, C.byref(good), 8, 8, 2, None, out, fp, 2, devs, 2) == -3
     assert L.dfr_stack_host_multi(src, 2, 8, 8, arr, C.byref(good), 8, 8, 1, (C.c_float * 2)(1.0, float("nan")),
                                   out, fp, 2, devs, 2) == -9
-    assert L.dfr_probe_rates(None, 12) == -1 and L.dfr_probe_rates((C.c_double * 4)(), 4) == -2
+    # the instruction-rate probes live in their own library, outside the product ABI
+    assert not hasattr(L, "dfr_probe_rates")
+    LP = P.probe_lib()
+    assert LP.dfr_probe_rates(None, 12) == -1 and LP.dfr_probe_rates((C.c_double * 4)(), 4) == -2
 
 
 def test_shard_range_is_a_partition_and_matches_the_python_rule(P):
