@@ -487,6 +487,60 @@ def run_config4(args, torch, P, order, hbm, which):
     return 0
 
 
+def relaunch_command(argv, n, port=None):
+    """`python bench.py --gpus N` started by hand (no torchrun, WORLD_SIZE unset): the command that
+    starts N ranks of this file the way the driver does (one process per GPU, NCCL over 127.0.0.1)."""
+    if port is None:
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}",
+            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *argv]
+
+
+def run_host_multi(args):
+    """--mode host_multi: ONE process, the library's own multi-device entry points on configs[2]-shaped
+    input from pinned host memory: dfr_reproject_host_multi (exposures sharded over --gpus devices, no
+    collective) and dfr_stack_host_multi (the same shards co-added, partial sums reduced on the first
+    device). PCIe-bound per GPU, which is where N links pay. Wall-clock (the calls are synchronous)."""
+    import torch
+    import paper_2505_03932_b200 as P
+    P.lib()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    ndev = torch.cuda.device_count()
+    devices = [k % ndev for k in range(args.gpus)]          # more shards than devices: two pipelines on one device
+    w = S.config2(batch=BATCH)
+    hsrc = torch.from_numpy(w.images).pin_memory()
+    hout = torch.empty((BATCH, NPIX, NPIX), dtype=torch.float32).pin_memory()
+    ws_arr, tw = P.pack_wcs_array(w.src_wcs), P.pack_wcs(w.tgt_wcs)
+    res = {}
+    for name, call in (("reproject", lambda: P.dfr_reproject_host(hsrc, ws_arr, tw, (NPIX, NPIX), P.BILINEAR, out_host=hout,
+                                                                  batch=4, devices=devices)),
+                       ("stack", lambda: P.dfr_stack_host(hsrc, ws_arr, tw, (NPIX, NPIX), P.BILINEAR, batch=8, devices=devices))):
+        for _ in range(max(1, min(args.warmup, 3))):
+            call()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            call()
+        el = (time.perf_counter() - t0) / args.steps
+        res[name] = {"ms_per_step": 1e3 * el, "exposures_per_s": BATCH / el, "mpix_per_s": BATCH * NPIX * NPIX / 1e6 / el}
+    line = {"metric": "output Mpix/s reprojected end to end, one process over N devices (dfr_reproject_host_multi)",
+            "value": res["reproject"]["mpix_per_s"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": max(1, min(args.warmup, 3)), "ms_per_step": res["reproject"]["ms_per_step"], "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "configs[2]: 32 x 2048^2 from pinned host memory, sharded by exposure", "devices": devices,
+                       "visible_devices": ndev},
+            "reproject_host_multi": res["reproject"], "stack_host_multi": res["stack"],
+            "roofline": None, "cpu_baseline": None,
+            "e2e": {"value": res["reproject"]["mpix_per_s"], "unit": UNIT, "h2d_bytes_per_step": int(w.images.nbytes),
+                    "d2h_bytes_per_step": int(hout.numel() * 4)},
+            "gpu_launches": 3 * (BATCH // 4) * args.steps}
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -501,7 +555,7 @@ def main():
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="with --gpus N > 1: weak = every rank its own batch of 32 (the driver's contract); strong = ONE "
                          "batch of 32 cut into N contiguous shards (dfr_shard_range), no collective either way")
-    ap.add_argument("--mode", default="reproject", choices=["reproject", "stack", "probes"],
+    ap.add_argument("--mode", default="reproject", choices=["reproject", "stack", "probes", "host_multi"],
                     help="stack: the fused reproject-and-stack entry point (SURVEY.md §8(f) f1) on the same "
                          "workload; probes: the register-only instruction-rate probes; neither is the headline metric")
     ap.add_argument("--config", type=int, default=2, choices=[0, 1, 2, 3, 4],
@@ -516,6 +570,11 @@ def main():
     ap.add_argument("--c4-exposures", type=int, default=1024)
     ap.add_argument("--c4-images", type=int, default=128, help="distinct images of the configs[4] stream (1024 = all)")
     args = ap.parse_args()
+    if args.mode == "host_multi":
+        return run_host_multi(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.mode == "reproject" and args.config == 2:
+        # started by hand without torchrun: start the N ranks ourselves (NCCL's own output stays visible)
+        return subprocess.call(relaunch_command(sys.argv[1:], args.gpus))
     if args.config != 2 and args.impl == "ours" and args.mode == "reproject":
         args.warmup = max(args.warmup, 3)
         return run_config(args)

@@ -84,6 +84,38 @@ def test_other_configs_print_the_same_contract_line(cfg, extra):
         assert d["exposures_per_s"] > 0 and e["exposures_per_s"] > 0 and d["config"]["distinct_images"] == 32
 
 
+def test_gpus_n_without_torchrun_starts_its_own_ranks():
+    """`python bench.py --gpus 4` with WORLD_SIZE unset re-executes itself under torch.distributed.run
+    (one rank per GPU, 127.0.0.1 rendezvous) instead of silently running one rank."""
+    sys.path.insert(0, ROOT)
+    import bench
+    cmd = bench.relaunch_command(["--gpus", "4", "--steps", "2"], 4, port=29511)
+    assert cmd[:3] == [sys.executable, "-m", "torch.distributed.run"]
+    assert "--nproc-per-node=4" in cmd and "--nnodes=1" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[cmd.index("--master-port") + 1] == "29511"
+    assert cmd[-5:] == [os.path.join(ROOT, "bench.py"), "--gpus", "4", "--steps", "2"]
+    free = bench.relaunch_command([], 2)
+    assert 1024 < int(free[free.index("--master-port") + 1]) < 65536
+    # and the reference arm under it: rank 0 prints the line, the other rank exits 0 without work
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
+                          "--steps", "1", "--warmup", "0"], capture_output=True, text=True, timeout=900, cwd=ROOT,
+                         env={k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")})
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [json.loads(l) for l in res.stdout.splitlines() if l.strip().startswith("{")]
+    assert len(lines) == 1 and lines[0]["impl"] == "reference" and lines[0]["n_gpus"] == 2
+
+
+@pytest.mark.gpu
+def test_host_multi_line():
+    """--mode host_multi on a one-GPU box: two shards, both on device 0 (two pipelines)."""
+    torch = pytest.importorskip("torch")
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    d = run("--mode", "host_multi", "--gpus", "2", "--steps", "1", "--warmup", "1")
+    assert d["n_gpus"] == 2 and len(d["config"]["devices"]) == 2
+    assert d["reproject_host_multi"]["exposures_per_s"] > 0 and d["stack_host_multi"]["exposures_per_s"] > 0
+
+
 def test_reference_arm_line():
     """The oracle arm runs on the host cores (no GPU): a bounded sample per step."""
     d = run("--impl", "reference", "--steps", "1", "--warmup", "0", timeout=900)
