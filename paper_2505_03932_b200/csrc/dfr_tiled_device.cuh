@@ -37,6 +37,39 @@ constexpr double kCentre = 0.5 * (TS - 1);    // 15.5: tile centre relative to i
 // ---------------------------------------------------------------------------------
 // pieces of the main kernel
 // ---------------------------------------------------------------------------------
+// The source coordinate of a FAST tile, ONE definition for every kernel that needs it (the
+// reprojection and stacking kernels, the footprint pass, and dfr_src_coords, which SURVEY.md §8(b)
+// requires to run "the same __device__ function as dfr_reproject"):
+//   x(lane, r) = ix0 + sum_q X[q] dj^q,   dj = r - kCentre,   X[q] = sum_p cx[q][p] di^p,   di = lane - kCentre
+// (and y likewise), all in fp32 with the fused multiply-adds in exactly this order.
+// column_polys: the per-lane polynomials in dj from the tile record's 2 x 16 coefficients.
+__device__ __forceinline__ void column_polys(const TileRec *__restrict__ rec, int lane, float X[4], float Y[4])
+{
+    const float di = (float)lane - (float)kCentre;
+    const float4 *c4 = reinterpret_cast<const float4 *>(rec->cx);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const float4 a = __ldg(c4 + q), b = __ldg(c4 + 4 + q);
+        X[q] = fmaf(fmaf(fmaf(a.w, di, a.z), di, a.y), di, a.x);
+        Y[q] = fmaf(fmaf(fmaf(b.w, di, b.z), di, b.y), di, b.x);
+    }
+}
+// truncate_degree: the setup kernel found that the dj^3 (dj^2) terms cannot move a coordinate of this
+// tile by 2.5e-7 px (TileRec::deg): they are dropped, on every path alike.
+__device__ __forceinline__ void truncate_degree(int deg, float X[4], float Y[4])
+{
+    if (deg < 3) { X[3] = 0.0f; Y[3] = 0.0f; }
+    if (deg < 2) { X[2] = 0.0f; Y[2] = 0.0f; }
+}
+// tile_coord: the coordinate (relative to ix0, iy0) in row r of the tile, scalar form (the packed
+// interior loop of warp_tile evaluates the same Horner chain two rows at a time).
+__device__ __forceinline__ void tile_coord(const float X[4], const float Y[4], int r, float &xl, float &yl)
+{
+    const float dj = (float)r - (float)kCentre;
+    xl = fmaf(fmaf(fmaf(X[3], dj, X[2]), dj, X[1]), dj, X[0]);
+    yl = fmaf(fmaf(fmaf(Y[3], dj, Y[2]), dj, Y[1]), dj, Y[0]);
+}
+
 constexpr float kMagic = 12582912.0f;              // 1.5 * 2^23: ulp 1 on [2^23, 2^24)
 constexpr int kMagicBits = 0x4B400000;
 
@@ -449,8 +482,7 @@ __device__ __forceinline__ void warp_tile(const TiledParams &P, const TargetDev 
         G.gbase = img + ((long long)(Aly - tlo) * P.snx + (Alx - tlo));
     }
 
-    if (deg < 3) { X[3] = 0.0f; Y[3] = 0.0f; }                  // same polynomial on every path
-    if (deg < 2) { X[2] = 0.0f; Y[2] = 0.0f; }
+    truncate_degree(deg, X, Y);                                 // same polynomial on every path
     constexpr int U = 4;                      // rows in flight per thread
     float dj = -(float)kCentre;
     int r = 0;

@@ -88,16 +88,7 @@ tiled_reproject_kernel(const __grid_constant__ TiledParams P, const __grid_const
     }
     // per-lane column polynomials in dj (FAST tiles; harmless otherwise)
     float X[4], Y[4];
-    {
-        const float di = (float)lane - (float)kCentre;
-        const float4 *c4 = reinterpret_cast<const float4 *>(rec->cx);
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const float4 a = __ldg(c4 + q), b = __ldg(c4 + 4 + q);
-            X[q] = fmaf(fmaf(fmaf(a.w, di, a.z), di, a.y), di, a.x);
-            Y[q] = fmaf(fmaf(fmaf(b.w, di, b.z), di, b.y), di, b.x);
-        }
-    }
+    column_polys(rec, lane, X, Y);
     if (STAGE) {
         __syncthreads();                // the mbarrier is initialised before anybody polls it
         if (has_box) {
@@ -162,20 +153,11 @@ tiled_coords_kernel(const __grid_constant__ TiledParams P, const __grid_constant
         return;
     }
     float X[4], Y[4];
-    const float di = (float)lane - (float)kCentre;
-    const float4 *c4 = reinterpret_cast<const float4 *>(rec->cx);
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        const float4 a = __ldg(c4 + q), b = __ldg(c4 + 4 + q);
-        X[q] = fmaf(fmaf(fmaf(a.w, di, a.z), di, a.y), di, a.x);
-        Y[q] = fmaf(fmaf(fmaf(b.w, di, b.z), di, b.y), di, b.x);
-    }
-    if (deg < 3) { X[3] = 0.0f; Y[3] = 0.0f; }                  // as the main kernel does
-    if (deg < 2) { X[2] = 0.0f; Y[2] = 0.0f; }
+    column_polys(rec, lane, X, Y);                              // the main kernel's own functions
+    truncate_degree(deg, X, Y);
     for (int r = 0; r < rows; ++r) {
-        const float dj = (float)r - (float)kCentre;
-        const float xl = fmaf(fmaf(fmaf(X[3], dj, X[2]), dj, X[1]), dj, X[0]);
-        const float yl = fmaf(fmaf(fmaf(Y[3], dj, Y[2]), dj, Y[1]), dj, Y[0]);
+        float xl, yl;
+        tile_coord(X, Y, r, xl, yl);
         xo[o + (size_t)r * P.onx] = (double)ix0 + (double)xl;
         yo[o + (size_t)r * P.onx] = (double)iy0 + (double)yl;
     }
@@ -215,20 +197,11 @@ tiled_footprint_kernel(const __grid_constant__ TiledParams P, const __grid_const
         return;
     }
     float X[4], Y[4];
-    const float di = (float)lane - (float)kCentre;
-    const float4 *c4 = reinterpret_cast<const float4 *>(rec->cx);
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        const float4 a = __ldg(c4 + q), b = __ldg(c4 + 4 + q);
-        X[q] = fmaf(fmaf(fmaf(a.w, di, a.z), di, a.y), di, a.x);
-        Y[q] = fmaf(fmaf(fmaf(b.w, di, b.z), di, b.y), di, b.x);
-    }
-    if (deg < 3) { X[3] = 0.0f; Y[3] = 0.0f; }                  // as the main kernel does
-    if (deg < 2) { X[2] = 0.0f; Y[2] = 0.0f; }
+    column_polys(rec, lane, X, Y);                              // the main kernel's own functions
+    truncate_degree(deg, X, Y);
     for (int r = 0; r < rows; ++r) {
-        const float dj = (float)r - (float)kCentre;
-        const float xl = fmaf(fmaf(fmaf(X[3], dj, X[2]), dj, X[1]), dj, X[0]);
-        const float yl = fmaf(fmaf(fmaf(Y[3], dj, Y[2]), dj, Y[1]), dj, Y[0]);
+        float xl, yl;
+        tile_coord(X, Y, r, xl, yl);
         o[(size_t)r * P.onx] = footprint_value((double)ix0 + (double)xl, (double)iy0 + (double)yl, P.sny, P.snx, order, edge);
     }
 }

@@ -224,16 +224,7 @@ tiled_stack_kernel(const __grid_constant__ TiledParams P, const __grid_constant_
             sink.begin_exposure(__ldg(S.weights + e));
             // per-lane column polynomials in dj, while the box is in flight
             float X[4], Y[4];
-            {
-                const float di = (float)lane - (float)kCentre;
-                const float4 *c4 = reinterpret_cast<const float4 *>(rec->cx);
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const float4 a = __ldg(c4 + q), b = __ldg(c4 + 4 + q);
-                    X[q] = fmaf(fmaf(fmaf(a.w, di, a.z), di, a.y), di, a.x);
-                    Y[q] = fmaf(fmaf(fmaf(b.w, di, b.z), di, b.y), di, b.x);
-                }
-            }
+            column_polys(rec, lane, X, Y);
             if (has_box) {
                 mbar_wait(bar, phase);
                 phase ^= 1u;
